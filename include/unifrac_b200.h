@@ -1,0 +1,139 @@
+/*
+ * unifrac_b200.h -- C ABI of libunifrac_b200.so: Striped/Hybrid UniFrac all-pairs distance on one
+ * NVIDIA B200 (sm_100a).  Plain C; callers need no CUDA headers.
+ *
+ * What it computes ("a distance matrix of size N x N where N is the number of
+ * samples"; section II: UniFrac from a phylogeny and a sparse sample x feature
+ * table, "for both unweighted and the weighted normalized versions", with "fp32 compute
+ * support"; formulas per BASELINE.json:5, readings Q1-Q3, Q9):
+ *
+ *   x_sv = 1 if sample s has any count on a tip below branch v, else 0
+ *   u_sv = (sum of s's counts on tips below v) / (sum of all of s's counts)
+ *   unweighted           d(a,b) = sum_v len_v*(x_av xor x_bv) / sum_v len_v*(x_av or x_bv)
+ *   weighted-normalized  d(a,b) = sum_v len_v*|u_av - u_bv|   / sum_v len_v*(u_av + u_bv)
+ *   sums over all non-root nodes v; a zero denominator gives d = 0.
+ *
+ * Every step (plan/validate, per-branch embedding, stripe accumulation, finalize) runs in the
+ * library's own CUDA kernels; there is no CPU fallback.
+ */
+#ifndef UNIFRAC_B200_H
+#define UNIFRAC_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum { UNIFRAC_UNWEIGHTED = 0, UNIFRAC_WEIGHTED_NORMALIZED = 1 } unifrac_variant_t;
+typedef enum { UNIFRAC_FP32 = 0, UNIFRAC_FP64 = 1 } unifrac_precision_t;
+
+typedef enum {
+    UNIFRAC_OK = 0,
+    UNIFRAC_ERR_INVALID_ARG = -1,   /* null pointer, bad enum, n_samples < 2, n_nodes < 2 ...          */
+    UNIFRAC_ERR_INVALID_TREE = -2,  /* not exactly one root, parent out of range, postorder not a
+                                       permutation with children before parent and root last,
+                                       negative / non-finite branch length                           */
+    UNIFRAC_ERR_INVALID_TABLE = -3, /* indptr not monotone from 0, column not a tip node id, columns
+                                       not strictly increasing within a row, negative count          */
+    UNIFRAC_ERR_EMPTY_SAMPLE = -4,  /* a sample whose counts sum to 0 (u would be 0/0)                */
+    UNIFRAC_ERR_WORKSPACE = -5,     /* the allocator returned NULL / device memory exhausted          */
+    UNIFRAC_ERR_CUDA = -6,          /* a CUDA runtime call failed (see unifrac_last_cuda_error)       */
+    UNIFRAC_ERR_UNSUPPORTED = -7    /* a sample total >= 2^32, or n_samples / n_nodes beyond limits   */
+} unifrac_status_t;
+
+/* flags (bit mask) */
+#define UNIFRAC_FLAG_LITERAL          1u  /* debug: accumulate BOTH pairwise sums exactly as BASELINE.json:5
+                                             words them (len*|u-v| and len*(u+v); len*xor and len*or) in a
+                                             plain one-thread-per-pair fp64 kernel.  Slow; small inputs.   */
+#define UNIFRAC_FLAG_TENSOR_GRAM      2u  /* unweighted + fp32 only: allow the tcgen05 int8 Gram path
+                                             (X^T diag(len) X with len in 24-bit fixed point)              */
+#define UNIFRAC_FLAG_SKIP_VALIDATION  4u  /* trust the inputs (tree/table checks are skipped)            */
+#define UNIFRAC_FLAG_ABSDIFF          8u  /* stripe kernel accumulates |u~_i - u~_j| over rows present in
+                                             EITHER tile (direct form) instead of min(u~_i,u~_j) over rows
+                                             present in BOTH (separable form, I2-I5)            */
+
+/* CSR table, rows = samples, columns = tip NODE ids (reading Q6). */
+typedef struct {
+    const int64_t *indptr;   /* [n_samples+1]  indptr[0] = 0, non-decreasing                          */
+    const int32_t *indices;  /* [nnz]          node id of a tip; strictly increasing within a row    */
+    const int32_t *counts;   /* [nnz]          >= 0 (0 = absent)                                      */
+} unifrac_csr_t;
+
+/* Device-memory allocator supplied by the caller (e.g. backed by torch.empty).  Must return a
+ * device pointer aligned to 256 bytes, or NULL.  Buffers are owned by the caller and must stay
+ * valid until the work unifrac_dm enqueued on `stream` has completed; the library never frees
+ * them.  If `alloc` is NULL the library uses cudaMallocAsync / cudaFreeAsync on `stream`. */
+typedef void *(*unifrac_alloc_fn)(size_t bytes, void *user);
+
+/*
+ * unifrac_dm -- fill the condensed N x N UniFrac distance matrix.
+ *
+ * All array arguments are DEVICE pointers, read-only, owned by the caller, not retained.
+ *   n_nodes       number of tree nodes (tips + internal + root), >= 2
+ *   tree_parent   [n_nodes] parent node id; exactly one entry is -1 (the root)
+ *   branch_len    [n_nodes] length of the edge v -> parent[v]; >= 0 and finite; root's ignored
+ *   postorder     [n_nodes] permutation of node ids, children before parent, root last
+ *   table         CSR counts, see unifrac_csr_t
+ *   n_samples     N >= 2
+ *   variant       unweighted / weighted-normalized
+ *   precision     UNIFRAC_FP32: embeddings, stripe accumulators and output are float (partial
+ *                 sums are folded into fp64 every 512 rows; per-sample sums and the final
+ *                 division are fp64);  UNIFRAC_FP64: everything double.
+ *   out_condensed device; N*(N-1)/2 float or double; row-major upper triangle (scipy
+ *                 squareform order): index(i,j) = i*(2N-i-1)/2 + (j-i-1), i < j.
+ *   alloc/user    workspace allocator (see above); may be NULL.
+ *   flags         UNIFRAC_FLAG_* mask
+ *   stream        cudaStream_t (NULL = default stream)
+ *
+ * Returns a unifrac_status_t.  Host-checkable errors return before anything is enqueued.  The
+ * plan step reads a few words back (one or more stream synchronisations), so data errors
+ * (tree / table / empty sample) are also returned synchronously and leave `out_condensed`
+ * untouched; after planning and embedding the stripe kernel is enqueued asynchronously and the
+ * call returns without waiting for it.  Never throws, never aborts.
+ */
+int unifrac_dm(int32_t n_nodes, const int32_t *tree_parent, const double *branch_len,
+               const int32_t *postorder, unifrac_csr_t table, int32_t n_samples,
+               unifrac_variant_t variant, unifrac_precision_t precision, void *out_condensed,
+               unifrac_alloc_fn alloc, void *alloc_user, uint32_t flags, void *stream);
+
+/*
+ * unifrac_dm_host -- same computation with HOST buffers (pageable or pinned).  The library
+ * allocates device memory itself (cudaMalloc), copies the inputs in, runs unifrac_dm on an
+ * internal stream, copies the condensed result out to `out_condensed_host`, frees everything
+ * and returns after completion (synchronous).  `nnz` is read from indptr[n_samples].
+ */
+int unifrac_dm_host(int32_t n_nodes, const int32_t *tree_parent, const double *branch_len,
+                    const int32_t *postorder, unifrac_csr_t table_host, int32_t n_samples,
+                    unifrac_variant_t variant, unifrac_precision_t precision,
+                    void *out_condensed_host, uint32_t flags);
+
+/* Statistics of the calling thread's last unifrac_dm call (work counters are exact, computed on
+ * the device from the per-branch sample counts; times are CUDA-event milliseconds, valid only
+ * if UNIFRAC_B200_TIMING=1 is set in the environment -- timing synchronises the stream). */
+typedef struct {
+    uint64_t branches_embedded;  /* B_emb = #{v : len_v > 0 and some sample present}                 */
+    uint64_t updates_dense;      /* W_dense = P * B_emb           (the metric's "pair x branch")      */
+    uint64_t updates_union;      /* W_union = sum_v [C(N,2) - C(N-n_v,2)]                             */
+    uint64_t updates_inter;      /* W_inter = sum_v C(n_v,2)                                          */
+    uint64_t updates_executed;   /* (pair, row) updates the stripe kernel actually executed           */
+    uint64_t rows_staged;        /* rows the producer staged into shared memory, over all tile pairs  */
+    uint64_t embed_rows;         /* sum over sample tiles of non-empty rows (compact embedding rows)  */
+    uint64_t workspace_bytes;    /* device bytes requested from the allocator                         */
+    uint32_t n_tile_pairs;       /* 128x128 tile pairs in the upper triangle                          */
+    uint32_t n_levels;           /* tree depth levels                                                 */
+    uint32_t stripe_launches;    /* stripe-kernel launches in this call                               */
+    uint32_t kernel_launches;    /* all kernel launches in this call                                  */
+    float ms_plan, ms_embed, ms_stripe, ms_total;
+} unifrac_stats_t;
+int unifrac_last_stats(unifrac_stats_t *out);
+
+const char *unifrac_status_string(int status);
+const char *unifrac_last_cuda_error(void);   /* text of the last CUDA error seen by this thread  */
+int unifrac_abi_version(void);               /* 1                                                */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* UNIFRAC_B200_H */

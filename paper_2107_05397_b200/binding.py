@@ -1,0 +1,170 @@
+"""Thin ctypes binding of include/unifrac_b200.h -- same names, argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels; PyTorch is used here only for device
+memory (the workspace allocator handed to the library is backed by ``torch.empty``) and for the
+stream.  There is no CPU fallback: if the library cannot be loaded, ``load()`` raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+
+from . import build as _build
+
+UNWEIGHTED, WEIGHTED_NORMALIZED = 0, 1
+FP32, FP64 = 0, 1
+FLAG_LITERAL, FLAG_TENSOR_GRAM, FLAG_SKIP_VALIDATION, FLAG_ABSDIFF = 1, 2, 4, 8
+
+OK = 0
+ERR_INVALID_ARG, ERR_INVALID_TREE, ERR_INVALID_TABLE, ERR_EMPTY_SAMPLE = -1, -2, -3, -4
+ERR_WORKSPACE, ERR_CUDA, ERR_UNSUPPORTED = -5, -6, -7
+
+EXPORTS = ("unifrac_dm", "unifrac_dm_host", "unifrac_last_stats", "unifrac_status_string",
+           "unifrac_last_cuda_error", "unifrac_abi_version")
+
+
+class CSR(C.Structure):
+    _fields_ = [("indptr", C.c_void_p), ("indices", C.c_void_p), ("counts", C.c_void_p)]
+
+
+class Stats(C.Structure):
+    _fields_ = [("branches_embedded", C.c_uint64), ("updates_dense", C.c_uint64), ("updates_union", C.c_uint64),
+                ("updates_inter", C.c_uint64), ("updates_executed", C.c_uint64), ("rows_staged", C.c_uint64),
+                ("embed_rows", C.c_uint64), ("workspace_bytes", C.c_uint64), ("n_tile_pairs", C.c_uint32),
+                ("n_levels", C.c_uint32), ("stripe_launches", C.c_uint32), ("kernel_launches", C.c_uint32),
+                ("ms_plan", C.c_float), ("ms_embed", C.c_float), ("ms_stripe", C.c_float), ("ms_total", C.c_float)]
+
+
+ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
+
+
+class UnifracError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"unifrac_b200 status {status}: {msg}")
+        self.status = status
+
+
+_lib = None
+
+
+def load(build_if_missing: bool = True) -> C.CDLL:
+    """dlopen libunifrac_b200.so (built in-tree by build.py).  Raises if it cannot be had."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if not os.path.exists(path) or (build_if_missing and _build.needs_build()):
+        if not build_if_missing:
+            raise FileNotFoundError(path)
+        try:
+            _build.build()
+        except Exception:
+            if not os.path.exists(path):
+                raise
+    lib = C.CDLL(path)
+    lib.unifrac_dm.restype = C.c_int
+    lib.unifrac_dm.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, CSR, C.c_int32, C.c_int, C.c_int,
+                               C.c_void_p, ALLOC_FN, C.c_void_p, C.c_uint32, C.c_void_p]
+    lib.unifrac_dm_host.restype = C.c_int
+    lib.unifrac_dm_host.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, CSR, C.c_int32, C.c_int, C.c_int,
+                                    C.c_void_p, C.c_uint32]
+    lib.unifrac_last_stats.restype = C.c_int
+    lib.unifrac_last_stats.argtypes = [C.POINTER(Stats)]
+    lib.unifrac_status_string.restype = C.c_char_p
+    lib.unifrac_status_string.argtypes = [C.c_int]
+    lib.unifrac_last_cuda_error.restype = C.c_char_p
+    lib.unifrac_abi_version.restype = C.c_int
+    _lib = lib
+    return lib
+
+
+def _check(lib, rc: int):
+    if rc != 0:
+        msg = lib.unifrac_status_string(rc).decode()
+        if rc == ERR_CUDA:
+            msg += ": " + lib.unifrac_last_cuda_error().decode()
+        raise UnifracError(rc, msg)
+
+
+def unifrac_dm(tree_parent, branch_len, postorder, indptr, indices, counts, n_samples: int, variant: int,
+               precision: int, out=None, flags: int = 0, stream=None):
+    """Device entry point.  All inputs are CUDA torch tensors (int32 / float64 / int32 / int64 / int32 /
+    int32); returns the condensed matrix as a CUDA tensor (float32 or float64).  Asynchronous on
+    `stream` (default: torch's current stream) after the plan/embedding steps."""
+    import torch
+    lib = load()
+    dev = tree_parent.device
+    assert dev.type == "cuda", "unifrac_dm takes device tensors; use unifrac_dm_host for host arrays"
+    for t, dt in ((tree_parent, torch.int32), (branch_len, torch.float64), (postorder, torch.int32),
+                  (indptr, torch.int64), (indices, torch.int32), (counts, torch.int32)):
+        assert t.dtype == dt and t.is_contiguous() and t.device == dev
+    n = int(n_samples)
+    if out is None:
+        out = torch.empty(n * (n - 1) // 2, dtype=torch.float32 if precision == FP32 else torch.float64, device=dev)
+    held = []
+
+    def _alloc(nbytes, _user):
+        try:
+            t = torch.empty(int(nbytes), dtype=torch.uint8, device=dev)
+        except Exception:
+            return None
+        held.append(t)
+        return t.data_ptr()
+
+    cb = ALLOC_FN(_alloc)
+    with torch.cuda.device(dev):
+        s = stream if stream is not None else torch.cuda.current_stream(dev)
+        with torch.cuda.stream(s):
+            rc = lib.unifrac_dm(int(tree_parent.shape[0]), tree_parent.data_ptr(), branch_len.data_ptr(),
+                                postorder.data_ptr(), CSR(indptr.data_ptr(), indices.data_ptr(), counts.data_ptr()),
+                                n, int(variant), int(precision), out.data_ptr(), cb, None, int(flags),
+                                C.c_void_p(s.cuda_stream))
+    # workspace tensors were allocated under `s`; dropping them here is stream-ordered safe
+    del held
+    _check(lib, rc)
+    return out
+
+
+def unifrac_dm_host(tree_parent, branch_len, postorder, indptr, indices, counts, n_samples: int, variant: int,
+                    precision: int, out: Optional[np.ndarray] = None, flags: int = 0) -> np.ndarray:
+    """Host entry point: numpy arrays in, numpy condensed matrix out (synchronous; the library does
+    the host<->device copies itself)."""
+    lib = load()
+    a = [np.ascontiguousarray(tree_parent, np.int32), np.ascontiguousarray(branch_len, np.float64),
+         np.ascontiguousarray(postorder, np.int32), np.ascontiguousarray(indptr, np.int64),
+         np.ascontiguousarray(indices, np.int32), np.ascontiguousarray(counts, np.int32)]
+    n = int(n_samples)
+    if out is None:
+        out = np.empty(n * (n - 1) // 2, dtype=np.float32 if precision == FP32 else np.float64)
+    rc = lib.unifrac_dm_host(int(a[0].shape[0]), a[0].ctypes.data, a[1].ctypes.data, a[2].ctypes.data,
+                             CSR(a[3].ctypes.data, a[4].ctypes.data, a[5].ctypes.data), n, int(variant),
+                             int(precision), out.ctypes.data, int(flags))
+    _check(lib, rc)
+    return out
+
+
+def unifrac_last_stats() -> dict:
+    lib = load()
+    s = Stats()
+    _check(lib, lib.unifrac_last_stats(C.byref(s)))
+    return {k: getattr(s, k) for k, _ in Stats._fields_}
+
+
+def unifrac_status_string(status: int) -> str:
+    return load().unifrac_status_string(int(status)).decode()
+
+
+def unifrac_abi_version() -> int:
+    return int(load().unifrac_abi_version())
+
+
+def to_device(problem, device="cuda:0"):
+    """Marshal a synth.Problem (numpy) into the six device tensors unifrac_dm takes."""
+    import torch
+    f = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(device)
+    return (f(problem.parent.astype(np.int32)), f(problem.branch_len.astype(np.float64)),
+            f(problem.postorder.astype(np.int32)), f(problem.indptr.astype(np.int64)),
+            f(problem.indices.astype(np.int32)), f(problem.counts.astype(np.int32)))

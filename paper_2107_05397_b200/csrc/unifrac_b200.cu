@@ -1,0 +1,383 @@
+// unifrac_b200.cu -- host side of the C ABI declared in include/unifrac_b200.h.
+// Enqueues the plan (a-0), embedding (a-1..a-4) and stripe+finalize (a-5, a-6) kernels on one stream.
+// No CPU fallback: every step of the path runs in the kernels of plan.cuh / embed.cuh / stripe.cuh.
+#include "../../include/unifrac_b200.h"
+#include "common.cuh"
+#include "plan.cuh"
+#include "embed.cuh"
+#include "stripe.cuh"
+
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+#include <vector>
+
+using namespace ufb;
+
+namespace {
+
+thread_local std::string g_cuda_err;
+thread_local unifrac_stats_t g_stats;
+thread_local unsigned long long* g_stats_pinned = nullptr;   // [2] stripe counters, pinned host
+thread_local cudaEvent_t g_stats_event = nullptr;
+thread_local bool g_stats_pending = false;
+
+struct CudaFail { cudaError_t e; const char* what; int line; };
+
+#define CU(x)                                                                                   \
+    do {                                                                                        \
+        cudaError_t e_ = (x);                                                                   \
+        if (e_ != cudaSuccess) throw CudaFail{e_, #x, __LINE__};                                \
+    } while (0)
+#define CU_LAUNCH() CU(cudaGetLastError())
+
+struct WorkspaceFail {};
+struct StatusFail { int status; };
+
+// bump of caller-provided (or stream-ordered) device allocations
+struct Arena {
+    unifrac_alloc_fn fn; void* user; cudaStream_t stream;
+    std::vector<void*> owned;
+    size_t total = 0;
+    void* get(size_t bytes) {
+        if (bytes == 0) bytes = 256;
+        bytes = (bytes + 255) & ~(size_t)255;
+        void* p = nullptr;
+        if (fn) { p = fn(bytes, user); if (!p) throw WorkspaceFail{}; }
+        else {
+            cudaError_t e = cudaMallocAsync(&p, bytes, stream);
+            if (e != cudaSuccess) { cudaGetLastError(); throw WorkspaceFail{}; }
+            owned.push_back(p);
+        }
+        total += bytes;
+        return p;
+    }
+    template <typename U> U* get_n(size_t n) { return reinterpret_cast<U*>(get(n * sizeof(U))); }
+    void release() { for (void* p : owned) cudaFreeAsync(p, stream); owned.clear(); }
+};
+
+inline int cdiv(long long a, long long b) { return (int)((a + b - 1) / b); }
+
+struct Timer {
+    bool on; cudaStream_t s; cudaEvent_t ev[5]; int n = 0;
+    Timer(bool on_, cudaStream_t s_) : on(on_), s(s_) { if (on) for (auto& e : ev) cudaEventCreate(&e); }
+    ~Timer() { if (on) for (auto& e : ev) cudaEventDestroy(e); }
+    void mark() { if (on && n < 5) cudaEventRecord(ev[n++], s); }
+    float ms(int a, int b) { float m = 0; if (on && b < n) cudaEventElapsedTime(&m, ev[a], ev[b]); return m; }
+};
+
+template <typename T>
+void run(int32_t n, const int32_t* parent, const double* len, const int32_t* postorder, unifrac_csr_t tab,
+         int32_t N, int weighted, void* out, Arena& A, uint32_t flags, cudaStream_t st)
+{
+    const bool validate = !(flags & UNIFRAC_FLAG_SKIP_VALIDATION);
+    const bool timing = getenv("UNIFRAC_B200_TIMING") && atoi(getenv("UNIFRAC_B200_TIMING")) != 0;
+    Timer tm(timing, st);
+    unsigned launches = 0;
+    tm.mark();
+
+    // ------------------------------------------------------------------ a-0 plan / validate
+    const int TB = 256;
+    PlanWords* pw = A.get_n<PlanWords>(1);
+    int32_t* child_count = A.get_n<int32_t>(n);
+    int32_t* seen = A.get_n<int32_t>(n);
+    int32_t* pos = A.get_n<int32_t>(n);
+    unsigned long long* Tsum = A.get_n<unsigned long long>(N);
+    CU(cudaMemsetAsync(pw, 0, sizeof(PlanWords), st));
+    CU(cudaMemsetAsync(child_count, 0, sizeof(int32_t) * n, st));
+    k_tree_check<<<cdiv(n, TB), TB, 0, st>>>(n, parent, len, child_count, pw, validate); CU_LAUNCH(); ++launches;
+    k_root_check<<<1, 1, 0, st>>>(pw); CU_LAUNCH(); ++launches;
+    if (validate) {
+        CU(cudaMemsetAsync(seen, 0, sizeof(int32_t) * n, st));
+        k_post_check1<<<cdiv(n, TB), TB, 0, st>>>(n, postorder, seen, pos, pw); CU_LAUNCH(); ++launches;
+        k_post_check2<<<cdiv(n, TB), TB, 0, st>>>(n, parent, postorder, pos, pw); CU_LAUNCH(); ++launches;
+    }
+    PlanWords h{};
+    CU(cudaMemcpyAsync(&h, pw, sizeof(h), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    if (h.err & ERRBIT_TREE) throw StatusFail{UNIFRAC_ERR_INVALID_TREE};
+
+    k_csr_check<<<cdiv((long long)N * 32, TB), TB, 0, st>>>(n, N, tab.indptr, tab.indices, tab.counts, child_count,
+                                                             Tsum, pw, validate); CU_LAUNCH(); ++launches;
+    // depths by pointer jumping
+    int32_t* anc[2] = {A.get_n<int32_t>(n), A.get_n<int32_t>(n)};
+    int32_t* dist[2] = {A.get_n<int32_t>(n), A.get_n<int32_t>(n)};
+    k_jump_init<<<cdiv(n, TB), TB, 0, st>>>(n, parent, anc[0], dist[0]); CU_LAUNCH(); ++launches;
+    int cur = 0;
+    for (long long reach = 1; reach < n; reach <<= 1) {
+        k_jump_round<<<cdiv(n, TB), TB, 0, st>>>(n, anc[cur], dist[cur], anc[cur ^ 1], dist[cur ^ 1]); CU_LAUNCH(); ++launches;
+        cur ^= 1;
+    }
+    const int32_t* depth = dist[cur];
+    uint32_t* hist = A.get_n<uint32_t>((size_t)n + 1);
+    CU(cudaMemsetAsync(hist, 0, sizeof(uint32_t) * ((size_t)n + 1), st));
+    k_level_hist<<<cdiv(n, TB), TB, 0, st>>>(n, depth, child_count, hist, pw); CU_LAUNCH(); ++launches;
+    CU(cudaMemcpyAsync(&h, pw, sizeof(h), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    if (h.err & ERRBIT_TABLE) throw StatusFail{UNIFRAC_ERR_INVALID_TABLE};
+    if (h.err & ERRBIT_EMPTY) throw StatusFail{UNIFRAC_ERR_EMPTY_SAMPLE};
+    if (h.err & ERRBIT_UNSUPPORTED) throw StatusFail{UNIFRAC_ERR_UNSUPPORTED};
+    const int root = h.root;
+    const int n_levels = h.max_depth + 1;
+    const size_t n_internal = (size_t)h.n_internal;
+    std::vector<uint32_t> h_hist(n_levels), h_off(n_levels + 1);
+    CU(cudaMemcpyAsync(h_hist.data(), hist, sizeof(uint32_t) * n_levels, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    h_off[0] = 0;
+    for (int d = 0; d < n_levels; ++d) h_off[d + 1] = h_off[d] + h_hist[d];
+    uint32_t* cursor = A.get_n<uint32_t>(n_levels);
+    int32_t* level_nodes = A.get_n<int32_t>(n_internal ? n_internal : 1);
+    CU(cudaMemcpyAsync(cursor, h_off.data(), sizeof(uint32_t) * n_levels, cudaMemcpyHostToDevice, st));
+    k_level_fill<<<cdiv(n, TB), TB, 0, st>>>(n, depth, child_count, cursor, level_nodes); CU_LAUNCH(); ++launches;
+    uint32_t* child_off = A.get_n<uint32_t>((size_t)n + 1);
+    uint32_t* child_cur = A.get_n<uint32_t>((size_t)n + 1);
+    int32_t* child_idx = A.get_n<int32_t>(n);
+    k_exclusive_scan<int32_t><<<1, 1024, 0, st>>>(n, child_count, child_off); CU_LAUNCH(); ++launches;
+    CU(cudaMemcpyAsync(child_cur, child_off, sizeof(uint32_t) * ((size_t)n + 1), cudaMemcpyDeviceToDevice, st));
+    k_child_fill<<<cdiv(n, TB), TB, 0, st>>>(n, parent, child_cur, child_idx); CU_LAUNCH(); ++launches;
+    tm.mark();
+
+    // ------------------------------------------------------------------ a-1 .. a-4 embedding, per sample batch
+    const int n_tiles = cdiv(N, TILE);
+    const uint32_t nwords = (uint32_t)cdiv(n, 32);
+    size_t batch_budget = (size_t)4 << 30;                      // bytes of the dense count buffer
+    if (const char* e = getenv("UNIFRAC_B200_BATCH_MB")) batch_budget = (size_t)atoll(e) << 20;
+    long long tiles_per_batch = (long long)(batch_budget / ((size_t)n * TILE * 4));
+    if (tiles_per_batch < 1) tiles_per_batch = 1;
+    if (tiles_per_batch > n_tiles) tiles_per_batch = n_tiles;
+    const int Wb = (int)tiles_per_batch * TILE;
+
+    uint32_t* cnt = A.get_n<uint32_t>((size_t)n * Wb);
+    uint32_t* rflags = A.get_n<uint32_t>((size_t)n_tiles * nwords);
+    uint32_t* rrank = A.get_n<uint32_t>((size_t)n_tiles * nwords);
+    uint32_t* rows = A.get_n<uint32_t>(n_tiles);
+    uint8_t* qtmp = A.get_n<uint8_t>((size_t)tiles_per_batch * n);
+    uint32_t* nv = A.get_n<uint32_t>(n);
+    double* sums = A.get_n<double>((size_t)n_tiles * TILE);
+    T** tileE = A.get_n<T*>(n_tiles);
+    uint8_t** tileQ = A.get_n<uint8_t*>(n_tiles);
+    CU(cudaMemsetAsync(nv, 0, sizeof(uint32_t) * n, st));
+    CU(cudaMemsetAsync(sums, 0, sizeof(double) * (size_t)n_tiles * TILE, st));
+    std::vector<uint32_t> h_rows(n_tiles);
+    std::vector<T*> h_tileE(n_tiles);
+    std::vector<uint8_t*> h_tileQ(n_tiles);
+    uint64_t embed_rows = 0;
+
+    for (int t0 = 0; t0 < n_tiles; t0 += (int)tiles_per_batch) {
+        const int tb = (int)std::min<long long>(tiles_per_batch, n_tiles - t0);
+        const int s0 = t0 * TILE, s1 = std::min(N, (t0 + tb) * TILE);
+        CU(cudaMemsetAsync(cnt, 0, sizeof(uint32_t) * (size_t)n * Wb, st));
+        k_tip_scatter<<<cdiv((long long)(s1 - s0) * 32, TB), TB, 0, st>>>(s0, s1, tab.indptr, tab.indices, tab.counts, cnt, Wb);
+        CU_LAUNCH(); ++launches;
+        for (int d = n_levels - 1; d >= 0; --d) {            // deepest parents first
+            const uint32_t cntl = h_hist[d];
+            if (!cntl) continue;
+            const long long threads = (long long)cntl * (Wb / 4);
+            k_level_pull<<<cdiv(threads, TB), TB, 0, st>>>(level_nodes + h_off[d], (int)cntl, root, child_off, child_idx, cnt, Wb);
+            CU_LAUNCH(); ++launches;
+        }
+        k_row_flags<<<dim3(nwords, tb), 1024, 0, st>>>(n, parent, len, cnt, Wb, rflags, nwords, t0, qtmp, nv); CU_LAUNCH(); ++launches;
+        k_rank_scan<<<tb, 1024, 0, st>>>(rflags, rrank, nwords, t0, rows); CU_LAUNCH(); ++launches;
+        CU(cudaMemcpyAsync(h_rows.data() + t0, rows + t0, sizeof(uint32_t) * tb, cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        size_t tot = 0;
+        for (int t = t0; t < t0 + tb; ++t) tot += h_rows[t];
+        embed_rows += tot;
+        T* Eb = A.get_n<T>((tot ? tot : 1) * TILE);
+        uint8_t* Qb = A.get_n<uint8_t>(tot ? tot : 1);
+        size_t run_rows = 0;
+        for (int t = t0; t < t0 + tb; ++t) { h_tileE[t] = Eb + run_rows * TILE; h_tileQ[t] = Qb + run_rows; run_rows += h_rows[t]; }
+        CU(cudaMemcpyAsync(tileE + t0, h_tileE.data() + t0, sizeof(T*) * tb, cudaMemcpyHostToDevice, st));
+        CU(cudaMemcpyAsync(tileQ + t0, h_tileQ.data() + t0, sizeof(uint8_t*) * tb, cudaMemcpyHostToDevice, st));
+        k_compact<T><<<dim3(cdiv(nwords, COMPACT_WORDS), tb), 256, 0, st>>>(n, len, cnt, Wb, rflags, rrank, nwords, t0, Tsum, N,
+                                                                             weighted, tileE, tileQ, qtmp, sums);
+        CU_LAUNCH(); ++launches;
+        CU(cudaStreamSynchronize(st));   // h_tileE/h_tileQ staging copies are done; safe to reuse cnt
+    }
+    unsigned long long* work = A.get_n<unsigned long long>(8);
+    CU(cudaMemsetAsync(work, 0, sizeof(unsigned long long) * 8, st));
+    k_work_counts<<<cdiv(n, TB), TB, 0, st>>>(n, nv, (unsigned long long)N, work); CU_LAUNCH(); ++launches;
+    unsigned long long h_work[4];
+    CU(cudaMemcpyAsync(h_work, work, sizeof(h_work), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    tm.mark();
+
+    // ------------------------------------------------------------------ a-5 / a-6 stripe accumulation + finalize
+    std::vector<int2> h_pairs;
+    h_pairs.reserve((size_t)n_tiles * (n_tiles + 1) / 2);
+    for (int i = 0; i < n_tiles; ++i)
+        for (int j = i; j < n_tiles; ++j) h_pairs.push_back(make_int2(i, j));
+    const uint32_t n_pairs = (uint32_t)h_pairs.size();
+    int2* pairs = A.get_n<int2>(n_pairs);
+    CU(cudaMemcpyAsync(pairs, h_pairs.data(), sizeof(int2) * n_pairs, cudaMemcpyHostToDevice, st));
+    T* zero_row = A.get_n<T>(TILE);
+    CU(cudaMemsetAsync(zero_row, 0, sizeof(T) * TILE, st));
+    unsigned long long* kstats = work + 4;     // [0] rows executed, [1] rows staged (zeroed above)
+    uint32_t* counter = reinterpret_cast<uint32_t*>(work + 6);
+
+    StripeParams P{};
+    P.tileE = reinterpret_cast<const void* const*>(tileE);
+    P.tileQ = tileQ; P.flags = rflags; P.rank = rrank; P.nwords = nwords;
+    P.pairs = pairs; P.n_pairs = n_pairs; P.counter = counter; P.sums = sums;
+    P.n_samples = N; P.weighted = weighted; P.out = out; P.stats = kstats; P.zero_row = zero_row;
+
+    unsigned stripe_launches = 0;
+    if (flags & UNIFRAC_FLAG_LITERAL) {
+        k_literal<T><<<n_pairs, 256, 0, st>>>(P); CU_LAUNCH(); ++launches; ++stripe_launches;
+    } else {
+        int dev = 0, n_sm = 0;
+        CU(cudaGetDevice(&dev));
+        CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+        const size_t smem = stripe_smem_bytes<T>();
+        auto kern = (flags & UNIFRAC_FLAG_ABSDIFF) ? k_stripe<T, FORM_ABSDIFF> : k_stripe<T, FORM_MIN>;
+        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int occ = 0;
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, STRIPE_THREADS, smem));
+        if (occ < 1) occ = 1;
+        unsigned grid = (unsigned)std::min<long long>((long long)n_sm * occ, n_pairs);
+        P.scratch = A.get_n<double>((size_t)grid * 64 * 256);
+        kern<<<grid, STRIPE_THREADS, smem, st>>>(P); CU_LAUNCH(); ++launches; ++stripe_launches;
+    }
+    // stripe counters -> pinned host block (read lazily by unifrac_last_stats)
+    if (!g_stats_pinned) { CU(cudaHostAlloc(&g_stats_pinned, 2 * sizeof(unsigned long long), cudaHostAllocDefault)); }
+    if (!g_stats_event) { CU(cudaEventCreateWithFlags(&g_stats_event, cudaEventDisableTiming)); }
+    CU(cudaMemcpyAsync(g_stats_pinned, kstats, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    CU(cudaEventRecord(g_stats_event, st));
+    g_stats_pending = true;
+    tm.mark();
+
+    g_stats = unifrac_stats_t{};
+    g_stats.branches_embedded = h_work[0];
+    g_stats.updates_dense = (uint64_t)h_work[0] * ((uint64_t)N * (N - 1) / 2);
+    g_stats.updates_union = h_work[1];
+    g_stats.updates_inter = h_work[2];
+    g_stats.embed_rows = embed_rows;
+    g_stats.n_tile_pairs = n_pairs;
+    g_stats.n_levels = (uint32_t)n_levels;
+    g_stats.stripe_launches = stripe_launches;
+    g_stats.kernel_launches = launches;
+    A.release();
+    g_stats.workspace_bytes = A.total;
+    if (timing) {
+        CU(cudaStreamSynchronize(st));
+        g_stats.ms_plan = tm.ms(0, 1); g_stats.ms_embed = tm.ms(1, 2); g_stats.ms_stripe = tm.ms(2, 3); g_stats.ms_total = tm.ms(0, 3);
+    }
+}
+
+int guarded(int32_t n_nodes, const int32_t* parent, const double* len, const int32_t* postorder, unifrac_csr_t tab,
+            int32_t N, unifrac_variant_t variant, unifrac_precision_t precision, void* out, unifrac_alloc_fn alloc,
+            void* user, uint32_t flags, cudaStream_t st)
+{
+    if (!parent || !len || !postorder || !tab.indptr || !tab.indices || !tab.counts || !out) return UNIFRAC_ERR_INVALID_ARG;
+    if (n_nodes < 2 || N < 2) return UNIFRAC_ERR_INVALID_ARG;
+    if (variant != UNIFRAC_UNWEIGHTED && variant != UNIFRAC_WEIGHTED_NORMALIZED) return UNIFRAC_ERR_INVALID_ARG;
+    if (precision != UNIFRAC_FP32 && precision != UNIFRAC_FP64) return UNIFRAC_ERR_INVALID_ARG;
+    if (flags & ~(UNIFRAC_FLAG_LITERAL | UNIFRAC_FLAG_TENSOR_GRAM | UNIFRAC_FLAG_SKIP_VALIDATION | UNIFRAC_FLAG_ABSDIFF))
+        return UNIFRAC_ERR_INVALID_ARG;
+    if ((long long)N > (1ll << 23)) return UNIFRAC_ERR_UNSUPPORTED;
+    Arena A{alloc, user, st};
+    int rc = UNIFRAC_OK;
+    try {
+        if (precision == UNIFRAC_FP32) run<float>(n_nodes, parent, len, postorder, tab, N, variant == UNIFRAC_WEIGHTED_NORMALIZED, out, A, flags, st);
+        else run<double>(n_nodes, parent, len, postorder, tab, N, variant == UNIFRAC_WEIGHTED_NORMALIZED, out, A, flags, st);
+    } catch (const CudaFail& f) {
+        char buf[512];
+        snprintf(buf, sizeof(buf), "%s: %s (unifrac_b200.cu:%d)", f.what, cudaGetErrorString(f.e), f.line);
+        g_cuda_err = buf;
+        cudaGetLastError();
+        rc = UNIFRAC_ERR_CUDA;
+    } catch (const WorkspaceFail&) { rc = UNIFRAC_ERR_WORKSPACE; }
+    catch (const StatusFail& s) { rc = s.status; }
+    catch (...) { rc = UNIFRAC_ERR_CUDA; g_cuda_err = "unexpected C++ exception"; }
+    if (rc != UNIFRAC_OK) A.release();
+    return rc;
+}
+
+}  // namespace
+
+extern "C" {
+
+int unifrac_dm(int32_t n_nodes, const int32_t* tree_parent, const double* branch_len, const int32_t* postorder,
+               unifrac_csr_t table, int32_t n_samples, unifrac_variant_t variant, unifrac_precision_t precision,
+               void* out_condensed, unifrac_alloc_fn alloc, void* alloc_user, uint32_t flags, void* stream)
+{
+    return guarded(n_nodes, tree_parent, branch_len, postorder, table, n_samples, variant, precision, out_condensed,
+                   alloc, alloc_user, flags, reinterpret_cast<cudaStream_t>(stream));
+}
+
+int unifrac_dm_host(int32_t n_nodes, const int32_t* tree_parent, const double* branch_len, const int32_t* postorder,
+                    unifrac_csr_t th, int32_t N, unifrac_variant_t variant, unifrac_precision_t precision,
+                    void* out_host, uint32_t flags)
+{
+    if (!tree_parent || !branch_len || !postorder || !th.indptr || !th.indices || !th.counts || !out_host) return UNIFRAC_ERR_INVALID_ARG;
+    if (n_nodes < 2 || N < 2) return UNIFRAC_ERR_INVALID_ARG;
+    if (precision != UNIFRAC_FP32 && precision != UNIFRAC_FP64) return UNIFRAC_ERR_INVALID_ARG;
+    const int64_t nnz = th.indptr[N];
+    if (nnz < 0) return UNIFRAC_ERR_INVALID_TABLE;
+    const size_t esz = precision == UNIFRAC_FP32 ? 4 : 8;
+    const size_t n_out = (size_t)N * (N - 1) / 2;
+    cudaStream_t st = nullptr;
+    void *d_parent = nullptr, *d_len = nullptr, *d_post = nullptr, *d_indptr = nullptr, *d_idx = nullptr, *d_cnt = nullptr, *d_out = nullptr;
+    int rc = UNIFRAC_OK;
+    auto ok = [&](cudaError_t e) { if (e != cudaSuccess && rc == UNIFRAC_OK) { g_cuda_err = cudaGetErrorString(e); cudaGetLastError(); rc = e == cudaErrorMemoryAllocation ? UNIFRAC_ERR_WORKSPACE : UNIFRAC_ERR_CUDA; } return rc == UNIFRAC_OK; };
+    ok(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
+    ok(cudaMalloc(&d_parent, sizeof(int32_t) * n_nodes)) && ok(cudaMalloc(&d_len, sizeof(double) * n_nodes)) &&
+    ok(cudaMalloc(&d_post, sizeof(int32_t) * n_nodes)) && ok(cudaMalloc(&d_indptr, sizeof(int64_t) * ((size_t)N + 1))) &&
+    ok(cudaMalloc(&d_idx, sizeof(int32_t) * (size_t)(nnz ? nnz : 1))) && ok(cudaMalloc(&d_cnt, sizeof(int32_t) * (size_t)(nnz ? nnz : 1))) &&
+    ok(cudaMalloc(&d_out, esz * n_out));
+    if (rc == UNIFRAC_OK) {
+        ok(cudaMemcpyAsync(d_parent, tree_parent, sizeof(int32_t) * n_nodes, cudaMemcpyHostToDevice, st));
+        ok(cudaMemcpyAsync(d_len, branch_len, sizeof(double) * n_nodes, cudaMemcpyHostToDevice, st));
+        ok(cudaMemcpyAsync(d_post, postorder, sizeof(int32_t) * n_nodes, cudaMemcpyHostToDevice, st));
+        ok(cudaMemcpyAsync(d_indptr, th.indptr, sizeof(int64_t) * ((size_t)N + 1), cudaMemcpyHostToDevice, st));
+        ok(cudaMemcpyAsync(d_idx, th.indices, sizeof(int32_t) * (size_t)nnz, cudaMemcpyHostToDevice, st));
+        ok(cudaMemcpyAsync(d_cnt, th.counts, sizeof(int32_t) * (size_t)nnz, cudaMemcpyHostToDevice, st));
+    }
+    if (rc == UNIFRAC_OK) {
+        unifrac_csr_t td{reinterpret_cast<const int64_t*>(d_indptr), reinterpret_cast<const int32_t*>(d_idx), reinterpret_cast<const int32_t*>(d_cnt)};
+        rc = guarded(n_nodes, reinterpret_cast<const int32_t*>(d_parent), reinterpret_cast<const double*>(d_len),
+                     reinterpret_cast<const int32_t*>(d_post), td, N, variant, precision, d_out, nullptr, nullptr, flags, st);
+    }
+    if (rc == UNIFRAC_OK) {
+        ok(cudaMemcpyAsync(out_host, d_out, esz * n_out, cudaMemcpyDeviceToHost, st));
+        ok(cudaStreamSynchronize(st));
+    }
+    if (st) cudaStreamSynchronize(st);
+    cudaFree(d_parent); cudaFree(d_len); cudaFree(d_post); cudaFree(d_indptr); cudaFree(d_idx); cudaFree(d_cnt); cudaFree(d_out);
+    if (st) cudaStreamDestroy(st);
+    return rc;
+}
+
+int unifrac_last_stats(unifrac_stats_t* out)
+{
+    if (!out) return UNIFRAC_ERR_INVALID_ARG;
+    if (g_stats_pending) {
+        if (cudaEventSynchronize(g_stats_event) != cudaSuccess) { cudaGetLastError(); return UNIFRAC_ERR_CUDA; }
+        g_stats.updates_executed = g_stats_pinned[0] * 2048ull;    // one (warp,row) = 32 x 64 pair updates
+        g_stats.rows_staged = g_stats_pinned[1];
+        g_stats_pending = false;
+    }
+    *out = g_stats;
+    return UNIFRAC_OK;
+}
+
+const char* unifrac_status_string(int status)
+{
+    switch (status) {
+        case UNIFRAC_OK: return "ok";
+        case UNIFRAC_ERR_INVALID_ARG: return "invalid argument";
+        case UNIFRAC_ERR_INVALID_TREE: return "invalid tree";
+        case UNIFRAC_ERR_INVALID_TABLE: return "invalid table";
+        case UNIFRAC_ERR_EMPTY_SAMPLE: return "empty sample";
+        case UNIFRAC_ERR_WORKSPACE: return "workspace allocation failed";
+        case UNIFRAC_ERR_CUDA: return "CUDA error";
+        case UNIFRAC_ERR_UNSUPPORTED: return "unsupported size";
+        default: return "unknown status";
+    }
+}
+
+const char* unifrac_last_cuda_error(void) { return g_cuda_err.c_str(); }
+int unifrac_abi_version(void) { return 1; }
+
+}  // extern "C"

@@ -1,0 +1,48 @@
+"""The C-ABI library builds for sm_100a, loads without a GPU, and exports every symbol that
+include/unifrac_b200.h declares (no compute calls here)."""
+import os
+import re
+import subprocess
+
+from paper_2107_05397_b200 import binding, build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared():
+    src = open(os.path.join(ROOT, "include", "unifrac_b200.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return set(re.findall(r"\b(unifrac_[a-z_]+)\s*\(", src)) - {"unifrac_alloc_fn"}
+
+
+def test_header_symbols_are_exported_and_bound():
+    lib = binding.load()
+    declared = _declared()
+    assert declared == set(binding.EXPORTS)
+    for name in declared:
+        assert getattr(lib, name) is not None
+    out = subprocess.run(["nm", "-D", "--defined-only", build.LIB], capture_output=True, text=True).stdout
+    for name in declared:
+        assert re.search(rf"\bT {name}\b", out), name
+
+
+def test_version_and_status_strings_without_gpu():
+    assert binding.unifrac_abi_version() == 1
+    assert binding.unifrac_status_string(0) == "ok"
+    assert "tree" in binding.unifrac_status_string(binding.ERR_INVALID_TREE)
+
+
+def test_host_checkable_errors_return_before_any_cuda_work():
+    import ctypes as C
+    lib = binding.load()
+    null = binding.CSR(None, None, None)
+    rc = lib.unifrac_dm(10, None, None, None, null, 5, 0, 0, None, binding.ALLOC_FN(0), None, 0, None)
+    assert rc == binding.ERR_INVALID_ARG
+    rc = lib.unifrac_dm_host(10, None, None, None, null, 5, 0, 0, None, 0)
+    assert rc == binding.ERR_INVALID_ARG
+
+
+def test_library_is_built_for_sm_100a_with_bulk_copies():
+    sass = subprocess.run(["cuobjdump", "-sass", build.LIB], capture_output=True, text=True).stdout
+    assert "sm_100a" in sass
+    assert "UBLKCP" in sass            # cp.async.bulk (TMA bulk copy) in the stripe kernel

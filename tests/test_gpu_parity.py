@@ -1,0 +1,199 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs.  Tolerances are BASELINE.json:5's: 1e-10 relative (fp64), 1e-5 relative
+(fp32); the absolute clause (1e-12 / 1e-7, reading Q12) only matters for d ~ 0."""
+import numpy as np
+import pytest
+
+from paper_2107_05397_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+U, W = 0, 1
+RTOL = {0: 1e-5, 1: 1e-10}       # precision enum -> rtol
+ATOL = {0: 1e-7, 1: 1e-12}
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2107_05397_b200 import binding
+    binding.load()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def O():
+    from oracle import oracle
+    return oracle
+
+
+def gpu_dm(B, p, variant, precision, flags=0):
+    import torch
+    args = B.to_device(p)
+    out = B.unifrac_dm(*args, p.n_samples, variant, precision, flags=flags)
+    torch.cuda.synchronize()
+    return out.cpu().numpy().astype(np.float64)
+
+
+def check(got, want, precision):
+    err = np.abs(got - want)
+    ok = (err <= RTOL[precision] * np.abs(want)) | (err <= ATOL[precision])
+    rel = err / np.maximum(np.abs(want), 1e-300)
+    assert ok.all(), f"max rel err {rel[~ok].max():.3e} at {np.argmax(~ok)} (got {got[np.argmax(~ok)]}, want {want[np.argmax(~ok)]})"
+    return float(rel[np.abs(want) > 1e-6].max()) if (np.abs(want) > 1e-6).any() else 0.0
+
+
+@pytest.mark.parametrize("variant", [U, W])
+@pytest.mark.parametrize("precision", [1, 0])
+@pytest.mark.parametrize("flags", [0, 8, 1])       # min form, direct |u-v| form, literal debug kernel
+def test_tiny_all_pairs(B, O, variant, precision, flags):
+    p = synth.make_config("tiny", seed=0)
+    want = O.all_pairs(p.parent, p.branch_len, p.indptr, p.indices, p.counts, variant)
+    check(gpu_dm(B, p, variant, precision, flags), want, precision)
+
+
+@pytest.mark.parametrize("variant", [U, W])
+@pytest.mark.parametrize("precision", [1, 0])
+@pytest.mark.parametrize("flags", [0, 8])
+def test_three_tiles_ragged_tail_all_pairs(B, O, variant, precision, flags):
+    """300 samples = 2 full 128-tiles + a 44-sample tail; 3000 tips -> 5998 branches (several stages)."""
+    p = synth.make_problem(3000, 300, 0.1, 1.1, synth.CONFIGS["small"][4], synth.CONFIGS["small"][5], seed=3)
+    want = O.all_pairs(p.parent, p.branch_len, p.indptr, p.indices, p.counts, variant)
+    check(gpu_dm(B, p, variant, precision, flags), want, precision)
+
+
+@pytest.mark.parametrize("n_samples", [2, 3, 127, 128, 129, 257])
+def test_tile_boundary_sample_counts(B, O, n_samples):
+    p = synth.make_problem(400, n_samples, 0.1, 1.1, synth._k_poisson40, synth._c_geometric, seed=n_samples)
+    for variant in (U, W):
+        want = O.all_pairs(p.parent, p.branch_len, p.indptr, p.indices, p.counts, variant)
+        check(gpu_dm(B, p, variant, 1), want, 1)
+        check(gpu_dm(B, p, variant, 0), want, 0)
+
+
+@pytest.mark.parametrize("seed", range(5))
+def test_general_trees_multifurcation_unary_zero_length(B, O, seed):
+    rng = np.random.default_rng(500 + seed)
+    parent, bl = synth.random_tree(int(rng.integers(5, 400)), rng, p_unary=0.25, p_zero_len=0.25)
+    tips = synth.tip_ids(parent)
+    p = synth.problem_from_parent(parent, bl, synth.random_table(tips, int(rng.integers(2, 150)), rng, density=0.2))
+    for variant in (U, W):
+        want = O.all_pairs(p.parent, p.branch_len, p.indptr, p.indices, p.counts, variant)
+        for flags in (0, 8, 1):
+            check(gpu_dm(B, p, variant, 1, flags), want, 1)
+        check(gpu_dm(B, p, variant, 0), want, 0)
+
+
+def test_duplicate_and_proportional_samples_give_zero(B):
+    parent, bl = synth.random_tree(60, np.random.default_rng(9), p_zero_len=0.0)
+    tips = synth.tip_ids(parent)
+    rows = synth.random_table(tips, 6, np.random.default_rng(10))
+    rows.append(dict(rows[1]))
+    rows.append({t: 7 * c for t, c in rows[2].items()})
+    p = synth.problem_from_parent(parent, bl, rows)
+    n = p.n_samples
+    for variant in (U, W):
+        for precision, tol in ((1, 1e-14), (0, 1e-6)):
+            d = gpu_dm(B, p, variant, precision)
+            assert abs(d[int(synth.condensed_index(n, 1, 6))]) <= tol
+            assert abs(d[int(synth.condensed_index(n, 2, 7))]) <= tol
+            assert np.all(d >= 0) and np.all(d <= 1 + 1e-6) and not np.isnan(d).any()
+        d = gpu_dm(B, p, variant, 1, flags=8)          # direct form: exactly 0
+        assert d[int(synth.condensed_index(n, 1, 6))] == 0.0 and d[int(synth.condensed_index(n, 2, 7))] == 0.0
+
+
+def test_zero_denominator_gives_zero(B):
+    parent, bl = synth.star_tree(3, [0.0, 0.0, 1.0])
+    p = synth.problem_from_parent(parent, bl, [{0: 1}, {1: 2}, {2: 1}])
+    for variant in (U, W):
+        for flags in (0, 8, 1):
+            d = gpu_dm(B, p, variant, 1, flags)
+            assert d[0] == 0.0 and d[1] == 1.0 and d[2] == 1.0
+
+
+def test_small_config_sampled_pairs(B, O):
+    """BASELINE.json config 'Small' (20k tips, 2048 samples, fp64, both variants): 20k seeded pairs +
+    tile-boundary neighbours + first/last condensed elements via the oracle's pair-list driver."""
+    p = synth.make_config("small", seed=0)
+    n = p.n_samples
+    pairs = synth.sample_pairs(n, 20000, seed=0)
+    extra = np.array([[0, 1], [0, n - 1], [n - 2, n - 1], [127, 128], [0, 128], [127, 255], [128, 129],
+                      [1919, 1920], [2047 - 128, 2047]], dtype=np.int32)
+    pairs = np.concatenate([pairs, extra])
+    idx = synth.condensed_index(n, pairs[:, 0], pairs[:, 1])
+    for variant in (U, W):
+        want = O.pair_list(p.parent, p.branch_len, p.indptr, p.indices, p.counts, variant, pairs)
+        got = gpu_dm(B, p, variant, 1)
+        check(got[idx], want, 1)
+        got32 = gpu_dm(B, p, variant, 0)
+        check(got32[idx], want, 0)
+        assert np.all(got >= 0) and np.all(got <= 1)
+
+
+def test_host_entry_point_matches_device_entry_point(B, O):
+    p = synth.make_config("tiny", seed=2)
+    for variant in (U, W):
+        want = O.all_pairs(p.parent, p.branch_len, p.indptr, p.indices, p.counts, variant)
+        got = B.unifrac_dm_host(p.parent, p.branch_len, p.postorder, p.indptr, p.indices, p.counts,
+                                p.n_samples, variant, B.FP64)
+        check(got, want, 1)
+        got32 = B.unifrac_dm_host(p.parent, p.branch_len, p.postorder, p.indptr, p.indices, p.counts,
+                                  p.n_samples, variant, B.FP32).astype(np.float64)
+        check(got32, want, 0)
+
+
+def test_error_codes(B):
+    import torch
+    p = synth.make_config("tiny", seed=0)
+
+    def rc_of(**kw):
+        q = synth.Problem(kw.get("parent", p.parent), kw.get("bl", p.branch_len), kw.get("post", p.postorder),
+                          kw.get("indptr", p.indptr), kw.get("indices", p.indices), kw.get("counts", p.counts))
+        try:
+            B.unifrac_dm(*B.to_device(q), q.n_samples, U, B.FP64)
+            torch.cuda.synchronize()
+            return 0
+        except B.UnifracError as e:
+            return e.status
+
+    assert rc_of() == 0
+    bad = p.parent.copy(); bad[5] = -1
+    assert rc_of(parent=bad) == B.ERR_INVALID_TREE                       # two roots
+    bad = p.parent.copy(); bad[5] = p.n_nodes + 3
+    assert rc_of(parent=bad) == B.ERR_INVALID_TREE
+    post = p.postorder.copy(); post[[0, -1]] = post[[-1, 0]]
+    assert rc_of(post=post) == B.ERR_INVALID_TREE                        # root not last
+    post = p.postorder.copy(); post[3] = post[4]
+    assert rc_of(post=post) == B.ERR_INVALID_TREE                        # not a permutation
+    bl = p.branch_len.copy(); bl[7] = -1.0
+    assert rc_of(bl=bl) == B.ERR_INVALID_TREE
+    bl = p.branch_len.copy(); bl[7] = np.nan
+    assert rc_of(bl=bl) == B.ERR_INVALID_TREE
+    idx = p.indices.copy(); idx[0] = 0                                   # node 0 is the root (internal)
+    assert rc_of(indices=idx) == B.ERR_INVALID_TABLE
+    idx = p.indices.copy(); idx[[0, 1]] = idx[[1, 0]]
+    assert rc_of(indices=idx) == B.ERR_INVALID_TABLE                     # not increasing
+    cnt = p.counts.copy(); cnt[3] = -2
+    assert rc_of(counts=cnt) == B.ERR_INVALID_TABLE
+    cnt = p.counts.copy(); cnt[p.indptr[4]:p.indptr[5]] = 0
+    assert rc_of(counts=cnt) == B.ERR_EMPTY_SAMPLE
+
+
+def test_stats_work_counters_match_definitions(B):
+    """W_dense / W_union / W_inter against their closed forms computed from presence."""
+    import torch
+    import refmath
+    p = synth.make_config("tiny", seed=4)
+    B.unifrac_dm(*B.to_device(p), p.n_samples, U, B.FP64)
+    torch.cuda.synchronize()
+    st = B.unifrac_last_stats()
+    A, tips = refmath.ancestor_matrix(p.parent)
+    X = refmath.dense_counts(p, tips)
+    pres = (X @ A.T) > 0
+    keep = (p.parent >= 0) & (p.branch_len > 0)
+    nv = pres[:, keep].sum(0)
+    N = p.n_samples
+    assert st["branches_embedded"] == int((nv > 0).sum())
+    assert st["updates_dense"] == int((nv > 0).sum()) * N * (N - 1) // 2
+    assert st["updates_inter"] == int((nv * (nv - 1) // 2).sum())
+    assert st["updates_union"] == int((N * (N - 1) // 2 - (N - nv) * (N - nv - 1) // 2)[nv > 0].sum())
+    assert st["updates_executed"] > 0 and st["kernel_launches"] > 0 and st["stripe_launches"] == 1
