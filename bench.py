@@ -1,0 +1,284 @@
+#!/usr/bin/env python
+"""bench.py -- UniFrac all-pairs hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload emp|large|medium|small|tiny]
+                    [--impl ours|reference] [--no-cpu-baseline] [--no-e2e]
+
+A "step" is one pass of the whole hot path (plan, embedding, stripe accumulation, finalize) for
+every variant the workload lists (unweighted and weighted-normalized), inputs resident in HBM.
+metric = dense-equivalent sample-pair x branch updates per second  (BASELINE.json "metric"):
+         sum over the step's calls of P * B_emb, divided by the step time.
+Prints ONE JSON line (rank 0).  N > 1: one process per GPU, independent replicas (the path runs on
+one GPU), barrier + max-over-ranks timing, value = all ranks' updates / time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2107_05397_b200 import synth  # noqa: E402
+
+METRIC = "unifrac_dense_equivalent_pair_branch_updates_per_s"
+UNIT = "updates/s"
+SM_COUNT, FP32_LANES, SM_MAX_GHZ = 148, 128, 1.965        # B200_PROFILING.md / MEASURED_PEAKS.json
+ALU_PEAK_TFLOPS = SM_COUNT * FP32_LANES * SM_MAX_GHZ / 1e3    # FADD/FMNMX-class lane-ops (not FMA-doubled)
+
+WORKLOADS = {   # name -> (variants, precision)    BASELINE.json:7-11
+    "tiny": ((0, 1), 1), "small": ((0, 1), 1), "medium": ((0,), 0), "emp": ((0, 1), 0), "large": ((0, 1), 0),
+}
+
+
+def clocks_sampler(stop, out, gpu_index):
+    q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+    try:
+        pr = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), f"--query-gpu={q}", "--format=csv,noheader,nounits",
+                               "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+    except Exception:
+        return
+    def rd():
+        for line in pr.stdout:
+            out.append(line.strip())
+    th = threading.Thread(target=rd, daemon=True)
+    th.start()
+    stop.wait()
+    pr.terminate()
+    th.join(timeout=2)
+
+
+def summarize_clocks(lines):
+    sm, mx, reasons = [], [], set()
+    names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+    for ln in lines:
+        f = [x.strip() for x in ln.split(",")]
+        if len(f) < 7:
+            continue
+        try:
+            sm.append(float(f[0])); mx.append(float(f[1]))
+        except ValueError:
+            continue
+        for k, nm in enumerate(names):
+            if f[3 + k].lower().startswith("active"):
+                reasons.add(nm)
+    if not sm:
+        return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+    busy = sorted(sm)[len(sm) // 2:]           # upper half = under load
+    return {"sm_mhz": float(np.median(busy)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def reduce_over_ranks(ms_local: float, updates_local: float, world: int, device=None):
+    """Max of the per-rank step time and sum of the per-rank updates (replicas: no data-path collective)."""
+    if world <= 1:
+        return ms_local, updates_local
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms_local], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    u = torch.tensor([updates_local], dtype=torch.float64, device=device)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+def rank_seed(seed: int, rank: int) -> int:
+    """Replica r works on its own seeded problem."""
+    return seed + rank
+
+
+def oracle_leg(p, variants, budget_s, seed=0):
+    """Times the oracle's pair-list driver, as it stands, on a bounded seeded sample of pairs."""
+    from oracle import oracle
+    def run(npairs, variant):
+        pairs = synth.sample_pairs(p.n_samples, npairs, seed=seed)
+        t = time.perf_counter()
+        oracle.pair_list(p.parent, p.branch_len, p.indptr, p.indices, p.counts, variant, pairs)
+        return time.perf_counter() - t
+    probe = max(200, min(2000, p.n_pairs))
+    t_probe = run(probe, variants[0])
+    per_pair = t_probe / probe
+    npairs = int(max(probe, min(p.n_pairs, budget_s / max(per_pair, 1e-9) / len(variants))))
+    npairs = min(npairs, 2_000_000)
+    total_t, total_pairs = 0.0, 0
+    for v in variants:
+        total_t += run(npairs, v)
+        total_pairs += npairs
+    return dict(pairs=total_pairs, seconds=total_t, cores=oracle.num_threads(),
+                sample=f"{npairs} seeded pairs per variant x {len(variants)} variant(s), pair-list driver "
+                       f"(includes building the per-sample branch lists)")
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default=os.environ.get("UNIFRAC_BENCH_WORKLOAD", "emp"))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--seed", type=int, default=0)
+    ap.add_argument("--flags", type=int, default=0)
+    ap.add_argument("--cpu-budget-s", type=float, default=15.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    a = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    variants, precision = WORKLOADS[a.workload]
+    dtype = "f32" if precision == 0 else "f64"
+
+    # ---------------------------------------------------------------- reference arm = the oracle on host cores
+    if a.impl == "reference":
+        if rank != 0:
+            return 0
+        p = synth.make_config(a.workload, seed=a.seed)
+        legs = [oracle_leg(p, variants, a.cpu_budget_s / max(1, a.steps + a.warmup), seed=k) for k in range(a.warmup + a.steps)]
+        timed = legs[a.warmup:]
+        b_emb = int(((p.parent >= 0) & (p.branch_len > 0)).sum())      # upper bound of B_emb (all branches with len > 0)
+        upd = sum(l["pairs"] for l in timed) * b_emb
+        secs = sum(l["seconds"] for l in timed)
+        val = upd / secs
+        line = dict(metric=METRIC, value=val, unit=UNIT, n_gpus=a.gpus, steps=a.steps, warmup=a.warmup,
+                    ms_per_step=1e3 * secs / a.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
+                    dtype="f64", data="synthetic", impl="reference",
+                    config=dict(workload=a.workload, n_samples=p.n_samples, n_nodes=p.n_nodes, nnz=p.nnz, seed=a.seed,
+                                variants=list(variants), step="bounded pair sample of the workload"),
+                    cpu_baseline=dict(value=val, unit=UNIT, cores=timed[0]["cores"], kind="oracle", sample=timed[0]["sample"]),
+                    e2e=dict(value=val, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
+        print(json.dumps(line))
+        return 0
+
+    # ---------------------------------------------------------------- our arm
+    p = synth.make_config(a.workload, seed=rank_seed(a.seed, rank))       # generated before CUDA is touched (fork pool)
+    os.environ["UNIFRAC_B200_TIMING"] = "1"
+    import torch
+    from paper_2107_05397_b200 import binding
+    binding.load()
+    dev = torch.device("cuda", local_rank)
+    torch.cuda.set_device(dev)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    args = binding.to_device(p, dev)
+    outs = {v: torch.empty(p.n_pairs, dtype=torch.float32 if precision == 0 else torch.float64, device=dev) for v in variants}
+
+    def step():
+        stats = []
+        for v in variants:
+            binding.unifrac_dm(*args, p.n_samples, v, precision, out=outs[v], flags=a.flags)
+            stats.append(binding.unifrac_last_stats())     # waits for the call's stripe kernel (stats event)
+        return stats
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize(dev)
+
+    for _ in range(a.warmup):
+        step()
+    barrier()
+    stop, lines = threading.Event(), []
+    th = threading.Thread(target=clocks_sampler, args=(stop, lines, local_rank), daemon=True)
+    th.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    all_stats = []
+    e0.record()
+    for _ in range(a.steps):
+        all_stats.append(step())
+    e1.record()
+    barrier()
+    stop.set()
+    th.join(timeout=3)
+    flat = [s for st in all_stats for s in st]
+    ms, upd_all = reduce_over_ranks(e0.elapsed_time(e1), float(sum(s["updates_dense"] for s in flat)), world, dev)
+    value = upd_all / (ms * 1e-3)
+
+    # ---------------- end to end through the host-buffer C-ABI call (H2D + D2H inside the timed region)
+    e2e = None
+    if not a.no_e2e:
+        pin = lambda arr: torch.from_numpy(np.ascontiguousarray(arr)).pin_memory().numpy()
+        hp = [pin(x) for x in (p.parent, p.branch_len, p.postorder, p.indptr, p.indices, p.counts)]
+        hout = torch.empty(p.n_pairs, dtype=torch.float32 if precision == 0 else torch.float64).pin_memory().numpy()
+        del outs
+        torch.cuda.empty_cache()
+        barrier()
+        t0 = time.perf_counter()
+        for v in variants:
+            binding.unifrac_dm_host(*hp, p.n_samples, v, precision, out=hout)
+        barrier()
+        t_e2e = time.perf_counter() - t0
+        t_e2e, _ = reduce_over_ranks(t_e2e, 0.0, world, dev)
+        h2d = sum(x.nbytes for x in hp) * len(variants)
+        d2h = hout.nbytes * len(variants)
+        e2e = dict(value=(upd_all / a.steps) / t_e2e, unit=UNIT, h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h),
+                   seconds_per_step=t_e2e)
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    # ---------------- roofline of the dominant kernel (stripe accumulation): plain FP32 ALU work
+    t_stripe = sum(s["ms_stripe"] for s in flat) * 1e-3
+    n_launch = sum(s["stripe_launches"] for s in flat)
+    w_exec = sum(s["updates_executed"] for s in flat)
+    w_inter = sum(s["updates_inter"] for s in flat)
+    w_union = sum(s["updates_union"] for s in flat)
+    achieved = 2.0 * w_exec / t_stripe / 1e12 if t_stripe > 0 else 0.0
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    roofline = dict(bound="alu", achieved=achieved, peak=ALU_PEAK_TFLOPS, unit="TFLOP/s", frac=achieved / ALU_PEAK_TFLOPS,
+                    traffic=None, kernel="k_stripe", launches=n_launch, ms_per_launch=1e3 * t_stripe / max(1, n_launch),
+                    executed_updates_per_launch=w_exec / max(1, n_launch),
+                    peak_source=f"{SM_COUNT} SMs x {FP32_LANES} FP32 lanes x {SM_MAX_GHZ} GHz (sm_max_mhz of MEASURED_PEAKS.json"
+                                f"{'' if peaks else ' fallback'}); 2 FP32 lane-ops (FMNMX+FADD or FADD+FADD) per update",
+                    frac_algorithmic_inter=2.0 * w_inter / t_stripe / 1e12 / ALU_PEAK_TFLOPS if t_stripe > 0 else 0.0,
+                    frac_algorithmic_union=2.0 * w_union / t_stripe / 1e12 / ALU_PEAK_TFLOPS if t_stripe > 0 else 0.0,
+                    stripe_share_of_step=t_stripe / (ms * 1e-3))
+
+    cpu = None
+    if not a.no_cpu_baseline:
+        leg = oracle_leg(p, variants, a.cpu_budget_s)
+        b_emb = flat[0]["branches_embedded"]
+        cpu = dict(value=leg["pairs"] * b_emb / leg["seconds"], unit=UNIT, cores=leg["cores"], kind="oracle",
+                   sample=leg["sample"], seconds=leg["seconds"])
+
+    per_variant = {}
+    for k, v in enumerate(variants):
+        ss = [st[k] for st in all_stats]
+        per_variant["unweighted" if v == 0 else "weighted_normalized"] = dict(
+            ms_total=float(np.mean([s["ms_total"] for s in ss])), ms_plan=float(np.mean([s["ms_plan"] for s in ss])),
+            ms_embed=float(np.mean([s["ms_embed"] for s in ss])), ms_stripe=float(np.mean([s["ms_stripe"] for s in ss])),
+            updates_dense=ss[0]["updates_dense"], updates_executed=ss[0]["updates_executed"],
+            updates_union=ss[0]["updates_union"], updates_inter=ss[0]["updates_inter"],
+            branches_embedded=ss[0]["branches_embedded"], workspace_gb=ss[0]["workspace_bytes"] / 2**30)
+
+    line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=a.steps, warmup=a.warmup, ms_per_step=ms / a.steps,
+                higher_is_better=True, scaling="weak", vs_baseline=None, dtype=dtype, data="synthetic",
+                config=dict(workload=a.workload, n_samples=p.n_samples, n_nodes=p.n_nodes, nnz=p.nnz, seed=a.seed,
+                            variants=list(variants), precision=dtype, flags=a.flags, parallelism=f"replicas x{world}",
+                            l2="inputs larger than L2 (compact embedding >> 126 MB)"),
+                clocks=summarize_clocks(lines), e2e=e2e, gpu_launches=int(sum(s["kernel_launches"] for s in flat)),
+                roofline=roofline, cpu_baseline=cpu, wall=per_variant)
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -8,7 +8,9 @@ one module shared by the CUDA path's tests/bench and the oracle's tests.
 """
 from __future__ import annotations
 
+import os
 from dataclasses import dataclass, field
+
 import numpy as np
 
 
@@ -128,7 +130,7 @@ def _distinct_ranks(k: int, cdf: np.ndarray, rng: np.random.Generator) -> np.nda
     got = np.empty(0, dtype=np.int64)
     while got.shape[0] < k:
         need = k - got.shape[0]
-        m = int(need * 1.5) + 16
+        m = 2 * need + 32
         r = np.searchsorted(cdf, rng.random(m), side="right")
         np.minimum(r, n - 1, out=r)
         allr = np.concatenate([got, r])
@@ -138,8 +140,25 @@ def _distinct_ranks(k: int, cdf: np.ndarray, rng: np.random.Generator) -> np.nda
     return got
 
 
+_TAB = {}          # state inherited by forked workers (read-only)
+
+
+def _sample_rows(lo: int, hi: int):
+    """Rows lo..hi-1.  Sample s uses its own generator default_rng(SeedSequence(seed, spawn_key=(1, s))),
+    so the table does not depend on how the samples are split over worker processes."""
+    t = _TAB
+    idx, cnt = [], []
+    for s in range(lo, hi):
+        rng = np.random.default_rng(np.random.SeedSequence(t["seed"], spawn_key=(1, s)))
+        ranks = _distinct_ranks(int(t["ks"][s]), t["cdf"], rng)
+        cols = np.sort(t["tips"][t["perm"][ranks]])
+        idx.append(cols)
+        cnt.append(t["count_draw"](cols.shape[0], rng))
+    return lo, np.concatenate(idx).astype(np.int32), np.concatenate(cnt).astype(np.int32)
+
+
 def make_table(tips: np.ndarray, n_samples: int, zipf_a: float, k_draw, count_draw,
-               rng: np.random.Generator):
+               rng: np.random.Generator, seed: int = 0, workers: int | None = None):
     n_tips = tips.shape[0]
     perm = rng.permutation(n_tips)                 # rank r -> tips[perm[r]]
     w = np.arange(1, n_tips + 1, dtype=np.float64) ** (-zipf_a)
@@ -149,15 +168,22 @@ def make_table(tips: np.ndarray, n_samples: int, zipf_a: float, k_draw, count_dr
     ks = np.clip(ks, 1, n_tips).astype(np.int64)
     indptr = np.zeros(n_samples + 1, dtype=np.int64)
     np.cumsum(ks, out=indptr[1:])
-    indices = np.empty(int(indptr[-1]), dtype=np.int32)
-    counts = np.empty(int(indptr[-1]), dtype=np.int32)
-    for s in range(n_samples):
-        ranks = _distinct_ranks(int(ks[s]), cdf, rng)
-        cols = np.sort(tips[perm[ranks]])
-        c = count_draw(cols.shape[0], rng)
-        a, b = int(indptr[s]), int(indptr[s + 1])
-        indices[a:b] = cols
-        counts[a:b] = c
+    _TAB.clear()
+    _TAB.update(seed=seed, ks=ks, cdf=cdf, tips=tips, perm=perm, count_draw=count_draw)
+    if workers is None:
+        workers = min(os.cpu_count() or 1, 32) if int(indptr[-1]) > 2_000_000 else 1
+    chunk = 256
+    jobs = [(lo, min(lo + chunk, n_samples)) for lo in range(0, n_samples, chunk)]
+    if workers > 1:
+        import multiprocessing as mp
+        with mp.get_context("fork").Pool(workers) as pool:
+            parts = pool.starmap(_sample_rows, jobs)
+    else:
+        parts = [_sample_rows(lo, hi) for lo, hi in jobs]
+    parts.sort(key=lambda p: p[0])
+    indices = np.concatenate([p[1] for p in parts])
+    counts = np.concatenate([p[2] for p in parts])
+    _TAB.clear()
     return indptr, indices, counts
 
 
@@ -192,7 +218,8 @@ CONFIGS = {
 def make_problem(n_tips: int, n_samples: int, mean_len: float, zipf_a: float, k_draw, count_draw,
                  seed: int = 0, name: str = "custom") -> Problem:
     """RNG = numpy default_rng(seed), consumed in this order: Yule picks, branch lengths,
-    popularity permutation, per-sample feature counts k, then per sample (ranks, counts)."""
+    popularity permutation, per-sample feature counts k; then sample s draws (ranks, counts)
+    from its own default_rng(SeedSequence(seed, spawn_key=(1, s)))."""
     rng = np.random.default_rng(seed)
     parent = yule_parent(n_tips, rng)
     n_nodes = parent.shape[0]
@@ -200,7 +227,7 @@ def make_problem(n_tips: int, n_samples: int, mean_len: float, zipf_a: float, k_
     branch_len[0] = 0.0
     post = dfs_postorder(parent)
     tips = tip_ids(parent)
-    indptr, indices, counts = make_table(tips, n_samples, zipf_a, k_draw, count_draw, rng)
+    indptr, indices, counts = make_table(tips, n_samples, zipf_a, k_draw, count_draw, rng, seed=seed)
     return Problem(parent, branch_len.astype(np.float64), post, indptr, indices, counts, name=name,
                    meta=dict(n_tips=n_tips, seed=seed, mean_len=mean_len, zipf_a=zipf_a))
 

@@ -1,0 +1,46 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (device
+entry point, fp32, default flags): sampled outputs the oracle computes one by one (pair-list
+driver) plus structured pairs (first/last rows, tile-boundary neighbours, last condensed
+element), and properties that hold at any size (range, no NaN)."""
+import numpy as np
+import pytest
+
+from paper_2107_05397_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+
+def _structured_pairs(n):
+    e = [[0, 1], [0, n - 1], [n - 2, n - 1], [127, 128], [0, 128], [127, 255], [128, 129], [0, 127],
+         [n - 129, n - 1], [n // 2, n // 2 + 1], [(n // 128) * 128 - 1, (n // 128) * 128], [1, n - 2]]
+    return np.array([p for p in e if 0 <= p[0] < p[1] < n], dtype=np.int32)
+
+
+@pytest.mark.parametrize("name,n_pairs", [("medium", 20000), ("emp", 20000), ("large", 20000)])
+def test_full_size_sampled_pairs(name, n_pairs):
+    import torch
+    from paper_2107_05397_b200 import binding as B
+    from oracle import oracle as O
+    free, _ = torch.cuda.mem_get_info()
+    if name == "large" and free < 90 * 2**30:
+        pytest.skip("needs ~80 GB of free HBM")
+    p = synth.make_config(name, seed=0)
+    n = p.n_samples
+    pairs = np.concatenate([synth.sample_pairs(n, n_pairs, seed=1), _structured_pairs(n)])
+    idx = torch.from_numpy(synth.condensed_index(n, pairs[:, 0], pairs[:, 1])).cuda()
+    args = B.to_device(p)
+    variants = (0,) if name == "medium" else (0, 1)
+    for variant in variants:
+        want = O.pair_list(p.parent, p.branch_len, p.indptr, p.indices, p.counts, variant, pairs)
+        out = B.unifrac_dm(*args, n, variant, B.FP32)
+        torch.cuda.synchronize()
+        got = out[idx].cpu().numpy().astype(np.float64)
+        lo, hi = float(out.min()), float(out.max())
+        assert 0.0 <= lo and hi <= 1.0 and not bool(torch.isnan(out).any())
+        del out
+        err = np.abs(got - want)
+        rel = err / np.maximum(np.abs(want), 1e-30)
+        ok = (err <= 1e-5 * np.abs(want)) | (err <= 1e-7)
+        assert ok.all(), f"{name} variant {variant}: max rel err {rel.max():.3e}"
+        print(f"{name} variant {variant}: max rel err {rel.max():.3e}, p99.99 {np.quantile(rel, 0.9999):.3e}, "
+              f"min d {want.min():.4f}, pairs {len(want)}")
