@@ -232,7 +232,7 @@ def main():
     # ---------------- roofline of the dominant kernel (stripe accumulation): plain FP32 ALU work
     t_stripe = sum(s["ms_stripe"] for s in flat) * 1e-3
     n_launch = sum(s["stripe_launches"] for s in flat)
-    w_exec = sum(s["updates_executed"] for s in flat)
+    w_exec = sum(s["updates_executed_head"] for s in flat)
     w_inter = sum(s["updates_inter"] for s in flat)
     w_union = sum(s["updates_union"] for s in flat)
     achieved = 2.0 * w_exec / t_stripe / 1e12 if t_stripe > 0 else 0.0
@@ -262,7 +262,11 @@ def main():
         ss = [st[k] for st in all_stats]
         per_variant["unweighted" if v == 0 else "weighted_normalized"] = dict(
             ms_total=float(np.mean([s["ms_total"] for s in ss])), ms_plan=float(np.mean([s["ms_plan"] for s in ss])),
-            ms_embed=float(np.mean([s["ms_embed"] for s in ss])), ms_stripe=float(np.mean([s["ms_stripe"] for s in ss])),
+            ms_embed=float(np.mean([s["ms_embed"] for s in ss])), ms_tail=float(np.mean([s["ms_tail"] for s in ss])),
+            ms_stripe=float(np.mean([s["ms_stripe"] for s in ss])),
+            head_rows=ss[0]["head_rows"], tail_rows=ss[0]["tail_rows"], tail_updates=ss[0]["tail_updates"],
+            tail_entries=ss[0]["tail_entries"], tail_launches=ss[0]["tail_launches"],
+            updates_executed_head=ss[0]["updates_executed_head"],
             updates_dense=ss[0]["updates_dense"], updates_executed=ss[0]["updates_executed"],
             updates_union=ss[0]["updates_union"], updates_inter=ss[0]["updates_inter"],
             branches_embedded=ss[0]["branches_embedded"], workspace_gb=ss[0]["workspace_bytes"] / 2**30)

@@ -52,7 +52,11 @@ typedef enum {
 #define UNIFRAC_FLAG_SKIP_VALIDATION  4u  /* trust the inputs (tree/table checks are skipped)            */
 #define UNIFRAC_FLAG_ABSDIFF          8u  /* stripe kernel accumulates |u~_i - u~_j| over rows present in
                                              EITHER tile (direct form) instead of min(u~_i,u~_j) over rows
-                                             present in BOTH (separable form, I2-I5)            */
+                                             present in BOTH (separable form, I2-I5); implies
+                                             NO_TAIL                                                      */
+#define UNIFRAC_FLAG_NO_TAIL         16u  /* every branch goes through the dense stripe kernel (no sparse
+                                             tail scatter)                 */
+#define UNIFRAC_FLAG_ALL_TAIL        32u  /* debug: every branch goes through the sparse tail scatter       */
 
 /* CSR table, rows = samples, columns = tip NODE ids (reading Q6). */
 typedef struct {
@@ -117,21 +121,27 @@ typedef struct {
     uint64_t updates_dense;      /* W_dense = P * B_emb           (the metric's "pair x branch")      */
     uint64_t updates_union;      /* W_union = sum_v [C(N,2) - C(N-n_v,2)]                             */
     uint64_t updates_inter;      /* W_inter = sum_v C(n_v,2)                                          */
-    uint64_t updates_executed;   /* (pair, row) updates the stripe kernel actually executed           */
+    uint64_t updates_executed;   /* (pair, branch) updates actually executed: head (stripe) + tail       */
+    uint64_t updates_executed_head; /* ... by the stripe kernel (head branches)                          */
+    uint64_t head_rows;          /* branches handled by the dense stripe kernel                       */
+    uint64_t tail_rows;          /* branches handled by the sparse tail scatter                       */
+    uint64_t tail_updates;       /* sum over tail branches of C(n_v,2) = RED.ADDs issued               */
+    uint64_t tail_entries;       /* sum over tail branches of n_v = (sample, value) list entries       */
     uint64_t rows_staged;        /* rows the producer staged into shared memory, over all tile pairs  */
     uint64_t embed_rows;         /* sum over sample tiles of non-empty rows (compact embedding rows)  */
     uint64_t workspace_bytes;    /* device bytes requested from the allocator                         */
     uint32_t n_tile_pairs;       /* 128x128 tile pairs in the upper triangle                          */
     uint32_t n_levels;           /* tree depth levels                                                 */
     uint32_t stripe_launches;    /* stripe-kernel launches in this call                               */
+    uint32_t tail_launches;      /* tail-scatter launches (one per L2-resident super tile)             */
     uint32_t kernel_launches;    /* all kernel launches in this call                                  */
-    float ms_plan, ms_embed, ms_stripe, ms_total;
+    float ms_plan, ms_embed, ms_tail, ms_stripe, ms_total;
 } unifrac_stats_t;
 int unifrac_last_stats(unifrac_stats_t *out);
 
 const char *unifrac_status_string(int status);
 const char *unifrac_last_cuda_error(void);   /* text of the last CUDA error seen by this thread  */
-int unifrac_abi_version(void);               /* 1                                                */
+int unifrac_abi_version(void);               /* 2                                                */
 
 #ifdef __cplusplus
 }

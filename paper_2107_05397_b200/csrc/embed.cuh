@@ -54,24 +54,22 @@ __global__ void __launch_bounds__(1024)
 k_row_flags(int n, const int32_t* __restrict__ parent, const double* __restrict__ len,
             const uint32_t* __restrict__ cnt, int Wb, uint32_t* __restrict__ flags /*[tile][nwords]*/,
             uint32_t nwords, int tile0, uint8_t* __restrict__ qtmp /*[tiles_in_batch][n]*/,
-            uint32_t* __restrict__ nv)
+            const uint8_t* __restrict__ cls /*[n] 1 = head row (stripe kernel), others are not flagged*/)
 {
     __shared__ uint32_t q_sm[32];
     int w = blockIdx.x, tb = blockIdx.y;
     int wv = threadIdx.x >> 5, lane = threadIdx.x & 31;
     int v = w * 32 + wv;
-    bool valid = v < n && parent[v] >= 0 && len[v] > 0.0;
+    bool valid = v < n && cls[v] == 1;
     uint4 c = make_uint4(0, 0, 0, 0);
     if (valid) c = reinterpret_cast<const uint4*>(cnt + (size_t)v * Wb + (size_t)tb * TILE)[lane];
     int nz = (c.x != 0) + (c.y != 0) + (c.z != 0) + (c.w != 0);
     uint32_t b = __ballot_sync(0xffffffffu, nz != 0);
     uint32_t q = ((b & 0x000000ffu) ? 1u : 0u) | ((b & 0x0000ff00u) ? 2u : 0u) |
                  ((b & 0x00ff0000u) ? 4u : 0u) | ((b & 0xff000000u) ? 8u : 0u);
-    for (int o = 16; o; o >>= 1) nz += __shfl_xor_sync(0xffffffffu, nz, o);
     if (lane == 0) {
         q_sm[wv] = q;
         if (v < n) qtmp[(size_t)tb * n + v] = (uint8_t)q;
-        if (nz) atomicAdd(&nv[v], (uint32_t)nz);
     }
     __syncthreads();
     if (threadIdx.x < 32) {
@@ -125,10 +123,8 @@ __global__ void __launch_bounds__(256)
 k_compact(int n, const double* __restrict__ len, const uint32_t* __restrict__ cnt, int Wb,
           const uint32_t* __restrict__ flags, const uint32_t* __restrict__ rank, uint32_t nwords, int tile0,
           const unsigned long long* __restrict__ Tsum, int n_samples, int weighted,
-          T* const* __restrict__ tileE, uint8_t* const* __restrict__ tileQ, const uint8_t* __restrict__ qtmp,
-          double* __restrict__ sums)
+          T* const* __restrict__ tileE, uint8_t* const* __restrict__ tileQ, const uint8_t* __restrict__ qtmp)
 {
-    __shared__ double red[8][TILE];
     int tb = blockIdx.y, tile = tile0 + tb;
     int wv = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t* f = flags + (size_t)tile * nwords;
@@ -141,7 +137,6 @@ k_compact(int n, const double* __restrict__ len, const uint32_t* __restrict__ cn
         int s = tile * TILE + lane * 4 + e;
         Tl[e] = s < n_samples ? (double)Tsum[s] : 1.0;
     }
-    double acc[4] = {0.0, 0.0, 0.0, 0.0};
     uint32_t w0 = blockIdx.x * COMPACT_WORDS;
     uint32_t w1 = w0 + COMPACT_WORDS; if (w1 > nwords) w1 = nwords;
     for (uint32_t w = w0; w < w1; ++w) {
@@ -169,18 +164,8 @@ k_compact(int n, const double* __restrict__ len, const uint32_t* __restrict__ cn
             }
             double back[4];
             Vec4<T>::store(E + (size_t)r * TILE + lane * 4, x0, x1, x2, x3, back);
-            acc[0] += back[0]; acc[1] += back[1]; acc[2] += back[2]; acc[3] += back[3];
             if (lane == 0) Q[r] = qtmp[(size_t)tb * n + v];
         }
-    }
-#pragma unroll
-    for (int e = 0; e < 4; ++e) red[wv][lane * 4 + e] = acc[e];
-    __syncthreads();
-    if (threadIdx.x < TILE) {
-        double s = 0.0;
-#pragma unroll
-        for (int k = 0; k < 8; ++k) s += red[k][threadIdx.x];
-        if (s != 0.0) atomicAdd(&sums[(size_t)tile * TILE + threadIdx.x], s);
     }
 }
 

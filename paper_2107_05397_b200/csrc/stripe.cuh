@@ -75,6 +75,7 @@ struct StripeParams {
     double* scratch;              // [grid][64][256] fp64 partial sums
     unsigned long long* stats;    // [0] rows executed by consumer warps, [1] rows staged
     const void* zero_row;         // 128 zero values of T (16-byte aligned)
+    int add_out;                  // min form: out[] already holds the tail branches' sum of min(u~_a,u~_b) (tail.cuh)
 };
 
 template <typename T>
@@ -312,6 +313,7 @@ k_stripe(const StripeParams P)
                 if (gi < gj && gj < N) {
                     const double ss = si + sj[b];
                     double num, den;
+                    if (FORM == FORM_MIN && P.add_out) tot += (double)reinterpret_cast<const T*>(P.out)[rowbase + gj];
                     if (FORM == FORM_MIN) {
                         num = ss - 2.0 * tot;
                         den = P.weighted ? ss : ss - tot;

@@ -1,0 +1,296 @@
+// tail.cuh -- the sparse half of the sparse-aware split ("sparse-aware optimizations";
+// the mechanism is ours).
+//
+// Branches are classified by n_v = number of samples present below them:
+//   head  (n_v large)  : dense enough that the register-tiled stripe kernel (stripe.cuh) is the
+//                        cheaper way to cover all N(N-1)/2 pairs;
+//   tail  (n_v small)  : only the C(n_v,2) pairs of samples that are BOTH present contribute
+//                        min(u~_a, u~_b) to M_ab (identities I3/I5), so the branch is stored as a
+//                        sorted list of (sample, u~) entries and its pair contributions are
+//                        scattered straight into the condensed matrix with fp32/fp64 RED.ADD.
+// The scatter is ordered by output "super tiles" (ranges of SUP samples x SUP samples whose
+// condensed rows fit the L2 cache), one launch per super tile, so the atomics resolve in L2
+// (measured: 1.9e11 RED/s L2-resident vs 2e10 RED/s when the footprint spills to HBM).
+//
+// Steps:  bit-packed presence up the tree (a-1/a-2 on bits, BASELINE.json:5 "presence bits,
+// bit-packed in 32/64-sample words ... level by level")  ->  n_v (popcount)  ->  classification
+// ->  per-batch fill of the tail lists  ->  super-tile segment offsets  ->  scatter.
+#pragma once
+#include "common.cuh"
+
+namespace ufb {
+
+enum : uint8_t { CLS_NONE = 0, CLS_HEAD = 1, CLS_TAIL = 2 };
+
+// ------------------------------------------------------------------ presence bits (all samples at once)
+// bits[v][w] bit b  <=>  sample 32*w + b has a positive count on some tip below v
+__global__ void k_bits_scatter(int n_samples, const int64_t* __restrict__ indptr, const int32_t* __restrict__ indices,
+                               const int32_t* __restrict__ counts, uint32_t* __restrict__ bits, uint32_t NW)
+{
+    int s = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    int lane = threadIdx.x & 31;
+    if (s >= n_samples) return;
+    long long lo = indptr[s], hi = indptr[s + 1];
+    const uint32_t w = (uint32_t)s >> 5, m = 1u << (s & 31);
+    for (long long k = lo + lane; k < hi; k += 32)
+        if (counts[k] > 0) atomicOr(&bits[(size_t)indices[k] * NW + w], m);
+}
+
+// parents of one depth level OR their children's rows (uint4 = 128 samples per thread); NW4 = NW/4
+__global__ void k_bits_pull(const int32_t* __restrict__ nodes, int n_nodes_level, int skip_node,
+                            const uint32_t* __restrict__ child_off, const int32_t* __restrict__ child_idx,
+                            uint4* __restrict__ bits, uint32_t NW4)
+{
+    long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    long long q = gid / NW4;
+    uint32_t ch = (uint32_t)(gid - q * NW4);
+    if (q >= n_nodes_level) return;
+    int v = nodes[q];
+    if (v == skip_node) return;
+    uint4 acc = make_uint4(0, 0, 0, 0);
+    for (uint32_t k = child_off[v]; k < child_off[v + 1]; ++k) {
+        uint4 c = bits[(size_t)child_idx[k] * NW4 + ch];
+        acc.x |= c.x; acc.y |= c.y; acc.z |= c.z; acc.w |= c.w;
+    }
+    bits[(size_t)v * NW4 + ch] = acc;
+}
+
+// n_v = popcount of row v (one warp per node); rows of the root / zero-length branches count as 0
+__global__ void k_bits_count(int n, const int32_t* __restrict__ parent, const double* __restrict__ len,
+                             const uint4* __restrict__ bits, uint32_t NW4, uint32_t* __restrict__ nv)
+{
+    int v = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    int lane = threadIdx.x & 31;
+    if (v >= n) return;
+    uint32_t c = 0;
+    if (parent[v] >= 0 && len[v] > 0.0) {
+        for (uint32_t k = lane; k < NW4; k += 32) {
+            uint4 x = bits[(size_t)v * NW4 + k];
+            c += __popc(x.x) + __popc(x.y) + __popc(x.z) + __popc(x.w);
+        }
+    }
+    for (int o = 16; o; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
+    if (lane == 0) nv[v] = c;
+}
+
+// head / tail rule, per branch (costs are additive over branches, so the per-branch rule is optimal):
+//   tail  iff  C(n_v,2) * tail_cost  <  P * head_cost      (costs in seconds per update)
+// tcnt[v] = n_v for tail branches else 0 (scanned into the list offsets); counters[0..3] = head rows,
+// tail rows, tail pair updates, tail entries.
+__global__ void k_classify(int n, const uint32_t* __restrict__ nv, double pairs_times_ratio, uint32_t force,
+                           uint8_t* __restrict__ cls, uint32_t* __restrict__ tcnt, unsigned long long* __restrict__ counters)
+{
+    int v = blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned long long h = 0, t = 0, tu = 0, te = 0;
+    if (v < n) {
+        unsigned long long k = nv[v];
+        uint8_t c = CLS_NONE;
+        if (k) {
+            double c2 = 0.5 * (double)k * (double)(k - 1);
+            bool tail = force == 2 ? true : force == 1 ? false : (c2 < pairs_times_ratio);
+            c = tail ? CLS_TAIL : CLS_HEAD;
+            if (tail) { t = 1; tu = k * (k - 1) / 2; te = k; } else h = 1;
+        }
+        cls[v] = c;
+        tcnt[v] = c == CLS_TAIL ? (uint32_t)k : 0u;
+    }
+    for (int o = 16; o; o >>= 1) {
+        h += __shfl_xor_sync(0xffffffffu, h, o);  t += __shfl_xor_sync(0xffffffffu, t, o);
+        tu += __shfl_xor_sync(0xffffffffu, tu, o); te += __shfl_xor_sync(0xffffffffu, te, o);
+    }
+    if ((threadIdx.x & 31) == 0 && (h | t)) {
+        atomicAdd(&counters[0], h); atomicAdd(&counters[1], t); atomicAdd(&counters[2], tu); atomicAdd(&counters[3], te);
+    }
+}
+
+// ------------------------------------------------------------------ tail lists, filled batch by batch
+// One warp per node; tail rows append (sample id, u~) for the samples of this batch, in sample order.
+// 64-bit list offsets: tptr[v] (exclusive scan of tcnt) + cursor[v] (entries written by earlier batches).
+template <typename T>
+__global__ void k_tail_fill(int n, const uint8_t* __restrict__ cls, const double* __restrict__ len,
+                            const uint32_t* __restrict__ cnt, int Wb, int s0, int s1,
+                            const unsigned long long* __restrict__ Tsum, int weighted,
+                            const uint32_t* __restrict__ tptr, uint32_t* __restrict__ cursor,
+                            uint32_t* __restrict__ ts, T* __restrict__ tv)
+{
+    int v = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    int lane = threadIdx.x & 31;
+    if (v >= n || cls[v] != CLS_TAIL) return;
+    const double l = len[v];
+    uint32_t pos = tptr[v] + cursor[v];
+    const uint32_t pos0 = pos;
+    const int W = s1 - s0;
+    const uint32_t* row = cnt + (size_t)v * Wb;
+    for (int c0 = 0; c0 < W; c0 += 32) {
+        int c = c0 + lane;
+        uint32_t x = c < W ? row[c] : 0u;
+        uint32_t m = __ballot_sync(0xffffffffu, x != 0);
+        if (!m) continue;
+        if (x) {
+            uint32_t p = pos + __popc(m & ((1u << lane) - 1u));
+            double val = weighted ? l * ((double)x / (double)Tsum[s0 + c]) : l;
+            ts[p] = (uint32_t)(s0 + c);
+            tv[p] = (T)val;
+        }
+        pos += __popc(m);
+    }
+    if (lane == 0 && pos != pos0) cursor[v] += pos - pos0;
+}
+
+// seg[v][k] = number of entries of row v with sample id < k*SUP, k = 0..nsup   (thread per (v,k))
+__global__ void k_tail_seg(int n, const uint32_t* __restrict__ tptr, const uint32_t* __restrict__ ts,
+                           int SUP, int nsup, uint32_t* __restrict__ seg)
+{
+    long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    long long v = gid / (nsup + 1);
+    int k = (int)(gid - v * (nsup + 1));
+    if (v >= n) return;
+    const uint32_t lo0 = tptr[v], hi0 = tptr[v + 1];
+    uint32_t lo = lo0, hi = hi0;
+    const uint32_t key = (uint32_t)k * (uint32_t)SUP;
+    while (lo < hi) {
+        uint32_t mid = lo + ((hi - lo) >> 1);
+        if (ts[mid] < key) lo = mid + 1; else hi = mid;
+    }
+    seg[(size_t)v * (nsup + 1) + k] = lo - lo0;
+}
+
+// ------------------------------------------------------------------ per-sample side sums (deterministic)
+// part[chunk][c] = sum over the nodes v of the chunk of u~_{s0+c, v}; lane <-> sample, warp <-> chunk.
+template <typename T>
+__global__ void k_side_sums_part(int n, const int32_t* __restrict__ parent, const double* __restrict__ len,
+                                 const uint32_t* __restrict__ cnt, int Wb, int s0, int s1,
+                                 const unsigned long long* __restrict__ Tsum, int weighted, int n_chunks,
+                                 double* __restrict__ part)
+{
+    const int strip = blockIdx.x;                       // 32 samples
+    const int chunk = blockIdx.y * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (chunk >= n_chunks) return;
+    const int c = strip * 32 + lane;
+    const bool ok = s0 + c < s1;
+    const double Ts = ok ? (double)Tsum[s0 + c] : 1.0;
+    const long long per = ((long long)n + n_chunks - 1) / n_chunks;
+    long long v0 = chunk * per, v1 = v0 + per;
+    if (v1 > n) v1 = n;
+    double acc = 0.0;
+    constexpr int U = 8;                                 // loads in flight per lane
+    for (long long vb = v0; vb < v1; vb += U) {
+        uint32_t x[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) x[u] = vb + u < v1 ? cnt[(size_t)(vb + u) * Wb + c] : 0u;
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            if (x[u]) {
+                const long long v = vb + u;
+                const double l = len[v];
+                if (parent[v] >= 0 && l > 0.0) {
+                    double val = weighted ? l * ((double)x[u] / Ts) : l;
+                    acc += (double)(T)val;
+                }
+            }
+        }
+    }
+    if (ok) part[(size_t)chunk * Wb + c] = acc;
+}
+__global__ void k_side_sums_reduce(int W, int Wb, int n_chunks, const double* __restrict__ part, int s0,
+                                   double* __restrict__ sums)
+{
+    int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= W) return;
+    double s = 0.0;
+    for (int k = 0; k < n_chunks; ++k) s += part[(size_t)k * Wb + c];
+    sums[s0 + c] = s;
+}
+
+// ------------------------------------------------------------------ the scatter
+// One launch per super tile (SI <= SJ).  A warp takes 32 consecutive nodes; rows whose cross product in
+// this super tile is small are done one per lane, larger ones by the whole warp (lanes over the longer
+// list).  out[idx(a,b)] += min(u~_a, u~_b)   for a in range SI, b in range SJ, a < b.
+template <typename T>
+__device__ __forceinline__ void red_add(T* p, T v) { atomicAdd(p, v); }
+
+struct TailParams {
+    const uint32_t* tptr;   // [n+1]
+    const uint32_t* seg;    // [n][nsup+1]
+    const uint32_t* ts;     // sample ids
+    const void* tv;         // values (T)
+    const uint32_t* tcnt;   // [n] (0 for non-tail rows)
+    int n, nsup, SI, SJ;
+    long long N;
+    void* out;
+    unsigned int* counter;  // dynamic chunk queue (one word per launch)
+};
+
+constexpr int TAIL_SMALL = 8;
+
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_tail_scatter(const TailParams P)
+{
+    const int lane = threadIdx.x & 31;
+    const T* tv = reinterpret_cast<const T*>(P.tv);
+    T* out = reinterpret_cast<T*>(P.out);
+    const long long N = P.N;
+    const int nchunks = (P.n + 31) >> 5;
+    const bool diag = P.SI == P.SJ;
+    for (;;) {
+        int chunk = 0;
+        if (lane == 0) chunk = (int)atomicAdd(P.counter, 1u);
+        chunk = __shfl_sync(0xffffffffu, chunk, 0);
+        if (chunk >= nchunks) break;
+        const int v = chunk * 32 + lane;
+        uint32_t i0 = 0, i1 = 0, j0 = 0, j1 = 0, base = 0;
+        if (v < P.n && P.tcnt[v]) {
+            const uint32_t* sg = P.seg + (size_t)v * (P.nsup + 1);
+            i0 = sg[P.SI]; i1 = sg[P.SI + 1];
+            if (diag) { j0 = i0; j1 = i1; } else { j0 = sg[P.SJ]; j1 = sg[P.SJ + 1]; }
+            base = P.tptr[v];
+        }
+        const uint32_t nI = i1 - i0, nJ = j1 - j0;
+        const uint32_t work = diag ? (nI * (nI - (nI ? 1u : 0u))) / 2u : nI * nJ;
+        // ---- small rows: one per lane
+        if (work && work <= (uint32_t)TAIL_SMALL) {
+            for (uint32_t k = i0; k < i1; ++k) {
+                const long long a = P.ts[base + k];
+                const T va = tv[base + k];
+                const long long rowoff = a * (2 * N - a - 1) / 2 - a - 1;
+                for (uint32_t l = diag ? k + 1 : j0; l < j1; ++l) {
+                    const T vb = tv[base + l];
+                    red_add(out + rowoff + P.ts[base + l], va < vb ? va : vb);
+                }
+            }
+        }
+        // ---- larger rows: whole warp, lanes over the longer list, loop over the shorter one
+        uint32_t big = __ballot_sync(0xffffffffu, work > (uint32_t)TAIL_SMALL);
+        while (big) {
+            const int src = __ffs(big) - 1;
+            big &= big - 1;
+            const uint32_t bi0 = __shfl_sync(0xffffffffu, i0, src), bi1 = __shfl_sync(0xffffffffu, i1, src);
+            const uint32_t bj0 = __shfl_sync(0xffffffffu, j0, src), bj1 = __shfl_sync(0xffffffffu, j1, src);
+            const uint32_t bb = __shfl_sync(0xffffffffu, base, src);
+            const bool lanesJ = diag || (bj1 - bj0) >= (bi1 - bi0);       // lane entries are the b's (else the a's)
+            const uint32_t p0 = lanesJ ? bj0 : bi0, p1 = lanesJ ? bj1 : bi1;   // lane list
+            const uint32_t q0 = lanesJ ? bi0 : bj0, q1 = lanesJ ? bi1 : bj1;   // loop list
+            for (uint32_t l0 = p0; l0 < p1; l0 += 32) {
+                const uint32_t l = l0 + lane;
+                const bool lv = l < p1;
+                const long long se = lv ? (long long)P.ts[bb + l] : 0;
+                const T ve = lv ? tv[bb + l] : (T)0;
+                const long long rowoff_e = se * (2 * N - se - 1) / 2 - se - 1;    // used when the lane entry is the a
+                const uint32_t kend = diag ? (l0 + 32 < q1 ? l0 + 32 : q1) : q1;  // diag: only k < l
+                for (uint32_t k = q0; k < kend; ++k) {
+                    const long long sf = P.ts[bb + k];        // warp-uniform (broadcast) loads
+                    const T vf = tv[bb + k];
+                    if (lv && (!diag || k < l)) {
+                        const T m = ve < vf ? ve : vf;
+                        if (lanesJ) red_add(out + (sf * (2 * N - sf - 1) / 2 - sf - 1) + se, m);
+                        else        red_add(out + rowoff_e + sf, m);
+                    }
+                }
+            }
+        }
+    }
+}
+
+}  // namespace ufb

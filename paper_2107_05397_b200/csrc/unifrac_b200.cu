@@ -5,6 +5,7 @@
 #include "common.cuh"
 #include "plan.cuh"
 #include "embed.cuh"
+#include "tail.cuh"
 #include "stripe.cuh"
 
 #include <cstdio>
@@ -60,10 +61,10 @@ struct Arena {
 inline int cdiv(long long a, long long b) { return (int)((a + b - 1) / b); }
 
 struct Timer {
-    bool on; cudaStream_t s; cudaEvent_t ev[5]; int n = 0;
+    bool on; cudaStream_t s; cudaEvent_t ev[8]; int n = 0;
     Timer(bool on_, cudaStream_t s_) : on(on_), s(s_) { if (on) for (auto& e : ev) cudaEventCreate(&e); }
     ~Timer() { if (on) for (auto& e : ev) cudaEventDestroy(e); }
-    void mark() { if (on && n < 5) cudaEventRecord(ev[n++], s); }
+    void mark() { if (on && n < 8) cudaEventRecord(ev[n++], s); }
     float ms(int a, int b) { float m = 0; if (on && b < n) cudaEventElapsedTime(&m, ev[a], ev[b]); return m; }
 };
 
@@ -138,6 +139,48 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     k_child_fill<<<cdiv(n, TB), TB, 0, st>>>(n, parent, child_cur, child_idx); CU_LAUNCH(); ++launches;
     tm.mark();
 
+    // ------------------------------------------------------------------ a-1/a-2 on presence bits -> n_v -> head/tail classes
+    const uint32_t NW = ((uint32_t)cdiv(N, 32) + 3u) & ~3u, NW4 = NW / 4;
+    uint32_t* nv = A.get_n<uint32_t>(n);
+    uint8_t* cls = A.get_n<uint8_t>(n);
+    uint32_t* tcnt = A.get_n<uint32_t>(n);
+    uint32_t* tptr = A.get_n<uint32_t>((size_t)n + 1);
+    unsigned long long* work = A.get_n<unsigned long long>(16);
+    CU(cudaMemsetAsync(work, 0, sizeof(unsigned long long) * 16, st));
+    {
+        uint32_t* bits = A.get_n<uint32_t>((size_t)n * NW);
+        CU(cudaMemsetAsync(bits, 0, sizeof(uint32_t) * (size_t)n * NW, st));
+        k_bits_scatter<<<cdiv((long long)N * 32, TB), TB, 0, st>>>(N, tab.indptr, tab.indices, tab.counts, bits, NW); CU_LAUNCH(); ++launches;
+        for (int d = n_levels - 1; d >= 0; --d) {
+            const uint32_t cntl = h_hist[d];
+            if (!cntl) continue;
+            k_bits_pull<<<cdiv((long long)cntl * NW4, TB), TB, 0, st>>>(level_nodes + h_off[d], (int)cntl, root, child_off, child_idx,
+                                                                       reinterpret_cast<uint4*>(bits), NW4);
+            CU_LAUNCH(); ++launches;
+        }
+        k_bits_count<<<cdiv((long long)n * 32, TB), TB, 0, st>>>(n, parent, len, reinterpret_cast<const uint4*>(bits), NW4, nv); CU_LAUNCH(); ++launches;
+    }
+    k_work_counts<<<cdiv(n, TB), TB, 0, st>>>(n, nv, (unsigned long long)N, work); CU_LAUNCH(); ++launches;
+    // per-branch rule: tail iff C(n_v,2) / R_tail < P / R_head; the ratio
+    // R_tail / R_head is measured (RED.ADD rate in L2 vs dense stripe rate) and can be overridden
+    double ratio = 0.022;
+    if (const char* e = getenv("UNIFRAC_B200_TAIL_RATIO")) ratio = atof(e);
+    uint32_t force = 0;
+    if (flags & (UNIFRAC_FLAG_NO_TAIL | UNIFRAC_FLAG_ABSDIFF | UNIFRAC_FLAG_LITERAL)) force = 1;
+    else if (flags & UNIFRAC_FLAG_ALL_TAIL) force = 2;
+    k_classify<<<cdiv(n, TB), TB, 0, st>>>(n, nv, 0.5 * (double)N * (double)(N - 1) * ratio, force, cls, tcnt, work + 8); CU_LAUNCH(); ++launches;
+    k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>(n, tcnt, tptr); CU_LAUNCH(); ++launches;
+    unsigned long long h_work[12];
+    CU(cudaMemcpyAsync(h_work, work, sizeof(h_work), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    const unsigned long long head_rows = h_work[8], tail_rows = h_work[9], tail_updates = h_work[10], tail_entries = h_work[11];
+    if (tail_entries >= (1ull << 32)) throw StatusFail{UNIFRAC_ERR_UNSUPPORTED};
+    uint32_t* ts = A.get_n<uint32_t>(tail_entries ? tail_entries : 1);
+    T* tv = A.get_n<T>(tail_entries ? tail_entries : 1);
+    uint32_t* tcursor = A.get_n<uint32_t>(n);
+    CU(cudaMemsetAsync(tcursor, 0, sizeof(uint32_t) * n, st));
+    tm.mark();
+
     // ------------------------------------------------------------------ a-1 .. a-4 embedding, per sample batch
     const int n_tiles = cdiv(N, TILE);
     const uint32_t nwords = (uint32_t)cdiv(n, 32);
@@ -153,11 +196,11 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     uint32_t* rrank = A.get_n<uint32_t>((size_t)n_tiles * nwords);
     uint32_t* rows = A.get_n<uint32_t>(n_tiles);
     uint8_t* qtmp = A.get_n<uint8_t>((size_t)tiles_per_batch * n);
-    uint32_t* nv = A.get_n<uint32_t>(n);
     double* sums = A.get_n<double>((size_t)n_tiles * TILE);
+    const int n_chunks = 512;
+    double* sums_part = A.get_n<double>((size_t)n_chunks * Wb);
     T** tileE = A.get_n<T*>(n_tiles);
     uint8_t** tileQ = A.get_n<uint8_t*>(n_tiles);
-    CU(cudaMemsetAsync(nv, 0, sizeof(uint32_t) * n, st));
     CU(cudaMemsetAsync(sums, 0, sizeof(double) * (size_t)n_tiles * TILE, st));
     std::vector<uint32_t> h_rows(n_tiles);
     std::vector<T*> h_tileE(n_tiles);
@@ -177,7 +220,14 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             k_level_pull<<<cdiv(threads, TB), TB, 0, st>>>(level_nodes + h_off[d], (int)cntl, root, child_off, child_idx, cnt, Wb);
             CU_LAUNCH(); ++launches;
         }
-        k_row_flags<<<dim3(nwords, tb), 1024, 0, st>>>(n, parent, len, cnt, Wb, rflags, nwords, t0, qtmp, nv); CU_LAUNCH(); ++launches;
+        k_side_sums_part<T><<<dim3(cdiv(s1 - s0, 32), cdiv(n_chunks, 8)), 256, 0, st>>>(n, parent, len, cnt, Wb, s0, s1, Tsum, weighted,
+                                                                                        n_chunks, sums_part); CU_LAUNCH(); ++launches;
+        k_side_sums_reduce<<<cdiv(s1 - s0, TB), TB, 0, st>>>(s1 - s0, Wb, n_chunks, sums_part, s0, sums); CU_LAUNCH(); ++launches;
+        if (tail_rows) {
+            k_tail_fill<T><<<cdiv((long long)n * 32, TB), TB, 0, st>>>(n, cls, len, cnt, Wb, s0, s1, Tsum, weighted, tptr, tcursor, ts, tv);
+            CU_LAUNCH(); ++launches;
+        }
+        k_row_flags<<<dim3(nwords, tb), 1024, 0, st>>>(n, parent, len, cnt, Wb, rflags, nwords, t0, qtmp, cls); CU_LAUNCH(); ++launches;
         k_rank_scan<<<tb, 1024, 0, st>>>(rflags, rrank, nwords, t0, rows); CU_LAUNCH(); ++launches;
         CU(cudaMemcpyAsync(h_rows.data() + t0, rows + t0, sizeof(uint32_t) * tb, cudaMemcpyDeviceToHost, st));
         CU(cudaStreamSynchronize(st));
@@ -191,16 +241,39 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         CU(cudaMemcpyAsync(tileE + t0, h_tileE.data() + t0, sizeof(T*) * tb, cudaMemcpyHostToDevice, st));
         CU(cudaMemcpyAsync(tileQ + t0, h_tileQ.data() + t0, sizeof(uint8_t*) * tb, cudaMemcpyHostToDevice, st));
         k_compact<T><<<dim3(cdiv(nwords, COMPACT_WORDS), tb), 256, 0, st>>>(n, len, cnt, Wb, rflags, rrank, nwords, t0, Tsum, N,
-                                                                             weighted, tileE, tileQ, qtmp, sums);
+                                                                             weighted, tileE, tileQ, qtmp);
         CU_LAUNCH(); ++launches;
         CU(cudaStreamSynchronize(st));   // h_tileE/h_tileQ staging copies are done; safe to reuse cnt
     }
-    unsigned long long* work = A.get_n<unsigned long long>(8);
-    CU(cudaMemsetAsync(work, 0, sizeof(unsigned long long) * 8, st));
-    k_work_counts<<<cdiv(n, TB), TB, 0, st>>>(n, nv, (unsigned long long)N, work); CU_LAUNCH(); ++launches;
-    unsigned long long h_work[4];
-    CU(cudaMemcpyAsync(h_work, work, sizeof(h_work), cudaMemcpyDeviceToHost, st));
-    CU(cudaStreamSynchronize(st));
+    tm.mark();
+
+    // ------------------------------------------------------------------ a-5 (tail branches): scatter into the condensed matrix
+    unsigned tail_launches = 0;
+    if (tail_rows) {
+        // super tiles: SUP x SUP samples whose condensed row segments (SUP * SUP * sizeof(T)) stay L2-resident
+        size_t l2_budget = (size_t)48 << 20;
+        if (const char* e = getenv("UNIFRAC_B200_TAIL_L2_MB")) l2_budget = (size_t)atoll(e) << 20;
+        int SUP = 128;
+        while ((size_t)(SUP + 128) * (SUP + 128) * sizeof(T) <= l2_budget) SUP += 128;
+        const int nsup = cdiv(N, SUP);
+        uint32_t* seg = A.get_n<uint32_t>((size_t)n * (nsup + 1));
+        k_tail_seg<<<cdiv((long long)n * (nsup + 1), TB), TB, 0, st>>>(n, tptr, ts, SUP, nsup, seg); CU_LAUNCH(); ++launches;
+        CU(cudaMemsetAsync(out, 0, sizeof(T) * ((size_t)N * (N - 1) / 2), st));
+        const int n_launch = nsup * (nsup + 1) / 2;
+        unsigned int* tcounters = A.get_n<unsigned int>(n_launch);
+        CU(cudaMemsetAsync(tcounters, 0, sizeof(unsigned int) * n_launch, st));
+        int dev = 0, n_sm = 0;
+        CU(cudaGetDevice(&dev));
+        CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+        TailParams TP{};
+        TP.tptr = tptr; TP.seg = seg; TP.ts = ts; TP.tv = tv; TP.tcnt = tcnt; TP.n = n; TP.nsup = nsup; TP.N = N; TP.out = out;
+        int li = 0;
+        for (int si = 0; si < nsup; ++si)
+            for (int sj = si; sj < nsup; ++sj) {
+                TP.SI = si; TP.SJ = sj; TP.counter = tcounters + li++;
+                k_tail_scatter<T><<<n_sm * 8, 256, 0, st>>>(TP); CU_LAUNCH(); ++launches; ++tail_launches;
+            }
+    }
     tm.mark();
 
     // ------------------------------------------------------------------ a-5 / a-6 stripe accumulation + finalize
@@ -217,6 +290,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     uint32_t* counter = reinterpret_cast<uint32_t*>(work + 6);
 
     StripeParams P{};
+    P.add_out = tail_rows ? 1 : 0;
     P.tileE = reinterpret_cast<const void* const*>(tileE);
     P.tileQ = tileQ; P.flags = rflags; P.rank = rrank; P.nwords = nwords;
     P.pairs = pairs; P.n_pairs = n_pairs; P.counter = counter; P.sums = sums;
@@ -253,6 +327,8 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     g_stats.updates_union = h_work[1];
     g_stats.updates_inter = h_work[2];
     g_stats.embed_rows = embed_rows;
+    g_stats.head_rows = head_rows; g_stats.tail_rows = tail_rows; g_stats.tail_updates = tail_updates; g_stats.tail_entries = tail_entries;
+    g_stats.tail_launches = tail_launches;
     g_stats.n_tile_pairs = n_pairs;
     g_stats.n_levels = (uint32_t)n_levels;
     g_stats.stripe_launches = stripe_launches;
@@ -261,7 +337,8 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     g_stats.workspace_bytes = A.total;
     if (timing) {
         CU(cudaStreamSynchronize(st));
-        g_stats.ms_plan = tm.ms(0, 1); g_stats.ms_embed = tm.ms(1, 2); g_stats.ms_stripe = tm.ms(2, 3); g_stats.ms_total = tm.ms(0, 3);
+        g_stats.ms_plan = tm.ms(0, 1); g_stats.ms_embed = tm.ms(1, 3); g_stats.ms_tail = tm.ms(3, 4); g_stats.ms_stripe = tm.ms(4, 5);
+        g_stats.ms_total = tm.ms(0, 5);
     }
 }
 
@@ -273,7 +350,8 @@ int guarded(int32_t n_nodes, const int32_t* parent, const double* len, const int
     if (n_nodes < 2 || N < 2) return UNIFRAC_ERR_INVALID_ARG;
     if (variant != UNIFRAC_UNWEIGHTED && variant != UNIFRAC_WEIGHTED_NORMALIZED) return UNIFRAC_ERR_INVALID_ARG;
     if (precision != UNIFRAC_FP32 && precision != UNIFRAC_FP64) return UNIFRAC_ERR_INVALID_ARG;
-    if (flags & ~(UNIFRAC_FLAG_LITERAL | UNIFRAC_FLAG_TENSOR_GRAM | UNIFRAC_FLAG_SKIP_VALIDATION | UNIFRAC_FLAG_ABSDIFF))
+    if (flags & ~(UNIFRAC_FLAG_LITERAL | UNIFRAC_FLAG_TENSOR_GRAM | UNIFRAC_FLAG_SKIP_VALIDATION | UNIFRAC_FLAG_ABSDIFF |
+                  UNIFRAC_FLAG_NO_TAIL | UNIFRAC_FLAG_ALL_TAIL))
         return UNIFRAC_ERR_INVALID_ARG;
     if ((long long)N > (1ll << 23)) return UNIFRAC_ERR_UNSUPPORTED;
     Arena A{alloc, user, st};
@@ -354,7 +432,8 @@ int unifrac_last_stats(unifrac_stats_t* out)
     if (!out) return UNIFRAC_ERR_INVALID_ARG;
     if (g_stats_pending) {
         if (cudaEventSynchronize(g_stats_event) != cudaSuccess) { cudaGetLastError(); return UNIFRAC_ERR_CUDA; }
-        g_stats.updates_executed = g_stats_pinned[0] * 2048ull;    // one (warp,row) = 32 x 64 pair updates
+        g_stats.updates_executed_head = g_stats_pinned[0] * 2048ull;    // one (warp,row) = 32 x 64 pair updates
+        g_stats.updates_executed = g_stats.updates_executed_head + g_stats.tail_updates;
         g_stats.rows_staged = g_stats_pinned[1];
         g_stats_pending = false;
     }
@@ -378,6 +457,6 @@ const char* unifrac_status_string(int status)
 }
 
 const char* unifrac_last_cuda_error(void) { return g_cuda_err.c_str(); }
-int unifrac_abi_version(void) { return 1; }
+int unifrac_abi_version(void) { return 2; }
 
 }  // extern "C"
