@@ -135,6 +135,9 @@ typedef struct {
     uint32_t stripe_launches;    /* stripe-kernel launches in this call                               */
     uint32_t tail_launches;      /* tail-scatter launches (one per L2-resident super tile)             */
     uint32_t kernel_launches;    /* all kernel launches in this call                                  */
+    uint32_t gram;               /* 1 if the head branches went through the tcgen05 int8 Gram kernel    */
+    uint32_t gram_k;             /* K (head branches, padded to 64) of that GEMM                       */
+    uint32_t gram_q;             /* fixed-point scale: L_v = round(len_v * 2^q)                        */
     float ms_plan, ms_embed, ms_tail, ms_stripe, ms_total;
 } unifrac_stats_t;
 int unifrac_last_stats(unifrac_stats_t *out);

@@ -38,7 +38,7 @@ class Stats(C.Structure):
                 ("tail_entries", C.c_uint64), ("rows_staged", C.c_uint64),
                 ("embed_rows", C.c_uint64), ("workspace_bytes", C.c_uint64), ("n_tile_pairs", C.c_uint32),
                 ("n_levels", C.c_uint32), ("stripe_launches", C.c_uint32), ("tail_launches", C.c_uint32),
-                ("kernel_launches", C.c_uint32),
+                ("kernel_launches", C.c_uint32), ("gram", C.c_uint32), ("gram_k", C.c_uint32), ("gram_q", C.c_uint32),
                 ("ms_plan", C.c_float), ("ms_embed", C.c_float), ("ms_tail", C.c_float), ("ms_stripe", C.c_float),
                 ("ms_total", C.c_float)]
 

@@ -73,6 +73,12 @@ __global__ void k_bits_count(int n, const int32_t* __restrict__ parent, const do
     if (lane == 0) nv[v] = c;
 }
 
+__global__ void k_mark_class(int n, const uint8_t* __restrict__ cls, uint8_t which, uint32_t* __restrict__ mark)
+{
+    int v = blockIdx.x * blockDim.x + threadIdx.x;
+    if (v < n) mark[v] = cls[v] == which ? 1u : 0u;
+}
+
 // head / tail rule, per branch (costs are additive over branches, so the per-branch rule is optimal):
 //   tail  iff  C(n_v,2) * tail_cost  <  P * head_cost      (costs in seconds per update)
 // tcnt[v] = n_v for tail branches else 0 (scanned into the list offsets); counters[0..3] = head rows,
@@ -110,13 +116,14 @@ template <typename T>
 __global__ void k_tail_fill(int n, const uint8_t* __restrict__ cls, const double* __restrict__ len,
                             const uint32_t* __restrict__ cnt, int Wb, int s0, int s1,
                             const unsigned long long* __restrict__ Tsum, int weighted,
+                            const double* __restrict__ uval /* unweighted: embedded value per branch, or NULL = len */,
                             const uint32_t* __restrict__ tptr, uint32_t* __restrict__ cursor,
                             uint32_t* __restrict__ ts, T* __restrict__ tv)
 {
     int v = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     int lane = threadIdx.x & 31;
     if (v >= n || cls[v] != CLS_TAIL) return;
-    const double l = len[v];
+    const double l = (!weighted && uval) ? uval[v] : len[v];
     uint32_t pos = tptr[v] + cursor[v];
     const uint32_t pos0 = pos;
     const int W = s1 - s0;
@@ -160,8 +167,8 @@ __global__ void k_tail_seg(int n, const uint32_t* __restrict__ tptr, const uint3
 template <typename T>
 __global__ void k_side_sums_part(int n, const int32_t* __restrict__ parent, const double* __restrict__ len,
                                  const uint32_t* __restrict__ cnt, int Wb, int s0, int s1,
-                                 const unsigned long long* __restrict__ Tsum, int weighted, int n_chunks,
-                                 double* __restrict__ part)
+                                 const unsigned long long* __restrict__ Tsum, int weighted,
+                                 const double* __restrict__ uval, int n_chunks, double* __restrict__ part)
 {
     const int strip = blockIdx.x;                       // 32 samples
     const int chunk = blockIdx.y * (blockDim.x >> 5) + (threadIdx.x >> 5);
@@ -185,7 +192,7 @@ __global__ void k_side_sums_part(int n, const int32_t* __restrict__ parent, cons
                 const long long v = vb + u;
                 const double l = len[v];
                 if (parent[v] >= 0 && l > 0.0) {
-                    double val = weighted ? l * ((double)x[u] / Ts) : l;
+                    double val = weighted ? l * ((double)x[u] / Ts) : (uval ? uval[v] : l);
                     acc += (double)(T)val;
                 }
             }

@@ -7,11 +7,13 @@
 #include "embed.cuh"
 #include "tail.cuh"
 #include "stripe.cuh"
+#include "gram.cuh"
 
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
 #include <string>
+#include <type_traits>
 #include <vector>
 
 using namespace ufb;
@@ -25,6 +27,8 @@ thread_local cudaEvent_t g_stats_event = nullptr;
 thread_local bool g_stats_pending = false;
 
 struct CudaFail { cudaError_t e; const char* what; int line; };
+struct WorkspaceFail {};
+struct StatusFail { int status; };
 
 #define CU(x)                                                                                   \
     do {                                                                                        \
@@ -32,9 +36,6 @@ struct CudaFail { cudaError_t e; const char* what; int line; };
         if (e_ != cudaSuccess) throw CudaFail{e_, #x, __LINE__};                                \
     } while (0)
 #define CU_LAUNCH() CU(cudaGetLastError())
-
-struct WorkspaceFail {};
-struct StatusFail { int status; };
 
 // bump of caller-provided (or stream-ordered) device allocations
 struct Arena {
@@ -59,6 +60,43 @@ struct Arena {
 };
 
 inline int cdiv(long long a, long long b) { return (int)((a + b - 1) / b); }
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point (the library does not link libcuda)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+CUtensorMap make_u8_rowmajor_map(void* base, uint64_t cols, uint64_t rows, uint32_t box_cols, uint32_t box_rows)
+{
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr);
+        if (e != cudaSuccess || qr != cudaDriverEntryPointSuccess || !p) throw CudaFail{e != cudaSuccess ? e : cudaErrorUnknown, "cuTensorMapEncodeTiled entry point", __LINE__};
+        fn = reinterpret_cast<EncodeTiledFn>(p);
+    }
+    CUtensorMap m;
+    cuuint64_t dims[2] = {cols, rows};
+    cuuint64_t strides[1] = {cols};              // bytes, dimension 1
+    cuuint32_t box[2] = {box_cols, box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = fn(&m, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                    CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) throw CudaFail{cudaErrorInvalidValue, "cuTensorMapEncodeTiled", __LINE__};
+    return m;
+}
+
+// tile pairs (I <= J) in BLK x BLK blocks of tiles, so that CTAs working on consecutive pairs share operand tiles in L2
+std::vector<int2> blocked_pairs(int n_tiles, int BLK)
+{
+    std::vector<int2> v;
+    v.reserve((size_t)n_tiles * (n_tiles + 1) / 2);
+    for (int bi = 0; bi < n_tiles; bi += BLK)
+        for (int bj = bi; bj < n_tiles; bj += BLK)
+            for (int i = bi; i < std::min(n_tiles, bi + BLK); ++i)
+                for (int j = std::max(i, bj); j < std::min(n_tiles, bj + BLK); ++j) v.push_back(make_int2(i, j));
+    return v;
+}
 
 struct Timer {
     bool on; cudaStream_t s; cudaEvent_t ev[8]; int n = 0;
@@ -147,8 +185,8 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     uint32_t* tptr = A.get_n<uint32_t>((size_t)n + 1);
     unsigned long long* work = A.get_n<unsigned long long>(16);
     CU(cudaMemsetAsync(work, 0, sizeof(unsigned long long) * 16, st));
+    uint32_t* bits = A.get_n<uint32_t>((size_t)n * NW);
     {
-        uint32_t* bits = A.get_n<uint32_t>((size_t)n * NW);
         CU(cudaMemsetAsync(bits, 0, sizeof(uint32_t) * (size_t)n * NW, st));
         k_bits_scatter<<<cdiv((long long)N * 32, TB), TB, 0, st>>>(N, tab.indptr, tab.indices, tab.counts, bits, NW); CU_LAUNCH(); ++launches;
         for (int d = n_levels - 1; d >= 0; --d) {
@@ -163,8 +201,10 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     k_work_counts<<<cdiv(n, TB), TB, 0, st>>>(n, nv, (unsigned long long)N, work); CU_LAUNCH(); ++launches;
     // per-branch rule: tail iff C(n_v,2) / R_tail < P / R_head; the ratio
     // R_tail / R_head is measured (RED.ADD rate in L2 vs dense stripe rate) and can be overridden
-    double ratio = 0.022;
-    if (const char* e = getenv("UNIFRAC_B200_TAIL_RATIO")) ratio = atof(e);
+    const bool gram = std::is_same<T, float>::value && !weighted && (flags & UNIFRAC_FLAG_TENSOR_GRAM) &&
+                      !(flags & (UNIFRAC_FLAG_NO_TAIL | UNIFRAC_FLAG_ABSDIFF | UNIFRAC_FLAG_LITERAL | UNIFRAC_FLAG_ALL_TAIL));
+    double ratio = gram ? 7.5e-4 : 0.022;
+    if (const char* e = getenv(gram ? "UNIFRAC_B200_TAIL_RATIO_GRAM" : "UNIFRAC_B200_TAIL_RATIO")) ratio = atof(e);
     uint32_t force = 0;
     if (flags & (UNIFRAC_FLAG_NO_TAIL | UNIFRAC_FLAG_ABSDIFF | UNIFRAC_FLAG_LITERAL)) force = 1;
     else if (flags & UNIFRAC_FLAG_ALL_TAIL) force = 2;
@@ -179,6 +219,37 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     T* tv = A.get_n<T>(tail_entries ? tail_entries : 1);
     uint32_t* tcursor = A.get_n<uint32_t>(n);
     CU(cudaMemsetAsync(tcursor, 0, sizeof(uint32_t) * n, st));
+
+    // ------------------------------------------------------------------ tensor-core Gram path: u8 operand matrices from the bits
+    bool use_gram = gram && head_rows > 0 && head_rows < (1ull << 23);
+    double* uval = nullptr;
+    uint8_t* XG[4] = {nullptr, nullptr, nullptr, nullptr};
+    uint32_t K_pad = 0;
+    int gram_q = 0;
+    if (use_gram) {
+        uint32_t* is_head = A.get_n<uint32_t>(n);
+        uint32_t* hrank = A.get_n<uint32_t>((size_t)n + 1);
+        k_mark_class<<<cdiv(n, TB), TB, 0, st>>>(n, cls, CLS_HEAD, is_head); CU_LAUNCH(); ++launches;
+        k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>(n, is_head, hrank); CU_LAUNCH(); ++launches;
+        unsigned long long* lmax = work + 12;
+        k_gram_lenmax<<<cdiv(n, TB), TB, 0, st>>>(n, cls, len, lmax); CU_LAUNCH(); ++launches;
+        unsigned long long h_lmax = 0;
+        CU(cudaMemcpyAsync(&h_lmax, lmax, sizeof(h_lmax), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        double lm; memcpy(&lm, &h_lmax, sizeof(lm));
+        int ex = 0; frexp(lm, &ex);
+        gram_q = 24 - ex;                                   // lmax * 2^q in [2^23, 2^24)
+        const uint32_t K = (uint32_t)head_rows;
+        K_pad = (K + GRAM_BK - 1) / GRAM_BK * GRAM_BK;
+        const size_t Npad = (size_t)NW * 32;
+        int32_t* hrows = A.get_n<int32_t>(K_pad);
+        uint32_t* Lq = A.get_n<uint32_t>(K_pad);
+        uval = A.get_n<double>(n);
+        for (auto& x : XG) x = A.get_n<uint8_t>((size_t)K_pad * Npad);
+        k_gram_quant<<<cdiv(n, TB), TB, 0, st>>>(n, cls, hrank, len, gram_q, hrows, Lq, uval); CU_LAUNCH(); ++launches;
+        k_gram_expand<<<cdiv((long long)K_pad * NW, TB), TB, 0, st>>>(K, K_pad, hrows, Lq, bits, NW, XG[0], XG[1], XG[2], XG[3]);
+        CU_LAUNCH(); ++launches;
+    }
     tm.mark();
 
     // ------------------------------------------------------------------ a-1 .. a-4 embedding, per sample batch
@@ -221,12 +292,13 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             CU_LAUNCH(); ++launches;
         }
         k_side_sums_part<T><<<dim3(cdiv(s1 - s0, 32), cdiv(n_chunks, 8)), 256, 0, st>>>(n, parent, len, cnt, Wb, s0, s1, Tsum, weighted,
-                                                                                        n_chunks, sums_part); CU_LAUNCH(); ++launches;
+                                                                                        uval, n_chunks, sums_part); CU_LAUNCH(); ++launches;
         k_side_sums_reduce<<<cdiv(s1 - s0, TB), TB, 0, st>>>(s1 - s0, Wb, n_chunks, sums_part, s0, sums); CU_LAUNCH(); ++launches;
         if (tail_rows) {
-            k_tail_fill<T><<<cdiv((long long)n * 32, TB), TB, 0, st>>>(n, cls, len, cnt, Wb, s0, s1, Tsum, weighted, tptr, tcursor, ts, tv);
+            k_tail_fill<T><<<cdiv((long long)n * 32, TB), TB, 0, st>>>(n, cls, len, cnt, Wb, s0, s1, Tsum, weighted, uval, tptr, tcursor, ts, tv);
             CU_LAUNCH(); ++launches;
         }
+        if (use_gram) continue;        // head branches go through the u8 operand matrices, not the compact fp rows
         k_row_flags<<<dim3(nwords, tb), 1024, 0, st>>>(n, parent, len, cnt, Wb, rflags, nwords, t0, qtmp, cls); CU_LAUNCH(); ++launches;
         k_rank_scan<<<tb, 1024, 0, st>>>(rflags, rrank, nwords, t0, rows); CU_LAUNCH(); ++launches;
         CU(cudaMemcpyAsync(h_rows.data() + t0, rows + t0, sizeof(uint32_t) * tb, cudaMemcpyDeviceToHost, st));
@@ -277,16 +349,41 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     tm.mark();
 
     // ------------------------------------------------------------------ a-5 / a-6 stripe accumulation + finalize
+    unsigned long long* kstats = work + 4;     // [0] rows executed, [1] rows staged (zeroed above)
+    unsigned stripe_launches = 0;
+    uint32_t n_pairs = 0;
+    int dev = 0, n_sm = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    if (use_gram) {
+        if constexpr (std::is_same<T, float>::value) {
+            std::vector<int2> h_pairs = blocked_pairs(n_tiles, 12);
+            n_pairs = (uint32_t)h_pairs.size();
+            int2* pairs = A.get_n<int2>(n_pairs);
+            CU(cudaMemcpyAsync(pairs, h_pairs.data(), sizeof(int2) * n_pairs, cudaMemcpyHostToDevice, st));
+            const size_t Npad = (size_t)NW * 32;
+            CUtensorMap tmA = make_u8_rowmajor_map(XG[0], Npad, K_pad, TILE, GRAM_BK);
+            CUtensorMap tmB0 = make_u8_rowmajor_map(XG[1], Npad, K_pad, TILE, GRAM_BK);
+            CUtensorMap tmB1 = make_u8_rowmajor_map(XG[2], Npad, K_pad, TILE, GRAM_BK);
+            CUtensorMap tmB2 = make_u8_rowmajor_map(XG[3], Npad, K_pad, TILE, GRAM_BK);
+            GramParams G{};
+            G.pairs = pairs; G.n_pairs = n_pairs; G.K_pad = K_pad; G.sums = sums; G.n_samples = N;
+            G.out = reinterpret_cast<float*>(out); G.add_out = tail_rows ? 1 : 0; G.q = gram_q;
+            CU(cudaFuncSetAttribute(k_gram, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GRAM_SMEM));
+            unsigned grid = (unsigned)std::min<long long>(n_sm, n_pairs);
+            k_gram<<<grid, GRAM_THREADS, GRAM_SMEM, st>>>(tmA, tmB0, tmB1, tmB2, G); CU_LAUNCH(); ++launches; ++stripe_launches;
+            CU(cudaStreamSynchronize(st));       // h_pairs staging copy done before it goes out of scope
+        }
+    } else {
     std::vector<int2> h_pairs;
     h_pairs.reserve((size_t)n_tiles * (n_tiles + 1) / 2);
     for (int i = 0; i < n_tiles; ++i)
         for (int j = i; j < n_tiles; ++j) h_pairs.push_back(make_int2(i, j));
-    const uint32_t n_pairs = (uint32_t)h_pairs.size();
+    n_pairs = (uint32_t)h_pairs.size();
     int2* pairs = A.get_n<int2>(n_pairs);
     CU(cudaMemcpyAsync(pairs, h_pairs.data(), sizeof(int2) * n_pairs, cudaMemcpyHostToDevice, st));
     T* zero_row = A.get_n<T>(TILE);
     CU(cudaMemsetAsync(zero_row, 0, sizeof(T) * TILE, st));
-    unsigned long long* kstats = work + 4;     // [0] rows executed, [1] rows staged (zeroed above)
     uint32_t* counter = reinterpret_cast<uint32_t*>(work + 6);
 
     StripeParams P{};
@@ -296,13 +393,9 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     P.pairs = pairs; P.n_pairs = n_pairs; P.counter = counter; P.sums = sums;
     P.n_samples = N; P.weighted = weighted; P.out = out; P.stats = kstats; P.zero_row = zero_row;
 
-    unsigned stripe_launches = 0;
     if (flags & UNIFRAC_FLAG_LITERAL) {
         k_literal<T><<<n_pairs, 256, 0, st>>>(P); CU_LAUNCH(); ++launches; ++stripe_launches;
     } else {
-        int dev = 0, n_sm = 0;
-        CU(cudaGetDevice(&dev));
-        CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
         const size_t smem = stripe_smem_bytes<T>();
         auto kern = (flags & UNIFRAC_FLAG_ABSDIFF) ? k_stripe<T, FORM_ABSDIFF> : k_stripe<T, FORM_MIN>;
         CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -312,6 +405,8 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         unsigned grid = (unsigned)std::min<long long>((long long)n_sm * occ, n_pairs);
         P.scratch = A.get_n<double>((size_t)grid * 64 * 256);
         kern<<<grid, STRIPE_THREADS, smem, st>>>(P); CU_LAUNCH(); ++launches; ++stripe_launches;
+    }
+    CU(cudaStreamSynchronize(st));           // h_pairs staging copy done before it goes out of scope
     }
     // stripe counters -> pinned host block (read lazily by unifrac_last_stats)
     if (!g_stats_pinned) { CU(cudaHostAlloc(&g_stats_pinned, 2 * sizeof(unsigned long long), cudaHostAllocDefault)); }
@@ -329,6 +424,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     g_stats.embed_rows = embed_rows;
     g_stats.head_rows = head_rows; g_stats.tail_rows = tail_rows; g_stats.tail_updates = tail_updates; g_stats.tail_entries = tail_entries;
     g_stats.tail_launches = tail_launches;
+    g_stats.gram = use_gram ? 1u : 0u; g_stats.gram_k = K_pad; g_stats.gram_q = (uint32_t)gram_q;
     g_stats.n_tile_pairs = n_pairs;
     g_stats.n_levels = (uint32_t)n_levels;
     g_stats.stripe_launches = stripe_launches;
@@ -433,6 +529,7 @@ int unifrac_last_stats(unifrac_stats_t* out)
     if (g_stats_pending) {
         if (cudaEventSynchronize(g_stats_event) != cudaSuccess) { cudaGetLastError(); return UNIFRAC_ERR_CUDA; }
         g_stats.updates_executed_head = g_stats_pinned[0] * 2048ull;    // one (warp,row) = 32 x 64 pair updates
+        if (g_stats.gram) g_stats.updates_executed_head = g_stats.head_rows * ((uint64_t)g_stats.updates_dense / (g_stats.branches_embedded ? g_stats.branches_embedded : 1));
         g_stats.updates_executed = g_stats.updates_executed_head + g_stats.tail_updates;
         g_stats.rows_staged = g_stats_pinned[1];
         g_stats_pending = false;

@@ -61,6 +61,24 @@ def test_three_tiles_ragged_tail_all_pairs(B, O, variant, precision, flags):
     check(gpu_dm(B, p, variant, precision, flags), want, precision)
 
 
+@pytest.mark.parametrize("name", ["tiny", "three_tiles", "deep"])
+def test_tensor_core_gram_path_unweighted_fp32(B, O, name):
+    """UNIFRAC_FLAG_TENSOR_GRAM: head branches through the tcgen05 int8 Gram kernel (24-bit fixed-point
+    lengths, exact int32 accumulation), tail branches through the scatter; same 1e-5 tolerance."""
+    if name == "tiny":
+        p = synth.make_config("tiny", seed=0)
+    elif name == "three_tiles":
+        p = synth.make_problem(3000, 300, 0.1, 1.1, synth.CONFIGS["small"][4], synth.CONFIGS["small"][5], seed=3)
+    else:
+        p = synth.make_problem(12000, 700, 0.05, 1.05, synth.CONFIGS["small"][4], synth.CONFIGS["small"][5], seed=5)
+    want = O.all_pairs(p.parent, p.branch_len, p.indptr, p.indices, p.counts, U)
+    got = gpu_dm(B, p, U, 0, flags=B.FLAG_TENSOR_GRAM)
+    st = B.unifrac_last_stats()
+    assert st["gram"] == 1 and st["gram_k"] >= st["head_rows"] > 0
+    rel = check(got, want, 0)
+    print(f"gram {name}: head {st['head_rows']} tail {st['tail_rows']} q {st['gram_q']} max rel err {rel:.3e}")
+
+
 @pytest.mark.parametrize("n_samples", [2, 3, 127, 128, 129, 257])
 def test_tile_boundary_sample_counts(B, O, n_samples):
     p = synth.make_problem(400, n_samples, 0.1, 1.1, synth._k_poisson40, synth._c_geometric, seed=n_samples)
