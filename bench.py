@@ -229,26 +229,59 @@ def main():
             dist.destroy_process_group()
         return 0
 
-    # ---------------- roofline of the dominant kernel (stripe accumulation): plain FP32 ALU work
-    t_stripe = sum(s["ms_stripe"] for s in flat) * 1e-3
-    n_launch = sum(s["stripe_launches"] for s in flat)
-    w_exec = sum(s["updates_executed_head"] for s in flat)
-    w_inter = sum(s["updates_inter"] for s in flat)
-    w_union = sum(s["updates_union"] for s in flat)
-    achieved = 2.0 * w_exec / t_stripe / 1e12 if t_stripe > 0 else 0.0
+    # ---------------- rooflines of the three a-5 kernels; the one with the most time in the step is "roofline"
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
     except Exception:
         pass
-    roofline = dict(bound="alu", achieved=achieved, peak=ALU_PEAK_TFLOPS, unit="TFLOP/s", frac=achieved / ALU_PEAK_TFLOPS,
-                    traffic=None, kernel="k_stripe", launches=n_launch, ms_per_launch=1e3 * t_stripe / max(1, n_launch),
-                    executed_updates_per_launch=w_exec / max(1, n_launch),
-                    peak_source=f"{SM_COUNT} SMs x {FP32_LANES} FP32 lanes x {SM_MAX_GHZ} GHz (sm_max_mhz of MEASURED_PEAKS.json"
-                                f"{'' if peaks else ' fallback'}); 2 FP32 lane-ops (FMNMX+FADD or FADD+FADD) per update",
-                    frac_algorithmic_inter=2.0 * w_inter / t_stripe / 1e12 / ALU_PEAK_TFLOPS if t_stripe > 0 else 0.0,
-                    frac_algorithmic_union=2.0 * w_union / t_stripe / 1e12 / ALU_PEAK_TFLOPS if t_stripe > 0 else 0.0,
-                    stripe_share_of_step=t_stripe / (ms * 1e-3))
+    src = "measured" if peaks else "fallback"
+    step_s = ms * 1e-3
+    rl = []
+    # (1) k_stripe: CUDA-core register-tile kernel (head branches; weighted, fp64, or NO_TENSOR)
+    ss = [s for s in flat if not s["gram"]]
+    if ss:
+        t = sum(s["ms_stripe"] for s in ss) * 1e-3
+        w_exec = sum(s["updates_executed_head"] for s in ss)
+        nl = sum(s["stripe_launches"] for s in ss)
+        ach = 2.0 * w_exec / t / 1e12 if t > 0 else 0.0
+        rl.append(dict(bound="alu", achieved=ach, peak=ALU_PEAK_TFLOPS, unit="TFLOP/s", frac=ach / ALU_PEAK_TFLOPS, traffic=None,
+                       kernel="k_stripe", launches=nl, ms_per_launch=1e3 * t / max(1, nl),
+                       executed_updates_per_launch=w_exec / max(1, nl), seconds=t, share_of_step=t / step_s,
+                       peak_source=f"{SM_COUNT} SMs x {FP32_LANES} FP32 lanes x {SM_MAX_GHZ} GHz (sm_max_mhz of MEASURED_PEAKS.json, {src}); "
+                                   "2 FP32-pipe lane-ops (FMNMX+FADD) per (pair, branch) update"))
+    # (2) k_gram: tcgen05 kind::i8 Gram kernel (head branches, unweighted fp32): 3 u8 digit MACs per update
+    gs = [s for s in flat if s["gram"]]
+    if gs:
+        t = sum(s["ms_stripe"] for s in gs) * 1e-3
+        macs = sum(float(s["gram_k"]) * s["n_tile_pairs"] * 128 * 128 * 3 for s in gs)
+        nl = sum(s["stripe_launches"] for s in gs)
+        bf16 = peaks.get("bf16_tflops", 1590.0)
+        peak = 2.0 * bf16                       # int8 : bf16 nominal ratio 2 (4.5 vs 2.25 PFLOP/s dense, B200_PROFILING.md)
+        ach = 2.0 * macs / t / 1e12 if t > 0 else 0.0
+        rl.append(dict(bound="tensor", achieved=ach, peak=peak, unit="TFLOP/s", frac=ach / peak, traffic=None, kernel="k_gram",
+                       launches=nl, ms_per_launch=1e3 * t / max(1, nl), macs_per_launch=macs / max(1, nl), seconds=t,
+                       share_of_step=t / step_s,
+                       peak_source=f"2 x bf16_tflops ({bf16}, {src} burst) = int8 dense peak by the guide's nominal 2:1 ratio; "
+                                   "algorithmic ops = 2 x 3 digit-MACs x 128 x 128 x K per tile pair",
+                       operand_gbs=sum(float(s["gram_k"]) * s["n_tile_pairs"] * 512 for s in gs) / t / 1e9 if t > 0 else 0.0))
+    # (3) k_tail_scatter: RED.ADD of min(u_a, u_b) into the L2-resident super tile
+    t = sum(s["ms_tail"] for s in flat) * 1e-3
+    reds = sum(s["tail_updates"] for s in flat)
+    nl = sum(s["tail_launches"] for s in flat)
+    if nl:
+        RED_PEAK = 1.93e11      # measured on this pool's B200: random fp32 RED.ADD into a 64 MB footprint (profiles/r01_ubench_red.txt)
+        rl.append(dict(bound="l2_atomic", achieved=reds / t / 1e9 if t > 0 else 0.0, peak=RED_PEAK / 1e9, unit="GRED/s",
+                       frac=reds / t / RED_PEAK if t > 0 else 0.0, traffic=None, kernel="k_tail_scatter", launches=nl,
+                       ms_per_launch=1e3 * t / max(1, nl), seconds=t, share_of_step=t / step_s,
+                       peak_source="micro-benchmark of scattered RED.ADD.F32 into an L2-resident footprint, same GPU pool"))
+    rl.sort(key=lambda r: -r["seconds"])
+    roofline = dict(rl[0])
+    roofline["others"] = rl[1:]
+    w_inter = sum(s["updates_inter"] for s in flat)
+    w_exec_all = sum(s["updates_executed"] for s in flat)
+    roofline["step_updates"] = dict(dense=upd_all / max(1, world), executed=w_exec_all, inter=w_inter,
+                                    embed_seconds=sum(s["ms_embed"] for s in flat) * 1e-3)
 
     cpu = None
     if not a.no_cpu_baseline:
@@ -265,6 +298,7 @@ def main():
             ms_embed=float(np.mean([s["ms_embed"] for s in ss])), ms_tail=float(np.mean([s["ms_tail"] for s in ss])),
             ms_stripe=float(np.mean([s["ms_stripe"] for s in ss])),
             head_rows=ss[0]["head_rows"], tail_rows=ss[0]["tail_rows"], tail_updates=ss[0]["tail_updates"],
+            gram=ss[0]["gram"], gram_k=ss[0]["gram_k"], gram_q=ss[0]["gram_q"],
             tail_entries=ss[0]["tail_entries"], tail_launches=ss[0]["tail_launches"],
             updates_executed_head=ss[0]["updates_executed_head"],
             updates_dense=ss[0]["updates_dense"], updates_executed=ss[0]["updates_executed"],

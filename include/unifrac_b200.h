@@ -47,8 +47,10 @@ typedef enum {
 #define UNIFRAC_FLAG_LITERAL          1u  /* debug: accumulate BOTH pairwise sums exactly as BASELINE.json:5
                                              words them (len*|u-v| and len*(u+v); len*xor and len*or) in a
                                              plain one-thread-per-pair fp64 kernel.  Slow; small inputs.   */
-#define UNIFRAC_FLAG_TENSOR_GRAM      2u  /* unweighted + fp32 only: allow the tcgen05 int8 Gram path
-                                             (X^T diag(len) X with len in 24-bit fixed point)              */
+#define UNIFRAC_FLAG_TENSOR_GRAM      2u  /* accepted for compatibility: the tcgen05 int8 Gram path (X^T diag(len) X,
+                                             len in 24-bit fixed point, exact int32 accumulation) is the DEFAULT for
+                                             the head branches of unweighted + fp32 (it meets the 1e-5 tolerance,
+                                             BASELINE.json:5); see UNIFRAC_FLAG_NO_TENSOR                    */
 #define UNIFRAC_FLAG_SKIP_VALIDATION  4u  /* trust the inputs (tree/table checks are skipped)            */
 #define UNIFRAC_FLAG_ABSDIFF          8u  /* stripe kernel accumulates |u~_i - u~_j| over rows present in
                                              EITHER tile (direct form) instead of min(u~_i,u~_j) over rows
@@ -57,6 +59,8 @@ typedef enum {
 #define UNIFRAC_FLAG_NO_TAIL         16u  /* every branch goes through the dense stripe kernel (no sparse
                                              tail scatter)                 */
 #define UNIFRAC_FLAG_ALL_TAIL        32u  /* debug: every branch goes through the sparse tail scatter       */
+#define UNIFRAC_FLAG_NO_TENSOR       64u  /* unweighted + fp32: head branches on the CUDA-core stripe kernel
+                                             instead of the tensor-core Gram kernel                        */
 
 /* CSR table, rows = samples, columns = tip NODE ids (reading Q6). */
 typedef struct {

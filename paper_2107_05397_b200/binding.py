@@ -17,7 +17,7 @@ from . import build as _build
 UNWEIGHTED, WEIGHTED_NORMALIZED = 0, 1
 FP32, FP64 = 0, 1
 FLAG_LITERAL, FLAG_TENSOR_GRAM, FLAG_SKIP_VALIDATION, FLAG_ABSDIFF = 1, 2, 4, 8
-FLAG_NO_TAIL, FLAG_ALL_TAIL = 16, 32
+FLAG_NO_TAIL, FLAG_ALL_TAIL, FLAG_NO_TENSOR = 16, 32, 64
 
 OK = 0
 ERR_INVALID_ARG, ERR_INVALID_TREE, ERR_INVALID_TABLE, ERR_EMPTY_SAMPLE = -1, -2, -3, -4

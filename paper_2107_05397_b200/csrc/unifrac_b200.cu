@@ -201,12 +201,12 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     k_work_counts<<<cdiv(n, TB), TB, 0, st>>>(n, nv, (unsigned long long)N, work); CU_LAUNCH(); ++launches;
     // per-branch rule: tail iff C(n_v,2) / R_tail < P / R_head; the ratio
     // R_tail / R_head is measured (RED.ADD rate in L2 vs dense stripe rate) and can be overridden
-    const bool gram = std::is_same<T, float>::value && !weighted && (flags & UNIFRAC_FLAG_TENSOR_GRAM) &&
-                      !(flags & (UNIFRAC_FLAG_NO_TAIL | UNIFRAC_FLAG_ABSDIFF | UNIFRAC_FLAG_LITERAL | UNIFRAC_FLAG_ALL_TAIL));
+    const bool gram = std::is_same<T, float>::value && !weighted &&
+                      !(flags & (UNIFRAC_FLAG_NO_TENSOR | UNIFRAC_FLAG_ABSDIFF | UNIFRAC_FLAG_LITERAL | UNIFRAC_FLAG_ALL_TAIL));
     double ratio = gram ? 7.5e-4 : 0.022;
     if (const char* e = getenv(gram ? "UNIFRAC_B200_TAIL_RATIO_GRAM" : "UNIFRAC_B200_TAIL_RATIO")) ratio = atof(e);
     uint32_t force = 0;
-    if (flags & (UNIFRAC_FLAG_NO_TAIL | UNIFRAC_FLAG_ABSDIFF | UNIFRAC_FLAG_LITERAL)) force = 1;
+    if (flags & (UNIFRAC_FLAG_NO_TAIL | UNIFRAC_FLAG_ABSDIFF | UNIFRAC_FLAG_LITERAL)) force = 1;   // NO_TAIL + Gram = dense GEMM over every branch
     else if (flags & UNIFRAC_FLAG_ALL_TAIL) force = 2;
     k_classify<<<cdiv(n, TB), TB, 0, st>>>(n, nv, 0.5 * (double)N * (double)(N - 1) * ratio, force, cls, tcnt, work + 8); CU_LAUNCH(); ++launches;
     k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>(n, tcnt, tptr); CU_LAUNCH(); ++launches;
@@ -447,7 +447,7 @@ int guarded(int32_t n_nodes, const int32_t* parent, const double* len, const int
     if (variant != UNIFRAC_UNWEIGHTED && variant != UNIFRAC_WEIGHTED_NORMALIZED) return UNIFRAC_ERR_INVALID_ARG;
     if (precision != UNIFRAC_FP32 && precision != UNIFRAC_FP64) return UNIFRAC_ERR_INVALID_ARG;
     if (flags & ~(UNIFRAC_FLAG_LITERAL | UNIFRAC_FLAG_TENSOR_GRAM | UNIFRAC_FLAG_SKIP_VALIDATION | UNIFRAC_FLAG_ABSDIFF |
-                  UNIFRAC_FLAG_NO_TAIL | UNIFRAC_FLAG_ALL_TAIL))
+                  UNIFRAC_FLAG_NO_TAIL | UNIFRAC_FLAG_ALL_TAIL | UNIFRAC_FLAG_NO_TENSOR))
         return UNIFRAC_ERR_INVALID_ARG;
     if ((long long)N > (1ll << 23)) return UNIFRAC_ERR_UNSUPPORTED;
     Arena A{alloc, user, st};

@@ -72,11 +72,15 @@ def test_tensor_core_gram_path_unweighted_fp32(B, O, name):
     else:
         p = synth.make_problem(12000, 700, 0.05, 1.05, synth.CONFIGS["small"][4], synth.CONFIGS["small"][5], seed=5)
     want = O.all_pairs(p.parent, p.branch_len, p.indptr, p.indices, p.counts, U)
-    got = gpu_dm(B, p, U, 0, flags=B.FLAG_TENSOR_GRAM)
-    st = B.unifrac_last_stats()
-    assert st["gram"] == 1 and st["gram_k"] >= st["head_rows"] > 0
-    rel = check(got, want, 0)
-    print(f"gram {name}: head {st['head_rows']} tail {st['tail_rows']} q {st['gram_q']} max rel err {rel:.3e}")
+    for flags in (0, B.FLAG_NO_TAIL):                 # default head/tail split; dense GEMM over every branch
+        got = gpu_dm(B, p, U, 0, flags=flags)
+        st = B.unifrac_last_stats()
+        assert st["gram"] == 1 and st["gram_k"] >= st["head_rows"] > 0
+        rel = check(got, want, 0)
+        print(f"gram {name} flags {flags}: head {st['head_rows']} tail {st['tail_rows']} q {st['gram_q']} max rel err {rel:.3e}")
+    got = gpu_dm(B, p, U, 0, flags=B.FLAG_NO_TENSOR)
+    assert B.unifrac_last_stats()["gram"] == 0
+    check(got, want, 0)
 
 
 @pytest.mark.parametrize("n_samples", [2, 3, 127, 128, 129, 257])
@@ -98,7 +102,7 @@ def test_general_trees_multifurcation_unary_zero_length(B, O, seed):
         want = O.all_pairs(p.parent, p.branch_len, p.indptr, p.indices, p.counts, variant)
         for flags in (0, 16, 32, 8, 1):
             check(gpu_dm(B, p, variant, 1, flags), want, 1)
-        for flags in (0, 16, 32):
+        for flags in (0, 16, 32, 64, 64 + 16):
             check(gpu_dm(B, p, variant, 0, flags), want, 0)
 
 
@@ -149,6 +153,7 @@ def test_small_config_sampled_pairs(B, O):
         st = B.unifrac_last_stats()
         assert st["head_rows"] > 0 and st["tail_rows"] > 0          # the default split uses both paths here
         check(gpu_dm(B, p, variant, 0, flags=16)[idx], want, 0)     # all head
+        check(gpu_dm(B, p, variant, 0, flags=64)[idx], want, 0)     # CUDA-core head for unweighted too
 
 
 def test_host_entry_point_matches_device_entry_point(B, O):
