@@ -295,7 +295,8 @@ def main():
         ss = [st[k] for st in all_stats]
         per_variant["unweighted" if v == 0 else "weighted_normalized"] = dict(
             ms_total=float(np.mean([s["ms_total"] for s in ss])), ms_plan=float(np.mean([s["ms_plan"] for s in ss])),
-            ms_embed=float(np.mean([s["ms_embed"] for s in ss])), ms_tail=float(np.mean([s["ms_tail"] for s in ss])),
+            ms_embed=float(np.mean([s["ms_embed"] for s in ss])), ms_tail=float(np.mean([s["ms_tail"] for s in ss])), ms_mid=float(np.mean([s["ms_mid"] for s in ss])),
+            mid_rows=ss[0]["mid_rows"], mid_updates=ss[0]["mid_updates"], mid_F=ss[0]["mid_F"],
             ms_stripe=float(np.mean([s["ms_stripe"] for s in ss])),
             head_rows=ss[0]["head_rows"], tail_rows=ss[0]["tail_rows"], tail_updates=ss[0]["tail_updates"],
             gram=ss[0]["gram"], gram_k=ss[0]["gram_k"], gram_q=ss[0]["gram_q"],

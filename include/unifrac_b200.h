@@ -59,6 +59,8 @@ typedef enum {
 #define UNIFRAC_FLAG_NO_TAIL         16u  /* every branch goes through the dense stripe kernel (no sparse
                                              tail scatter)                 */
 #define UNIFRAC_FLAG_ALL_TAIL        32u  /* debug: every branch goes through the sparse tail scatter       */
+#define UNIFRAC_FLAG_NO_MID         128u  /* fp32: no shared-memory fixed-point "mid" kernel; branches are split into
+                                             head and tail only                                            */
 #define UNIFRAC_FLAG_NO_TENSOR       64u  /* unweighted + fp32: head branches on the CUDA-core stripe kernel
                                              instead of the tensor-core Gram kernel                        */
 
@@ -130,7 +132,9 @@ typedef struct {
     uint64_t head_rows;          /* branches handled by the dense stripe kernel                       */
     uint64_t tail_rows;          /* branches handled by the sparse tail scatter                       */
     uint64_t tail_updates;       /* sum over tail branches of C(n_v,2) = RED.ADDs issued               */
-    uint64_t tail_entries;       /* sum over tail branches of n_v = (sample, value) list entries       */
+    uint64_t tail_entries;       /* sum over tail and mid branches of n_v = (sample, value) list entries */
+    uint64_t mid_rows;           /* branches handled by the shared-memory fixed-point kernel (fp32 mode)  */
+    uint64_t mid_updates;        /* sum over mid branches of C(n_v,2) = shared-memory atomic adds          */
     uint64_t rows_staged;        /* rows the producer staged into shared memory, over all tile pairs  */
     uint64_t embed_rows;         /* sum over sample tiles of non-empty rows (compact embedding rows)  */
     uint64_t workspace_bytes;    /* device bytes requested from the allocator                         */
@@ -139,10 +143,12 @@ typedef struct {
     uint32_t stripe_launches;    /* stripe-kernel launches in this call                               */
     uint32_t tail_launches;      /* tail-scatter launches (one per L2-resident super tile)             */
     uint32_t kernel_launches;    /* all kernel launches in this call                                  */
+    uint32_t mid_launches;       /* launches of the mid kernel                                          */
+    uint32_t mid_F;              /* its fixed-point scale: u_q = round(u * 2^F)                          */
     uint32_t gram;               /* 1 if the head branches went through the tcgen05 int8 Gram kernel    */
     uint32_t gram_k;             /* K (head branches, padded to 64) of that GEMM                       */
     uint32_t gram_q;             /* fixed-point scale: L_v = round(len_v * 2^q)                        */
-    float ms_plan, ms_embed, ms_tail, ms_stripe, ms_total;
+    float ms_plan, ms_embed, ms_tail, ms_mid, ms_stripe, ms_total;
 } unifrac_stats_t;
 int unifrac_last_stats(unifrac_stats_t *out);
 

@@ -20,7 +20,7 @@
 
 namespace ufb {
 
-enum : uint8_t { CLS_NONE = 0, CLS_HEAD = 1, CLS_TAIL = 2 };
+enum : uint8_t { CLS_NONE = 0, CLS_HEAD = 1, CLS_TAIL = 2, CLS_MID = 3 };
 
 // ------------------------------------------------------------------ presence bits (all samples at once)
 // bits[v][w] bit b  <=>  sample 32*w + b has a positive count on some tip below v
@@ -73,39 +73,54 @@ __global__ void k_bits_count(int n, const int32_t* __restrict__ parent, const do
     if (lane == 0) nv[v] = c;
 }
 
+// max over a vector of non-negative doubles (bit patterns order like the values)
+__global__ void k_max_positive(int n, const double* __restrict__ x, unsigned long long* __restrict__ out_bits)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned long long b = 0;
+    if (i < n && x[i] > 0.0) b = (unsigned long long)__double_as_longlong(x[i]);
+    for (int o = 16; o; o >>= 1) { unsigned long long t = __shfl_xor_sync(0xffffffffu, b, o); b = t > b ? t : b; }
+    if ((threadIdx.x & 31) == 0 && b) atomicMax(out_bits, b);
+}
+
 __global__ void k_mark_class(int n, const uint8_t* __restrict__ cls, uint8_t which, uint32_t* __restrict__ mark)
 {
     int v = blockIdx.x * blockDim.x + threadIdx.x;
     if (v < n) mark[v] = cls[v] == which ? 1u : 0u;
 }
 
-// head / tail rule, per branch (costs are additive over branches, so the per-branch rule is optimal):
-//   tail  iff  C(n_v,2) * tail_cost  <  P * head_cost      (costs in seconds per update)
-// tcnt[v] = n_v for tail branches else 0 (scanned into the list offsets); counters[0..3] = head rows,
-// tail rows, tail pair updates, tail entries.
-__global__ void k_classify(int n, const uint32_t* __restrict__ nv, double pairs_times_ratio, uint32_t force,
+// head / mid / tail rule, per branch (costs are additive over branches, so a per-branch rule is optimal):
+//   C(n_v,2) >= c2_head            -> head  (dense kernel: cost per branch independent of n_v)
+//   c2_mid <= C(n_v,2) < c2_head   -> mid   (pair contributions accumulated per 128 x 128 tile pair in shared memory, mid.cuh)
+//   C(n_v,2) < c2_mid              -> tail  (pair contributions scattered with global RED.ADD, k_tail_scatter)
+// mid and tail branches share one list format; tcnt[v] = n_v for both (0 for head rows), scanned into the
+// list offsets.  counters[0..5] = head rows, tail rows, tail pair updates, list entries, mid rows, mid pair updates.
+__global__ void k_classify(int n, const uint32_t* __restrict__ nv, double c2_head, double c2_mid, uint32_t force,
                            uint8_t* __restrict__ cls, uint32_t* __restrict__ tcnt, unsigned long long* __restrict__ counters)
 {
     int v = blockIdx.x * blockDim.x + threadIdx.x;
-    unsigned long long h = 0, t = 0, tu = 0, te = 0;
+    unsigned long long h = 0, t = 0, tu = 0, te = 0, m = 0, mu = 0;
     if (v < n) {
         unsigned long long k = nv[v];
         uint8_t c = CLS_NONE;
         if (k) {
             double c2 = 0.5 * (double)k * (double)(k - 1);
-            bool tail = force == 2 ? true : force == 1 ? false : (c2 < pairs_times_ratio);
-            c = tail ? CLS_TAIL : CLS_HEAD;
-            if (tail) { t = 1; tu = k * (k - 1) / 2; te = k; } else h = 1;
+            c = force == 2 ? CLS_TAIL : force == 1 ? CLS_HEAD : c2 >= c2_head ? CLS_HEAD : c2 >= c2_mid ? CLS_MID : CLS_TAIL;
+            if (c == CLS_TAIL) { t = 1; tu = k * (k - 1) / 2; te = k; }
+            else if (c == CLS_MID) { m = 1; mu = k * (k - 1) / 2; te = k; }
+            else h = 1;
         }
         cls[v] = c;
-        tcnt[v] = c == CLS_TAIL ? (uint32_t)k : 0u;
+        tcnt[v] = (c == CLS_TAIL || c == CLS_MID) ? (uint32_t)k : 0u;
     }
     for (int o = 16; o; o >>= 1) {
         h += __shfl_xor_sync(0xffffffffu, h, o);  t += __shfl_xor_sync(0xffffffffu, t, o);
         tu += __shfl_xor_sync(0xffffffffu, tu, o); te += __shfl_xor_sync(0xffffffffu, te, o);
+        m += __shfl_xor_sync(0xffffffffu, m, o);  mu += __shfl_xor_sync(0xffffffffu, mu, o);
     }
-    if ((threadIdx.x & 31) == 0 && (h | t)) {
+    if ((threadIdx.x & 31) == 0 && (h | t | m)) {
         atomicAdd(&counters[0], h); atomicAdd(&counters[1], t); atomicAdd(&counters[2], tu); atomicAdd(&counters[3], te);
+        atomicAdd(&counters[4], m); atomicAdd(&counters[5], mu);
     }
 }
 
@@ -122,7 +137,7 @@ __global__ void k_tail_fill(int n, const uint8_t* __restrict__ cls, const double
 {
     int v = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     int lane = threadIdx.x & 31;
-    if (v >= n || cls[v] != CLS_TAIL) return;
+    if (v >= n || (cls[v] != CLS_TAIL && cls[v] != CLS_MID)) return;
     const double l = (!weighted && uval) ? uval[v] : len[v];
     uint32_t pos = tptr[v] + cursor[v];
     const uint32_t pos0 = pos;
@@ -222,7 +237,7 @@ struct TailParams {
     const uint32_t* seg;    // [n][nsup+1]
     const uint32_t* ts;     // sample ids
     const void* tv;         // values (T)
-    const uint32_t* tcnt;   // [n] (0 for non-tail rows)
+    const uint8_t* cls;     // [n] only CLS_TAIL rows are scattered here
     int n, nsup, SI, SJ;
     long long N;
     void* out;
@@ -248,7 +263,7 @@ k_tail_scatter(const TailParams P)
         if (chunk >= nchunks) break;
         const int v = chunk * 32 + lane;
         uint32_t i0 = 0, i1 = 0, j0 = 0, j1 = 0, base = 0;
-        if (v < P.n && P.tcnt[v]) {
+        if (v < P.n && P.cls[v] == CLS_TAIL) {
             const uint32_t* sg = P.seg + (size_t)v * (P.nsup + 1);
             i0 = sg[P.SI]; i1 = sg[P.SI + 1];
             if (diag) { j0 = i0; j1 = i1; } else { j0 = sg[P.SJ]; j1 = sg[P.SJ + 1]; }

@@ -8,6 +8,7 @@
 #include "tail.cuh"
 #include "stripe.cuh"
 #include "gram.cuh"
+#include "mid.cuh"
 
 #include <cstdio>
 #include <cstdlib>
@@ -203,17 +204,32 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     // R_tail / R_head is measured (RED.ADD rate in L2 vs dense stripe rate) and can be overridden
     const bool gram = std::is_same<T, float>::value && !weighted &&
                       !(flags & (UNIFRAC_FLAG_NO_TENSOR | UNIFRAC_FLAG_ABSDIFF | UNIFRAC_FLAG_LITERAL | UNIFRAC_FLAG_ALL_TAIL));
-    double ratio = gram ? 7.5e-4 : 0.022;
-    if (const char* e = getenv(gram ? "UNIFRAC_B200_TAIL_RATIO_GRAM" : "UNIFRAC_B200_TAIL_RATIO")) ratio = atof(e);
+    const bool mid_ok = std::is_same<T, float>::value &&
+                        !(flags & (UNIFRAC_FLAG_NO_MID | UNIFRAC_FLAG_NO_TAIL | UNIFRAC_FLAG_ABSDIFF | UNIFRAC_FLAG_LITERAL | UNIFRAC_FLAG_ALL_TAIL));
+    // Per-branch class thresholds on C(n_v,2) from measured rates (all can be
+    // overridden through the environment for tuning):
+    //   R_tail  global RED.ADD pair updates / s           R_mid   shared-memory integer-atomic pair updates / s
+    //   R_head  dense-equivalent pair updates / s of k_stripe;  Gram kernel: seconds per branch = tile pairs * 512 B / operand rate
+    const int n_tiles_c = cdiv(N, TILE);
+    const double Pd = 0.5 * (double)N * (double)(N - 1), n_tp = 0.5 * (double)n_tiles_c * (n_tiles_c + 1);
+    auto envd = [](const char* k, double d) { const char* e = getenv(k); return e ? atof(e) : d; };
+    const double R_tail = envd("UNIFRAC_B200_R_TAIL", 1.6e11), R_mid = envd("UNIFRAC_B200_R_MID", 6e11);
+    const double R_head = envd("UNIFRAC_B200_R_HEAD", 1.07e13), gram_Bps = envd("UNIFRAC_B200_GRAM_BPS", 6.0e12);
+    const double c_row = envd("UNIFRAC_B200_MID_ROW_S", 1e-10);          // seconds per (mid row, tile pair) visit
+    const double head_s = gram ? n_tp * 512.0 / gram_Bps : Pd / R_head;  // seconds per head branch
+    double c2_head, c2_mid;
+    if (mid_ok) { c2_head = head_s * R_mid; c2_mid = n_tp * c_row / (1.0 / R_tail - 1.0 / R_mid); if (c2_mid > c2_head) c2_mid = c2_head; }
+    else { c2_head = head_s * R_tail; c2_mid = INFINITY; }
     uint32_t force = 0;
     if (flags & (UNIFRAC_FLAG_NO_TAIL | UNIFRAC_FLAG_ABSDIFF | UNIFRAC_FLAG_LITERAL)) force = 1;   // NO_TAIL + Gram = dense GEMM over every branch
     else if (flags & UNIFRAC_FLAG_ALL_TAIL) force = 2;
-    k_classify<<<cdiv(n, TB), TB, 0, st>>>(n, nv, 0.5 * (double)N * (double)(N - 1) * ratio, force, cls, tcnt, work + 8); CU_LAUNCH(); ++launches;
+    k_classify<<<cdiv(n, TB), TB, 0, st>>>(n, nv, c2_head, c2_mid, force, cls, tcnt, work + 8); CU_LAUNCH(); ++launches;
     k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>(n, tcnt, tptr); CU_LAUNCH(); ++launches;
-    unsigned long long h_work[12];
+    unsigned long long h_work[14];
     CU(cudaMemcpyAsync(h_work, work, sizeof(h_work), cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
     const unsigned long long head_rows = h_work[8], tail_rows = h_work[9], tail_updates = h_work[10], tail_entries = h_work[11];
+    const unsigned long long mid_rows = h_work[12], mid_updates = h_work[13];
     if (tail_entries >= (1ull << 32)) throw StatusFail{UNIFRAC_ERR_UNSUPPORTED};
     uint32_t* ts = A.get_n<uint32_t>(tail_entries ? tail_entries : 1);
     T* tv = A.get_n<T>(tail_entries ? tail_entries : 1);
@@ -231,7 +247,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         uint32_t* hrank = A.get_n<uint32_t>((size_t)n + 1);
         k_mark_class<<<cdiv(n, TB), TB, 0, st>>>(n, cls, CLS_HEAD, is_head); CU_LAUNCH(); ++launches;
         k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>(n, is_head, hrank); CU_LAUNCH(); ++launches;
-        unsigned long long* lmax = work + 12;
+        unsigned long long* lmax = work + 14;
         k_gram_lenmax<<<cdiv(n, TB), TB, 0, st>>>(n, cls, len, lmax); CU_LAUNCH(); ++launches;
         unsigned long long h_lmax = 0;
         CU(cudaMemcpyAsync(&h_lmax, lmax, sizeof(h_lmax), cudaMemcpyDeviceToHost, st));
@@ -294,7 +310,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         k_side_sums_part<T><<<dim3(cdiv(s1 - s0, 32), cdiv(n_chunks, 8)), 256, 0, st>>>(n, parent, len, cnt, Wb, s0, s1, Tsum, weighted,
                                                                                         uval, n_chunks, sums_part); CU_LAUNCH(); ++launches;
         k_side_sums_reduce<<<cdiv(s1 - s0, TB), TB, 0, st>>>(s1 - s0, Wb, n_chunks, sums_part, s0, sums); CU_LAUNCH(); ++launches;
-        if (tail_rows) {
+        if (tail_rows || mid_rows) {
             k_tail_fill<T><<<cdiv((long long)n * 32, TB), TB, 0, st>>>(n, cls, len, cnt, Wb, s0, s1, Tsum, weighted, uval, tptr, tcursor, ts, tv);
             CU_LAUNCH(); ++launches;
         }
@@ -321,6 +337,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
 
     // ------------------------------------------------------------------ a-5 (tail branches): scatter into the condensed matrix
     unsigned tail_launches = 0;
+    if (tail_rows || mid_rows) CU(cudaMemsetAsync(out, 0, sizeof(T) * ((size_t)N * (N - 1) / 2), st));
     if (tail_rows) {
         // super tiles: SUP x SUP samples whose condensed row segments (SUP * SUP * sizeof(T)) stay L2-resident
         size_t l2_budget = (size_t)48 << 20;
@@ -330,7 +347,6 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         const int nsup = cdiv(N, SUP);
         uint32_t* seg = A.get_n<uint32_t>((size_t)n * (nsup + 1));
         k_tail_seg<<<cdiv((long long)n * (nsup + 1), TB), TB, 0, st>>>(n, tptr, ts, SUP, nsup, seg); CU_LAUNCH(); ++launches;
-        CU(cudaMemsetAsync(out, 0, sizeof(T) * ((size_t)N * (N - 1) / 2), st));
         const int n_launch = nsup * (nsup + 1) / 2;
         unsigned int* tcounters = A.get_n<unsigned int>(n_launch);
         CU(cudaMemsetAsync(tcounters, 0, sizeof(unsigned int) * n_launch, st));
@@ -338,13 +354,56 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         CU(cudaGetDevice(&dev));
         CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
         TailParams TP{};
-        TP.tptr = tptr; TP.seg = seg; TP.ts = ts; TP.tv = tv; TP.tcnt = tcnt; TP.n = n; TP.nsup = nsup; TP.N = N; TP.out = out;
+        TP.tptr = tptr; TP.seg = seg; TP.ts = ts; TP.tv = tv; TP.cls = cls; TP.n = n; TP.nsup = nsup; TP.N = N; TP.out = out;
         int li = 0;
         for (int si = 0; si < nsup; ++si)
             for (int sj = si; sj < nsup; ++sj) {
                 TP.SI = si; TP.SJ = sj; TP.counter = tcounters + li++;
                 k_tail_scatter<T><<<n_sm * 8, 256, 0, st>>>(TP); CU_LAUNCH(); ++launches; ++tail_launches;
             }
+    }
+    tm.mark();
+
+    // ------------------------------------------------------------------ a-5 (mid branches): per tile pair, fixed point in shared memory
+    unsigned mid_launches = 0;
+    int mid_F = 0;
+    if (mid_rows) {
+        if constexpr (std::is_same<T, float>::value) {
+            const uint32_t n_mid = (uint32_t)mid_rows;
+            uint32_t* mhist = A.get_n<uint32_t>((size_t)N + 2);
+            uint32_t* mcur = A.get_n<uint32_t>((size_t)N + 2);
+            int32_t* mrows = A.get_n<int32_t>(n_mid);
+            uint32_t* mbase = A.get_n<uint32_t>(n_mid);
+            CU(cudaMemsetAsync(mhist, 0, sizeof(uint32_t) * ((size_t)N + 2), st));
+            k_mid_hist<<<cdiv(n, TB), TB, 0, st>>>(n, cls, nv, mhist); CU_LAUNCH(); ++launches;
+            k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>(N + 1, mhist, mcur); CU_LAUNCH(); ++launches;
+            k_mid_rows<<<cdiv(n, TB), TB, 0, st>>>(n, cls, nv, mcur, tptr, mrows, mbase); CU_LAUNCH(); ++launches;
+            uint32_t* mseg = A.get_n<uint32_t>((size_t)(n_tiles + 1) * n_mid);
+            k_mid_seg<<<cdiv((long long)(n_tiles + 1) * n_mid, TB), TB, 0, st>>>(n_mid, mrows, tptr, ts, n_tiles, mseg); CU_LAUNCH(); ++launches;
+            unsigned long long* smax = work + 15;
+            k_max_positive<<<cdiv((long long)n_tiles * TILE, TB), TB, 0, st>>>(n_tiles * TILE, sums, smax); CU_LAUNCH(); ++launches;
+            unsigned long long h_smax = 0;
+            CU(cudaMemcpyAsync(&h_smax, smax, sizeof(h_smax), cudaMemcpyDeviceToHost, st));
+            std::vector<int2> h_mp = blocked_pairs(n_tiles, 12);
+            int2* mpairs = A.get_n<int2>(h_mp.size());
+            CU(cudaMemcpyAsync(mpairs, h_mp.data(), sizeof(int2) * h_mp.size(), cudaMemcpyHostToDevice, st));
+            CU(cudaStreamSynchronize(st));
+            double sm; memcpy(&sm, &h_smax, sizeof(sm));
+            int ex = 0; frexp(sm > 0 ? sm : 1.0, &ex);          // sm < 2^ex
+            mid_F = 30 - ex;                                     // acc <= min(R_a, R_b) * 2^F < 2^30 (+ rounding slack)
+            MidParams M{};
+            M.pairs = mpairs; M.n_pairs = (uint32_t)h_mp.size(); M.counter = reinterpret_cast<unsigned int*>(work + 7);
+            M.n_mid = n_mid; M.mbase = mbase; M.seg = mseg; M.ts = ts; M.tv = reinterpret_cast<const float*>(tv);
+            M.n_samples = N; M.out = reinterpret_cast<float*>(out); M.qscale = ldexpf(1.0f, mid_F); M.inv_qscale = ldexp(1.0, -mid_F);
+            CU(cudaFuncSetAttribute(k_mid, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MID_SMEM));
+            int occ = 0, dev2 = 0, n_sm2 = 0;
+            CU(cudaGetDevice(&dev2));
+            CU(cudaDeviceGetAttribute(&n_sm2, cudaDevAttrMultiProcessorCount, dev2));
+            CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_mid, MID_THREADS, MID_SMEM));
+            if (occ < 1) occ = 1;
+            k_mid<<<(unsigned)std::min<long long>((long long)n_sm2 * occ, (long long)h_mp.size()), MID_THREADS, MID_SMEM, st>>>(M);
+            CU_LAUNCH(); ++launches; ++mid_launches;
+        }
     }
     tm.mark();
 
@@ -368,7 +427,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             CUtensorMap tmB2 = make_u8_rowmajor_map(XG[3], Npad, K_pad, TILE, GRAM_BK);
             GramParams G{};
             G.pairs = pairs; G.n_pairs = n_pairs; G.K_pad = K_pad; G.sums = sums; G.n_samples = N;
-            G.out = reinterpret_cast<float*>(out); G.add_out = tail_rows ? 1 : 0; G.q = gram_q;
+            G.out = reinterpret_cast<float*>(out); G.add_out = (tail_rows || mid_rows) ? 1 : 0; G.q = gram_q;
             CU(cudaFuncSetAttribute(k_gram, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GRAM_SMEM));
             unsigned grid = (unsigned)std::min<long long>(n_sm, n_pairs);
             k_gram<<<grid, GRAM_THREADS, GRAM_SMEM, st>>>(tmA, tmB0, tmB1, tmB2, G); CU_LAUNCH(); ++launches; ++stripe_launches;
@@ -387,7 +446,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     uint32_t* counter = reinterpret_cast<uint32_t*>(work + 6);
 
     StripeParams P{};
-    P.add_out = tail_rows ? 1 : 0;
+    P.add_out = (tail_rows || mid_rows) ? 1 : 0;
     P.tileE = reinterpret_cast<const void* const*>(tileE);
     P.tileQ = tileQ; P.flags = rflags; P.rank = rrank; P.nwords = nwords;
     P.pairs = pairs; P.n_pairs = n_pairs; P.counter = counter; P.sums = sums;
@@ -424,6 +483,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     g_stats.embed_rows = embed_rows;
     g_stats.head_rows = head_rows; g_stats.tail_rows = tail_rows; g_stats.tail_updates = tail_updates; g_stats.tail_entries = tail_entries;
     g_stats.tail_launches = tail_launches;
+    g_stats.mid_rows = mid_rows; g_stats.mid_updates = mid_updates; g_stats.mid_launches = mid_launches; g_stats.mid_F = (uint32_t)mid_F;
     g_stats.gram = use_gram ? 1u : 0u; g_stats.gram_k = K_pad; g_stats.gram_q = (uint32_t)gram_q;
     g_stats.n_tile_pairs = n_pairs;
     g_stats.n_levels = (uint32_t)n_levels;
@@ -433,8 +493,8 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     g_stats.workspace_bytes = A.total;
     if (timing) {
         CU(cudaStreamSynchronize(st));
-        g_stats.ms_plan = tm.ms(0, 1); g_stats.ms_embed = tm.ms(1, 3); g_stats.ms_tail = tm.ms(3, 4); g_stats.ms_stripe = tm.ms(4, 5);
-        g_stats.ms_total = tm.ms(0, 5);
+        g_stats.ms_plan = tm.ms(0, 1); g_stats.ms_embed = tm.ms(1, 3); g_stats.ms_tail = tm.ms(3, 4); g_stats.ms_mid = tm.ms(4, 5); g_stats.ms_stripe = tm.ms(5, 6);
+        g_stats.ms_total = tm.ms(0, 6);
     }
 }
 
@@ -447,7 +507,7 @@ int guarded(int32_t n_nodes, const int32_t* parent, const double* len, const int
     if (variant != UNIFRAC_UNWEIGHTED && variant != UNIFRAC_WEIGHTED_NORMALIZED) return UNIFRAC_ERR_INVALID_ARG;
     if (precision != UNIFRAC_FP32 && precision != UNIFRAC_FP64) return UNIFRAC_ERR_INVALID_ARG;
     if (flags & ~(UNIFRAC_FLAG_LITERAL | UNIFRAC_FLAG_TENSOR_GRAM | UNIFRAC_FLAG_SKIP_VALIDATION | UNIFRAC_FLAG_ABSDIFF |
-                  UNIFRAC_FLAG_NO_TAIL | UNIFRAC_FLAG_ALL_TAIL | UNIFRAC_FLAG_NO_TENSOR))
+                  UNIFRAC_FLAG_NO_TAIL | UNIFRAC_FLAG_ALL_TAIL | UNIFRAC_FLAG_NO_TENSOR | UNIFRAC_FLAG_NO_MID))
         return UNIFRAC_ERR_INVALID_ARG;
     if ((long long)N > (1ll << 23)) return UNIFRAC_ERR_UNSUPPORTED;
     Arena A{alloc, user, st};
@@ -530,7 +590,7 @@ int unifrac_last_stats(unifrac_stats_t* out)
         if (cudaEventSynchronize(g_stats_event) != cudaSuccess) { cudaGetLastError(); return UNIFRAC_ERR_CUDA; }
         g_stats.updates_executed_head = g_stats_pinned[0] * 2048ull;    // one (warp,row) = 32 x 64 pair updates
         if (g_stats.gram) g_stats.updates_executed_head = g_stats.head_rows * ((uint64_t)g_stats.updates_dense / (g_stats.branches_embedded ? g_stats.branches_embedded : 1));
-        g_stats.updates_executed = g_stats.updates_executed_head + g_stats.tail_updates;
+        g_stats.updates_executed = g_stats.updates_executed_head + g_stats.tail_updates + g_stats.mid_updates;
         g_stats.rows_staged = g_stats_pinned[1];
         g_stats_pending = false;
     }

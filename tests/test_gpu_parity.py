@@ -44,7 +44,7 @@ def check(got, want, precision):
 
 @pytest.mark.parametrize("variant", [U, W])
 @pytest.mark.parametrize("precision", [1, 0])
-@pytest.mark.parametrize("flags", [0, 16, 32, 8, 1])   # head/tail split (default), all head, all tail, direct |u-v| form, literal
+@pytest.mark.parametrize("flags", [0, 128, 16, 32, 8, 1])   # head/mid/tail split (default), no mid, all head, all tail, direct |u-v| form, literal
 def test_tiny_all_pairs(B, O, variant, precision, flags):
     p = synth.make_config("tiny", seed=0)
     want = O.all_pairs(p.parent, p.branch_len, p.indptr, p.indices, p.counts, variant)
@@ -53,7 +53,7 @@ def test_tiny_all_pairs(B, O, variant, precision, flags):
 
 @pytest.mark.parametrize("variant", [U, W])
 @pytest.mark.parametrize("precision", [1, 0])
-@pytest.mark.parametrize("flags", [0, 16, 32, 8])
+@pytest.mark.parametrize("flags", [0, 128, 64, 16, 32, 8])
 def test_three_tiles_ragged_tail_all_pairs(B, O, variant, precision, flags):
     """300 samples = 2 full 128-tiles + a 44-sample tail; 3000 tips -> 5998 branches (several stages)."""
     p = synth.make_problem(3000, 300, 0.1, 1.1, synth.CONFIGS["small"][4], synth.CONFIGS["small"][5], seed=3)
@@ -102,7 +102,7 @@ def test_general_trees_multifurcation_unary_zero_length(B, O, seed):
         want = O.all_pairs(p.parent, p.branch_len, p.indptr, p.indices, p.counts, variant)
         for flags in (0, 16, 32, 8, 1):
             check(gpu_dm(B, p, variant, 1, flags), want, 1)
-        for flags in (0, 16, 32, 64, 64 + 16):
+        for flags in (0, 16, 32, 64, 64 + 16, 128, 64 + 128):
             check(gpu_dm(B, p, variant, 0, flags), want, 0)
 
 
@@ -151,7 +151,8 @@ def test_small_config_sampled_pairs(B, O):
         check(got32[idx], want, 0)
         assert np.all(got >= 0) and np.all(got <= 1)
         st = B.unifrac_last_stats()
-        assert st["head_rows"] > 0 and st["tail_rows"] > 0          # the default split uses both paths here
+        assert st["head_rows"] > 0 and st["tail_rows"] > 0 and st["mid_rows"] > 0     # the default split uses all three paths here
+        check(gpu_dm(B, p, variant, 0, flags=128)[idx], want, 0)    # head + tail only
         check(gpu_dm(B, p, variant, 0, flags=16)[idx], want, 0)     # all head
         check(gpu_dm(B, p, variant, 0, flags=64)[idx], want, 0)     # CUDA-core head for unweighted too
 
@@ -224,7 +225,7 @@ def test_stats_work_counters_match_definitions(B):
     assert st["updates_inter"] == int((nv * (nv - 1) // 2).sum())
     assert st["updates_union"] == int((N * (N - 1) // 2 - (N - nv) * (N - nv - 1) // 2)[nv > 0].sum())
     assert st["updates_executed"] > 0 and st["kernel_launches"] > 0 and st["stripe_launches"] == 1
-    assert st["head_rows"] + st["tail_rows"] == st["branches_embedded"]
+    assert st["head_rows"] + st["tail_rows"] + st["mid_rows"] == st["branches_embedded"]
     tail = nv[(nv > 0)]
     B.unifrac_dm(*B.to_device(p), p.n_samples, U, B.FP64, flags=B.FLAG_ALL_TAIL)
     torch.cuda.synchronize()
