@@ -14,7 +14,7 @@
 //
 // Steps:  bit-packed presence up the tree (a-1/a-2 on bits, BASELINE.json:5 "presence bits,
 // bit-packed in 32/64-sample words ... level by level")  ->  n_v (popcount)  ->  classification
-// ->  per-batch fill of the tail lists  ->  super-tile segment offsets  ->  scatter.
+// ->  sparse values / sample lists (embed.cuh, k_values)  ->  super-tile segment offsets  ->  scatter.
 #pragma once
 #include "common.cuh"
 
@@ -55,22 +55,22 @@ __global__ void k_bits_pull(const int32_t* __restrict__ nodes, int n_nodes_level
     bits[(size_t)v * NW4 + ch] = acc;
 }
 
-// n_v = popcount of row v (one warp per node); rows of the root / zero-length branches count as 0
+// ne[v] = popcount of row v (0 for the root); n_v = ne[v] if the branch has a positive length, else 0.  One warp per node.
 __global__ void k_bits_count(int n, const int32_t* __restrict__ parent, const double* __restrict__ len,
-                             const uint4* __restrict__ bits, uint32_t NW4, uint32_t* __restrict__ nv)
+                             const uint4* __restrict__ bits, uint32_t NW4, uint32_t* __restrict__ nv, uint32_t* __restrict__ ne)
 {
     int v = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     int lane = threadIdx.x & 31;
     if (v >= n) return;
     uint32_t c = 0;
-    if (parent[v] >= 0 && len[v] > 0.0) {
+    if (parent[v] >= 0) {
         for (uint32_t k = lane; k < NW4; k += 32) {
             uint4 x = bits[(size_t)v * NW4 + k];
             c += __popc(x.x) + __popc(x.y) + __popc(x.z) + __popc(x.w);
         }
     }
     for (int o = 16; o; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
-    if (lane == 0) nv[v] = c;
+    if (lane == 0) { ne[v] = c; nv[v] = len[v] > 0.0 ? c : 0u; }
 }
 
 // max over a vector of non-negative doubles (bit patterns order like the values)
@@ -94,8 +94,9 @@ __global__ void k_mark_class(int n, const uint8_t* __restrict__ cls, uint8_t whi
 //   c2_mid <= C(n_v,2) < c2_head   -> mid   (pair contributions accumulated per 128 x 128 tile pair in shared memory, mid.cuh)
 //   C(n_v,2) < c2_mid              -> tail  (pair contributions scattered with global RED.ADD, k_tail_scatter)
 // mid and tail branches share one list format; tcnt[v] = n_v for both (0 for head rows), scanned into the
-// list offsets.  counters[0..5] = head rows, tail rows, tail pair updates, list entries, mid rows, mid pair updates.
-__global__ void k_classify(int n, const uint32_t* __restrict__ nv, double c2_head, double c2_mid, uint32_t force,
+// list offsets.  counters[0..5] = head rows, tail rows, tail pair updates, list entries (all rows that keep a list), mid rows, mid pair updates.
+__global__ void k_classify(int n, const uint32_t* __restrict__ nv, const uint32_t* __restrict__ ne, int all_rows,
+                           double c2_head, double c2_mid, uint32_t force,
                            uint8_t* __restrict__ cls, uint32_t* __restrict__ tcnt, unsigned long long* __restrict__ counters)
 {
     int v = blockIdx.x * blockDim.x + threadIdx.x;
@@ -106,12 +107,16 @@ __global__ void k_classify(int n, const uint32_t* __restrict__ nv, double c2_hea
         if (k) {
             double c2 = 0.5 * (double)k * (double)(k - 1);
             c = force == 2 ? CLS_TAIL : force == 1 ? CLS_HEAD : c2 >= c2_head ? CLS_HEAD : c2 >= c2_mid ? CLS_MID : CLS_TAIL;
-            if (c == CLS_TAIL) { t = 1; tu = k * (k - 1) / 2; te = k; }
-            else if (c == CLS_MID) { m = 1; mu = k * (k - 1) / 2; te = k; }
+            if (c == CLS_TAIL) { t = 1; tu = k * (k - 1) / 2; }
+            else if (c == CLS_MID) { m = 1; mu = k * (k - 1) / 2; }
             else h = 1;
         }
         cls[v] = c;
-        tcnt[v] = (c == CLS_TAIL || c == CLS_MID) ? (uint32_t)k : 0u;
+        // rows that keep an entry list: mid and tail rows; all_rows (weighted): every row with a present sample,
+        // zero-length branches included (their counts still propagate to the parent)
+        const uint32_t keep = all_rows ? ne[v] : ((c == CLS_TAIL || c == CLS_MID) ? (uint32_t)k : 0u);
+        tcnt[v] = keep;
+        te = keep;
     }
     for (int o = 16; o; o >>= 1) {
         h += __shfl_xor_sync(0xffffffffu, h, o);  t += __shfl_xor_sync(0xffffffffu, t, o);
@@ -124,41 +129,7 @@ __global__ void k_classify(int n, const uint32_t* __restrict__ nv, double c2_hea
     }
 }
 
-// ------------------------------------------------------------------ tail lists, filled batch by batch
-// One warp per node; tail rows append (sample id, u~) for the samples of this batch, in sample order.
-// 64-bit list offsets: tptr[v] (exclusive scan of tcnt) + cursor[v] (entries written by earlier batches).
-template <typename T>
-__global__ void k_tail_fill(int n, const uint8_t* __restrict__ cls, const double* __restrict__ len,
-                            const uint32_t* __restrict__ cnt, int Wb, int s0, int s1,
-                            const unsigned long long* __restrict__ Tsum, int weighted,
-                            const double* __restrict__ uval /* unweighted: embedded value per branch, or NULL = len */,
-                            const uint32_t* __restrict__ tptr, uint32_t* __restrict__ cursor,
-                            uint32_t* __restrict__ ts, T* __restrict__ tv)
-{
-    int v = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    int lane = threadIdx.x & 31;
-    if (v >= n || (cls[v] != CLS_TAIL && cls[v] != CLS_MID)) return;
-    const double l = (!weighted && uval) ? uval[v] : len[v];
-    uint32_t pos = tptr[v] + cursor[v];
-    const uint32_t pos0 = pos;
-    const int W = s1 - s0;
-    const uint32_t* row = cnt + (size_t)v * Wb;
-    for (int c0 = 0; c0 < W; c0 += 32) {
-        int c = c0 + lane;
-        uint32_t x = c < W ? row[c] : 0u;
-        uint32_t m = __ballot_sync(0xffffffffu, x != 0);
-        if (!m) continue;
-        if (x) {
-            uint32_t p = pos + __popc(m & ((1u << lane) - 1u));
-            double val = weighted ? l * ((double)x / (double)Tsum[s0 + c]) : l;
-            ts[p] = (uint32_t)(s0 + c);
-            tv[p] = (T)val;
-        }
-        pos += __popc(m);
-    }
-    if (lane == 0 && pos != pos0) cursor[v] += pos - pos0;
-}
-
+// ------------------------------------------------------------------ super-tile segments of the lists
 // seg[v][k] = number of entries of row v with sample id < k*SUP, k = 0..nsup   (thread per (v,k))
 __global__ void k_tail_seg(int n, const uint32_t* __restrict__ tptr, const uint32_t* __restrict__ ts,
                            int SUP, int nsup, uint32_t* __restrict__ seg)
@@ -175,54 +146,6 @@ __global__ void k_tail_seg(int n, const uint32_t* __restrict__ tptr, const uint3
         if (ts[mid] < key) lo = mid + 1; else hi = mid;
     }
     seg[(size_t)v * (nsup + 1) + k] = lo - lo0;
-}
-
-// ------------------------------------------------------------------ per-sample side sums (deterministic)
-// part[chunk][c] = sum over the nodes v of the chunk of u~_{s0+c, v}; lane <-> sample, warp <-> chunk.
-template <typename T>
-__global__ void k_side_sums_part(int n, const int32_t* __restrict__ parent, const double* __restrict__ len,
-                                 const uint32_t* __restrict__ cnt, int Wb, int s0, int s1,
-                                 const unsigned long long* __restrict__ Tsum, int weighted,
-                                 const double* __restrict__ uval, int n_chunks, double* __restrict__ part)
-{
-    const int strip = blockIdx.x;                       // 32 samples
-    const int chunk = blockIdx.y * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    const int lane = threadIdx.x & 31;
-    if (chunk >= n_chunks) return;
-    const int c = strip * 32 + lane;
-    const bool ok = s0 + c < s1;
-    const double Ts = ok ? (double)Tsum[s0 + c] : 1.0;
-    const long long per = ((long long)n + n_chunks - 1) / n_chunks;
-    long long v0 = chunk * per, v1 = v0 + per;
-    if (v1 > n) v1 = n;
-    double acc = 0.0;
-    constexpr int U = 8;                                 // loads in flight per lane
-    for (long long vb = v0; vb < v1; vb += U) {
-        uint32_t x[U];
-#pragma unroll
-        for (int u = 0; u < U; ++u) x[u] = vb + u < v1 ? cnt[(size_t)(vb + u) * Wb + c] : 0u;
-#pragma unroll
-        for (int u = 0; u < U; ++u) {
-            if (x[u]) {
-                const long long v = vb + u;
-                const double l = len[v];
-                if (parent[v] >= 0 && l > 0.0) {
-                    double val = weighted ? l * ((double)x[u] / Ts) : (uval ? uval[v] : l);
-                    acc += (double)(T)val;
-                }
-            }
-        }
-    }
-    if (ok) part[(size_t)chunk * Wb + c] = acc;
-}
-__global__ void k_side_sums_reduce(int W, int Wb, int n_chunks, const double* __restrict__ part, int s0,
-                                   double* __restrict__ sums)
-{
-    int c = blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= W) return;
-    double s = 0.0;
-    for (int k = 0; k < n_chunks; ++k) s += part[(size_t)k * Wb + c];
-    sums[s0 + c] = s;
 }
 
 // ------------------------------------------------------------------ the scatter

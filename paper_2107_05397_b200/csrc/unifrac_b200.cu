@@ -178,14 +178,15 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     k_child_fill<<<cdiv(n, TB), TB, 0, st>>>(n, parent, child_cur, child_idx); CU_LAUNCH(); ++launches;
     tm.mark();
 
-    // ------------------------------------------------------------------ a-1/a-2 on presence bits -> n_v -> head/tail classes
+    // ------------------------------------------------------------------ a-1/a-2 on presence bits -> n_v -> head/mid/tail classes
     const uint32_t NW = ((uint32_t)cdiv(N, 32) + 3u) & ~3u, NW4 = NW / 4;
     uint32_t* nv = A.get_n<uint32_t>(n);
+    uint32_t* ne = A.get_n<uint32_t>(n);
     uint8_t* cls = A.get_n<uint8_t>(n);
     uint32_t* tcnt = A.get_n<uint32_t>(n);
     uint32_t* tptr = A.get_n<uint32_t>((size_t)n + 1);
-    unsigned long long* work = A.get_n<unsigned long long>(16);
-    CU(cudaMemsetAsync(work, 0, sizeof(unsigned long long) * 16, st));
+    unsigned long long* work = A.get_n<unsigned long long>(24);
+    CU(cudaMemsetAsync(work, 0, sizeof(unsigned long long) * 24, st));
     uint32_t* bits = A.get_n<uint32_t>((size_t)n * NW);
     {
         CU(cudaMemsetAsync(bits, 0, sizeof(uint32_t) * (size_t)n * NW, st));
@@ -197,11 +198,9 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
                                                                        reinterpret_cast<uint4*>(bits), NW4);
             CU_LAUNCH(); ++launches;
         }
-        k_bits_count<<<cdiv((long long)n * 32, TB), TB, 0, st>>>(n, parent, len, reinterpret_cast<const uint4*>(bits), NW4, nv); CU_LAUNCH(); ++launches;
+        k_bits_count<<<cdiv((long long)n * 32, TB), TB, 0, st>>>(n, parent, len, reinterpret_cast<const uint4*>(bits), NW4, nv, ne); CU_LAUNCH(); ++launches;
     }
     k_work_counts<<<cdiv(n, TB), TB, 0, st>>>(n, nv, (unsigned long long)N, work); CU_LAUNCH(); ++launches;
-    // per-branch rule: tail iff C(n_v,2) / R_tail < P / R_head; the ratio
-    // R_tail / R_head is measured (RED.ADD rate in L2 vs dense stripe rate) and can be overridden
     const bool gram = std::is_same<T, float>::value && !weighted &&
                       !(flags & (UNIFRAC_FLAG_NO_TENSOR | UNIFRAC_FLAG_ABSDIFF | UNIFRAC_FLAG_LITERAL | UNIFRAC_FLAG_ALL_TAIL));
     const bool mid_ok = std::is_same<T, float>::value &&
@@ -210,8 +209,8 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     // overridden through the environment for tuning):
     //   R_tail  global RED.ADD pair updates / s           R_mid   shared-memory integer-atomic pair updates / s
     //   R_head  dense-equivalent pair updates / s of k_stripe;  Gram kernel: seconds per branch = tile pairs * 512 B / operand rate
-    const int n_tiles_c = cdiv(N, TILE);
-    const double Pd = 0.5 * (double)N * (double)(N - 1), n_tp = 0.5 * (double)n_tiles_c * (n_tiles_c + 1);
+    const int n_tiles = cdiv(N, TILE);
+    const double Pd = 0.5 * (double)N * (double)(N - 1), n_tp = 0.5 * (double)n_tiles * (n_tiles + 1);
     auto envd = [](const char* k, double d) { const char* e = getenv(k); return e ? atof(e) : d; };
     const double R_tail = envd("UNIFRAC_B200_R_TAIL", 1.6e11), R_mid = envd("UNIFRAC_B200_R_MID", 6e11);
     const double R_head = envd("UNIFRAC_B200_R_HEAD", 1.07e13), gram_Bps = envd("UNIFRAC_B200_GRAM_BPS", 6.0e12);
@@ -223,18 +222,24 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     uint32_t force = 0;
     if (flags & (UNIFRAC_FLAG_NO_TAIL | UNIFRAC_FLAG_ABSDIFF | UNIFRAC_FLAG_LITERAL)) force = 1;   // NO_TAIL + Gram = dense GEMM over every branch
     else if (flags & UNIFRAC_FLAG_ALL_TAIL) force = 2;
-    k_classify<<<cdiv(n, TB), TB, 0, st>>>(n, nv, c2_head, c2_mid, force, cls, tcnt, work + 8); CU_LAUNCH(); ++launches;
+    // the weighted variant keeps an entry list (counts -> values) for every row; unweighted only for mid / tail rows
+    k_classify<<<cdiv(n, TB), TB, 0, st>>>(n, nv, ne, weighted, c2_head, c2_mid, force, cls, tcnt, work + 8); CU_LAUNCH(); ++launches;
     k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>(n, tcnt, tptr); CU_LAUNCH(); ++launches;
-    unsigned long long h_work[14];
+    uint32_t* cptr = nullptr;                                  // weighted: by-tip (CSC) offsets of the table
+    if (weighted) {
+        uint32_t* tipc = A.get_n<uint32_t>(n);
+        cptr = A.get_n<uint32_t>((size_t)n + 1);
+        k_tip_mark<<<cdiv(n, TB), TB, 0, st>>>(n, child_count, ne, tipc, work + 16); CU_LAUNCH(); ++launches;
+        k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>(n, tipc, cptr); CU_LAUNCH(); ++launches;
+    }
+    unsigned long long h_work[17];
     CU(cudaMemcpyAsync(h_work, work, sizeof(h_work), cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
     const unsigned long long head_rows = h_work[8], tail_rows = h_work[9], tail_updates = h_work[10], tail_entries = h_work[11];
-    const unsigned long long mid_rows = h_work[12], mid_updates = h_work[13];
-    if (tail_entries >= (1ull << 32)) throw StatusFail{UNIFRAC_ERR_UNSUPPORTED};
+    const unsigned long long mid_rows = h_work[12], mid_updates = h_work[13], nnz_pos = h_work[16];
+    if (tail_entries >= (1ull << 32) || nnz_pos >= (1ull << 32)) throw StatusFail{UNIFRAC_ERR_UNSUPPORTED};
     uint32_t* ts = A.get_n<uint32_t>(tail_entries ? tail_entries : 1);
     T* tv = A.get_n<T>(tail_entries ? tail_entries : 1);
-    uint32_t* tcursor = A.get_n<uint32_t>(n);
-    CU(cudaMemsetAsync(tcursor, 0, sizeof(uint32_t) * n, st));
 
     // ------------------------------------------------------------------ tensor-core Gram path: u8 operand matrices from the bits
     bool use_gram = gram && head_rows > 0 && head_rows < (1ull << 23);
@@ -242,11 +247,15 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     uint8_t* XG[4] = {nullptr, nullptr, nullptr, nullptr};
     uint32_t K_pad = 0;
     int gram_q = 0;
-    if (use_gram) {
+    uint32_t* hrank = nullptr;                                 // head rank of every node (exclusive scan of the head marks)
+    int32_t* hrows = nullptr;                                  // head rank -> node id
+    if (head_rows > 0 && (use_gram || weighted)) {
         uint32_t* is_head = A.get_n<uint32_t>(n);
-        uint32_t* hrank = A.get_n<uint32_t>((size_t)n + 1);
+        hrank = A.get_n<uint32_t>((size_t)n + 1);
         k_mark_class<<<cdiv(n, TB), TB, 0, st>>>(n, cls, CLS_HEAD, is_head); CU_LAUNCH(); ++launches;
         k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>(n, is_head, hrank); CU_LAUNCH(); ++launches;
+    }
+    if (use_gram) {
         unsigned long long* lmax = work + 14;
         k_gram_lenmax<<<cdiv(n, TB), TB, 0, st>>>(n, cls, len, lmax); CU_LAUNCH(); ++launches;
         unsigned long long h_lmax = 0;
@@ -258,7 +267,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         const uint32_t K = (uint32_t)head_rows;
         K_pad = (K + GRAM_BK - 1) / GRAM_BK * GRAM_BK;
         const size_t Npad = (size_t)NW * 32;
-        int32_t* hrows = A.get_n<int32_t>(K_pad);
+        hrows = A.get_n<int32_t>(K_pad);
         uint32_t* Lq = A.get_n<uint32_t>(K_pad);
         uval = A.get_n<double>(n);
         for (auto& x : XG) x = A.get_n<uint8_t>((size_t)K_pad * Npad);
@@ -268,70 +277,74 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     }
     tm.mark();
 
-    // ------------------------------------------------------------------ a-1 .. a-4 embedding, per sample batch
-    const int n_tiles = cdiv(N, TILE);
-    const uint32_t nwords = (uint32_t)cdiv(n, 32);
-    size_t batch_budget = (size_t)4 << 30;                      // bytes of the dense count buffer
-    if (const char* e = getenv("UNIFRAC_B200_BATCH_MB")) batch_budget = (size_t)atoll(e) << 20;
-    long long tiles_per_batch = (long long)(batch_budget / ((size_t)n * TILE * 4));
-    if (tiles_per_batch < 1) tiles_per_batch = 1;
-    if (tiles_per_batch > n_tiles) tiles_per_batch = n_tiles;
-    const int Wb = (int)tiles_per_batch * TILE;
-
-    uint32_t* cnt = A.get_n<uint32_t>((size_t)n * Wb);
-    uint32_t* rflags = A.get_n<uint32_t>((size_t)n_tiles * nwords);
-    uint32_t* rrank = A.get_n<uint32_t>((size_t)n_tiles * nwords);
-    uint32_t* rows = A.get_n<uint32_t>(n_tiles);
-    uint8_t* qtmp = A.get_n<uint8_t>((size_t)tiles_per_batch * n);
-    double* sums = A.get_n<double>((size_t)n_tiles * TILE);
-    const int n_chunks = 512;
-    double* sums_part = A.get_n<double>((size_t)n_chunks * Wb);
-    T** tileE = A.get_n<T*>(n_tiles);
-    uint8_t** tileQ = A.get_n<uint8_t*>(n_tiles);
-    CU(cudaMemsetAsync(sums, 0, sizeof(double) * (size_t)n_tiles * TILE, st));
-    std::vector<uint32_t> h_rows(n_tiles);
-    std::vector<T*> h_tileE(n_tiles);
-    std::vector<uint8_t*> h_tileQ(n_tiles);
-    uint64_t embed_rows = 0;
-
-    for (int t0 = 0; t0 < n_tiles; t0 += (int)tiles_per_batch) {
-        const int tb = (int)std::min<long long>(tiles_per_batch, n_tiles - t0);
-        const int s0 = t0 * TILE, s1 = std::min(N, (t0 + tb) * TILE);
-        CU(cudaMemsetAsync(cnt, 0, sizeof(uint32_t) * (size_t)n * Wb, st));
-        k_tip_scatter<<<cdiv((long long)(s1 - s0) * 32, TB), TB, 0, st>>>(s0, s1, tab.indptr, tab.indices, tab.counts, cnt, Wb);
-        CU_LAUNCH(); ++launches;
+    // ------------------------------------------------------------------ a-1 / a-2 counts in rank layout (weighted only)
+    uint32_t* cnt = nullptr;
+    if (weighted) {
+        cnt = A.get_n<uint32_t>(tail_entries ? tail_entries : 1);
+        uint32_t* csc_s = A.get_n<uint32_t>(nnz_pos ? nnz_pos : 1);
+        uint32_t* csc_c = A.get_n<uint32_t>(nnz_pos ? nnz_pos : 1);
+        uint32_t* ccur = A.get_n<uint32_t>(n);
+        CU(cudaMemsetAsync(ccur, 0, sizeof(uint32_t) * n, st));
+        k_csc_fill<<<cdiv((long long)N * 32, TB), TB, 0, st>>>(N, tab.indptr, tab.indices, tab.counts, cptr, ccur, csc_s, csc_c); CU_LAUNCH(); ++launches;
+        int dev0 = 0, n_sm0 = 0;
+        CU(cudaGetDevice(&dev0));
+        CU(cudaDeviceGetAttribute(&n_sm0, cudaDevAttrMultiProcessorCount, dev0));
+        int wpb = (int)std::min<size_t>(8, ((size_t)96 << 10) / ((size_t)NW * 4));
+        if (wpb < 1) throw StatusFail{UNIFRAC_ERR_UNSUPPORTED};
+        const size_t tsm = (size_t)wpb * NW * 4;
+        CU(cudaFuncSetAttribute(k_tip_cnt, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tsm));
+        k_tip_cnt<<<n_sm0 * 8, wpb * 32, tsm, st>>>(n, child_count, ne, cptr, csc_s, csc_c, bits, NW, tptr, cnt); CU_LAUNCH(); ++launches;
         for (int d = n_levels - 1; d >= 0; --d) {            // deepest parents first
             const uint32_t cntl = h_hist[d];
             if (!cntl) continue;
-            const long long threads = (long long)cntl * (Wb / 4);
-            k_level_pull<<<cdiv(threads, TB), TB, 0, st>>>(level_nodes + h_off[d], (int)cntl, root, child_off, child_idx, cnt, Wb);
+            k_cnt_pull<<<cdiv((long long)cntl * 32, TB), TB, 0, st>>>(level_nodes + h_off[d], (int)cntl, root, child_off, child_idx,
+                                                                     bits, NW, tptr, cnt);
             CU_LAUNCH(); ++launches;
         }
-        k_side_sums_part<T><<<dim3(cdiv(s1 - s0, 32), cdiv(n_chunks, 8)), 256, 0, st>>>(n, parent, len, cnt, Wb, s0, s1, Tsum, weighted,
-                                                                                        uval, n_chunks, sums_part); CU_LAUNCH(); ++launches;
-        k_side_sums_reduce<<<cdiv(s1 - s0, TB), TB, 0, st>>>(s1 - s0, Wb, n_chunks, sums_part, s0, sums); CU_LAUNCH(); ++launches;
-        if (tail_rows || mid_rows) {
-            k_tail_fill<T><<<cdiv((long long)n * 32, TB), TB, 0, st>>>(n, cls, len, cnt, Wb, s0, s1, Tsum, weighted, uval, tptr, tcursor, ts, tv);
-            CU_LAUNCH(); ++launches;
-        }
-        if (use_gram) continue;        // head branches go through the u8 operand matrices, not the compact fp rows
-        k_row_flags<<<dim3(nwords, tb), 1024, 0, st>>>(n, parent, len, cnt, Wb, rflags, nwords, t0, qtmp, cls); CU_LAUNCH(); ++launches;
-        k_rank_scan<<<tb, 1024, 0, st>>>(rflags, rrank, nwords, t0, rows); CU_LAUNCH(); ++launches;
-        CU(cudaMemcpyAsync(h_rows.data() + t0, rows + t0, sizeof(uint32_t) * tb, cudaMemcpyDeviceToHost, st));
+    }
+    // ------------------------------------------------------------------ a-3 / a-4 values, sample ids, side sums
+    double* sums = A.get_n<double>((size_t)n_tiles * TILE);
+    CU(cudaMemsetAsync(sums, 0, sizeof(double) * (size_t)n_tiles * TILE, st));
+    k_values<T><<<cdiv((long long)n * 32, TB), TB, 0, st>>>(n, nv, tcnt, tptr, len, uval, bits, NW, cnt, Tsum, ts, tv, sums); CU_LAUNCH(); ++launches;
+
+    // ------------------------------------------------------------------ head rows of the CUDA-core stripe kernel: compact dense per-tile rows
+    const uint32_t nwords = (uint32_t)cdiv(n, 32);
+    uint32_t* rflags = nullptr; uint32_t* rrank = nullptr;
+    T** tileE = nullptr; uint8_t** tileQ = nullptr;
+    uint64_t embed_rows = 0;
+    if (!use_gram) {
+        rflags = A.get_n<uint32_t>((size_t)n_tiles * nwords);
+        rrank = A.get_n<uint32_t>((size_t)n_tiles * nwords);
+        uint32_t* rows = A.get_n<uint32_t>(n_tiles);
+        tileE = A.get_n<T*>(n_tiles);
+        tileQ = A.get_n<uint8_t*>(n_tiles);
+        k_head_flags<<<cdiv((long long)nwords * 32, TB), TB, 0, st>>>(n, cls, bits, NW, n_tiles, rflags, nwords); CU_LAUNCH(); ++launches;
+        k_rank_scan<<<n_tiles, 1024, 0, st>>>(rflags, rrank, nwords, 0, rows); CU_LAUNCH(); ++launches;
+        std::vector<uint32_t> h_rows(n_tiles);
+        CU(cudaMemcpyAsync(h_rows.data(), rows, sizeof(uint32_t) * n_tiles, cudaMemcpyDeviceToHost, st));
         CU(cudaStreamSynchronize(st));
-        size_t tot = 0;
-        for (int t = t0; t < t0 + tb; ++t) tot += h_rows[t];
-        embed_rows += tot;
-        T* Eb = A.get_n<T>((tot ? tot : 1) * TILE);
-        uint8_t* Qb = A.get_n<uint8_t>(tot ? tot : 1);
+        for (int t = 0; t < n_tiles; ++t) embed_rows += h_rows[t];
+        T* Eb = A.get_n<T>((embed_rows ? embed_rows : 1) * TILE);
+        uint8_t* Qb = A.get_n<uint8_t>(embed_rows ? embed_rows : 1);
+        std::vector<T*> h_tileE(n_tiles);
+        std::vector<uint8_t*> h_tileQ(n_tiles);
         size_t run_rows = 0;
-        for (int t = t0; t < t0 + tb; ++t) { h_tileE[t] = Eb + run_rows * TILE; h_tileQ[t] = Qb + run_rows; run_rows += h_rows[t]; }
-        CU(cudaMemcpyAsync(tileE + t0, h_tileE.data() + t0, sizeof(T*) * tb, cudaMemcpyHostToDevice, st));
-        CU(cudaMemcpyAsync(tileQ + t0, h_tileQ.data() + t0, sizeof(uint8_t*) * tb, cudaMemcpyHostToDevice, st));
-        k_compact<T><<<dim3(cdiv(nwords, COMPACT_WORDS), tb), 256, 0, st>>>(n, len, cnt, Wb, rflags, rrank, nwords, t0, Tsum, N,
-                                                                             weighted, tileE, tileQ, qtmp);
-        CU_LAUNCH(); ++launches;
-        CU(cudaStreamSynchronize(st));   // h_tileE/h_tileQ staging copies are done; safe to reuse cnt
+        for (int t = 0; t < n_tiles; ++t) { h_tileE[t] = Eb + run_rows * TILE; h_tileQ[t] = Qb + run_rows; run_rows += h_rows[t]; }
+        CU(cudaMemcpyAsync(tileE, h_tileE.data(), sizeof(T*) * n_tiles, cudaMemcpyHostToDevice, st));
+        CU(cudaMemcpyAsync(tileQ, h_tileQ.data(), sizeof(uint8_t*) * n_tiles, cudaMemcpyHostToDevice, st));
+        uint32_t* hpref = nullptr;
+        if (weighted && head_rows > 0) {
+            hrows = A.get_n<int32_t>(head_rows);
+            hpref = A.get_n<uint32_t>((size_t)head_rows * n_tiles);
+            k_head_rows<<<cdiv(n, TB), TB, 0, st>>>(n, cls, hrank, hrows); CU_LAUNCH(); ++launches;
+            k_head_pref<<<cdiv((long long)head_rows * 32, TB), TB, 0, st>>>((uint32_t)head_rows, hrows, bits, NW, n_tiles, hpref); CU_LAUNCH(); ++launches;
+        }
+        if (embed_rows) {
+            k_compact<T><<<dim3(cdiv(nwords, COMPACT_WORDS), n_tiles), 256, 0, st>>>(n, len, bits, NW, rflags, rrank, nwords, n_tiles, tptr, hrank, hpref,
+                                                                                    weighted ? tv : nullptr, tileE, tileQ);
+            CU_LAUNCH(); ++launches;
+        }
+        CU(cudaStreamSynchronize(st));   // h_tileE / h_tileQ staging copies are done
     }
     tm.mark();
 
