@@ -19,10 +19,10 @@
 
 namespace ufb {
 
-constexpr int MID_THREADS = 512;
-constexpr int MID_PITCH = TILE + 1;                 // accumulator row pitch: bank = (a + b) mod 32 for both lane orders
+constexpr int MID_THREADS = 384;
+constexpr int MID_MINB = 3;                         // CTAs per SM (3 x 66 KB of accumulators)
+constexpr int MID_PITCH = TILE + 1;                 // accumulator row pitch: bank = (a + b) mod 32
 constexpr size_t MID_SMEM = (size_t)TILE * MID_PITCH * sizeof(uint32_t);
-constexpr int MID_SMALL = 4;
 
 // mid rows ordered by n_v (counting sort: histogram, scan, scatter) so that the rows a warp handles together
 // have similar list lengths; mbase[r] = list offset of row r.  The order inside a bucket is arbitrary --
@@ -33,13 +33,15 @@ __global__ void k_mid_hist(int n, const uint8_t* __restrict__ cls, const uint32_
     if (v < n && cls[v] == CLS_MID) atomicAdd(&hist[nv[v]], 1u);
 }
 __global__ void k_mid_rows(int n, const uint8_t* __restrict__ cls, const uint32_t* __restrict__ nv, uint32_t* __restrict__ cursor,
-                           const uint32_t* __restrict__ tptr, int32_t* __restrict__ mrows, uint32_t* __restrict__ mbase)
+                           const uint32_t* __restrict__ tptr, int32_t* __restrict__ mrows, uint32_t* __restrict__ mbase,
+                           uint32_t* __restrict__ mlen)
 {
     int v = blockIdx.x * blockDim.x + threadIdx.x;
     if (v < n && cls[v] == CLS_MID) {
         uint32_t r = atomicAdd(&cursor[nv[v]], 1u);
         mrows[r] = v;
         mbase[r] = tptr[v];
+        mlen[r] = nv[v];
     }
 }
 
@@ -61,30 +63,79 @@ __global__ void k_mid_seg(uint32_t n_mid, const int32_t* __restrict__ mrows, con
     seg[(size_t)t * n_mid + r] = lo - lo0;
 }
 
+// off[t][r], r = 0..n_mid: offset (within tile t's packed entries) of row r's first entry in tile t;
+// off[t][n_mid] = ttot[t] = number of packed entries of tile t.  One CTA per tile (exclusive scan over rows).
+__global__ void __launch_bounds__(1024)
+k_mid_off(uint32_t n_mid, const uint32_t* __restrict__ seg, uint32_t* __restrict__ off, uint32_t* __restrict__ ttot)
+{
+    __shared__ uint32_t part[1024];
+    const uint32_t t = blockIdx.x;
+    const uint32_t* s0 = seg + (size_t)t * n_mid;
+    const uint32_t* s1 = s0 + n_mid;
+    uint32_t* o = off + (size_t)t * (n_mid + 1);
+    const int th = threadIdx.x;
+    const uint32_t chunk = (n_mid + 1023u) / 1024u;
+    uint32_t lo = th * chunk, hi = lo + chunk;
+    if (lo > n_mid) lo = n_mid;
+    if (hi > n_mid) hi = n_mid;
+    uint32_t s = 0;
+    for (uint32_t r = lo; r < hi; ++r) s += s1[r] - s0[r];
+    part[th] = s;
+    __syncthreads();
+    for (int k = 1; k < 1024; k <<= 1) {
+        uint32_t add = th >= k ? part[th - k] : 0;
+        __syncthreads();
+        part[th] += add;
+        __syncthreads();
+    }
+    uint32_t run = th ? part[th - 1] : 0;
+    for (uint32_t r = lo; r < hi; ++r) { o[r] = run; run += s1[r] - s0[r]; }
+    if (th == 1023) { o[n_mid] = part[1023]; ttot[t] = part[1023]; }
+}
+
+// packed tile-major entries: pk[tbase[t] + off[t][r] + k] = { r << 7 | (sample - 128 t),  round(u~ * 2^F) }
+// One warp per mid row.
+__global__ void __launch_bounds__(256)
+k_mid_pack(uint32_t n_mid, const uint32_t* __restrict__ mbase, const uint32_t* __restrict__ mlen,
+           const uint32_t* __restrict__ ts, const float* __restrict__ tv, const uint32_t* __restrict__ seg,
+           const uint32_t* __restrict__ off, const uint32_t* __restrict__ tbase, float qscale, uint2* __restrict__ pk)
+{
+    const uint32_t r = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (r >= n_mid) return;
+    const uint32_t base = mbase[r], m = mlen[r];
+    for (uint32_t k = lane; k < m; k += 32) {
+        const uint32_t s = ts[base + k];
+        const uint32_t t = s >> 7;
+        const uint32_t pos = tbase[t] + off[(size_t)t * (n_mid + 1) + r] + (k - seg[(size_t)t * n_mid + r]);
+        pk[pos] = make_uint2((r << 7) | (s & 127u), __float2uint_rn(tv[base + k] * qscale));
+    }
+}
+
 struct MidParams {
     const int2* pairs; uint32_t n_pairs;
     unsigned int* counter;        // dynamic tile-pair queue
     uint32_t n_mid;
-    const uint32_t* mbase;        // [n_mid] list offset of the row
-    const uint32_t* seg;          // [n_tiles+1][n_mid]
-    const uint32_t* ts;
-    const float* tv;
+    const uint32_t* off;          // [n_tiles][n_mid+1]
+    const uint32_t* tbase;        // [n_tiles+1]
+    const uint2* pk;              // packed entries, tile-major, rows ascending within a tile
     int n_samples;
     float* out;
-    float qscale;                 // 2^F
     double inv_qscale;            // 2^-F
 };
 
-__device__ __forceinline__ uint32_t mid_q(float v, float qscale) { return __float2uint_rn(v * qscale); }
-
-__global__ void __launch_bounds__(MID_THREADS)
+// The join: every entry (row r, sample a, q_a) of tile I meets the entries (r, b, q_b) of the same row in tile J.
+// One lane per I entry, looping over the row's J entries; chunks of 32 consecutive I entries per warp, software
+// pipelined (entry loads two chunks ahead, offset gathers one chunk ahead).
+__global__ void __launch_bounds__(MID_THREADS, MID_MINB)
 k_mid(const MidParams P)
 {
     extern __shared__ uint32_t macc[];              // [128][129]
     __shared__ int s_pair;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    constexpr int NWARP = MID_THREADS / 32;
     const long long N = P.n_samples;
-    const uint32_t n_chunks = (P.n_mid + 31) >> 5;
+    const size_t pitch = (size_t)P.n_mid + 1;
 
     for (;;) {
         if (threadIdx.x == 0) s_pair = (int)atomicAdd(P.counter, 1u);
@@ -94,76 +145,52 @@ k_mid(const MidParams P)
         if ((uint32_t)pi >= P.n_pairs) break;
         const int2 ij = P.pairs[pi];
         const bool diag = ij.x == ij.y;
-        const uint32_t* segI0 = P.seg + (size_t)ij.x * P.n_mid;
-        const uint32_t* segI1 = segI0 + P.n_mid;
-        const uint32_t* segJ0 = P.seg + (size_t)ij.y * P.n_mid;
-        const uint32_t* segJ1 = segJ0 + P.n_mid;
-        const uint32_t sI = (uint32_t)ij.x * TILE, sJ = (uint32_t)ij.y * TILE;
+        const uint32_t eI0 = P.tbase[ij.x], eI1 = P.tbase[ij.x + 1], eJ0 = P.tbase[ij.y];
+        const uint32_t* offJ = P.off + (size_t)ij.y * pitch;
+        const uint32_t nchunk = (eI1 - eI0 + 31u) >> 5;
 
-        const int grp = lane >> 3, gl = lane & 7, gbase = lane & ~7;
-        for (uint32_t ch = warp; ch < n_chunks; ch += MID_THREADS / 32) {
-            const uint32_t r = ch * 32 + lane;
-            uint32_t i0 = 0, i1 = 0, j0 = 0, j1 = 0, base = 0;
-            if (r < P.n_mid) {
-                i0 = segI0[r]; i1 = segI1[r];
-                if (diag) { j0 = i0; j1 = i1; } else { j0 = segJ0[r]; j1 = segJ1[r]; }
-                base = P.mbase[r];
+        // pipeline registers: stage A = entry of chunk c+2, stage B = entry + J range of chunk c+1, stage C = current
+        uint2 entA = make_uint2(0u, 0u), entB = make_uint2(0u, 0u), entC;
+        uint32_t jB0 = 0, jB1 = 0, jC0, jC1;
+        bool vA = false, vB = false;
+        auto load_ent = [&](uint32_t c, uint2& ent, bool& valid) {
+            const uint32_t e = eI0 + c * 32u + lane;
+            valid = c < nchunk && e < eI1;
+            if (valid) ent = __ldg(P.pk + e);
+        };
+        auto load_range = [&](uint32_t c, const uint2& ent, bool valid, uint32_t& j0, uint32_t& j1) {
+            j0 = j1 = 0;
+            if (valid) {
+                const uint32_t r = ent.x >> 7;
+                j1 = eJ0 + offJ[r + 1];
+                j0 = diag ? (eI0 + c * 32u + lane + 1u) : (eJ0 + offJ[r]);       // diag: only the row's later entries (a < b)
             }
-            const uint32_t nI = i1 - i0, nJ = j1 - j0;
-            const uint32_t work = diag ? (nI * (nI - (nI ? 1u : 0u))) / 2u : nI * nJ;
-            // ---- tiny cross products: one row per lane
-            if (work && work <= (uint32_t)MID_SMALL) {
-                for (uint32_t k = i0; k < i1; ++k) {
-                    const uint32_t a = P.ts[base + k] - sI;
-                    const uint32_t qa = mid_q(P.tv[base + k], P.qscale);
-                    for (uint32_t l = diag ? k + 1 : j0; l < j1; ++l) {
-                        const uint32_t b = P.ts[base + l] - sJ;
-                        const uint32_t qb = mid_q(P.tv[base + l], P.qscale);
-                        atomicAdd(&macc[a * MID_PITCH + b], qa < qb ? qa : qb);
-                    }
-                }
-            }
-            // ---- the rest: four rows at a time, one per 8-lane group (four rows' loads in flight per warp);
-            //      lanes of a group over the longer list, loop over the shorter one
-            uint32_t rem = __ballot_sync(0xffffffffu, work > (uint32_t)MID_SMALL);
-            while (rem) {
-                uint32_t m = rem;
-                for (int t = 0; t < grp; ++t) m &= m - 1;
-                const bool act = m != 0;
-                const int src = act ? __ffs(m) - 1 : 0;
+        };
+        uint32_t c = warp;
+        load_ent(c, entB, vB);
+        load_range(c, entB, vB, jB0, jB1);
+        load_ent(c + NWARP, entA, vA);
+        for (; c < nchunk; c += NWARP) {
+            entC = entB; jC0 = jB0; jC1 = jB1;
+            entB = entA; vB = vA;
+            load_range(c + NWARP, entB, vB, jB0, jB1);
+            load_ent(c + 2 * NWARP, entA, vA);
+            uint32_t* arow = macc + (entC.x & 127u) * MID_PITCH;
+            const uint32_t qa = entC.y;
+            uint32_t l = jC0;
+            while (__any_sync(0xffffffffu, l < jC1)) {
+                uint2 f[4];
 #pragma unroll
-                for (int t = 0; t < 4; ++t) rem &= rem - 1;
-                uint32_t bi0 = __shfl_sync(0xffffffffu, i0, src), bi1 = __shfl_sync(0xffffffffu, i1, src);
-                uint32_t bj0 = __shfl_sync(0xffffffffu, j0, src), bj1 = __shfl_sync(0xffffffffu, j1, src);
-                const uint32_t bb = __shfl_sync(0xffffffffu, base, src);
-                if (!act) { bi0 = bi1 = bj0 = bj1 = 0; }
-                const bool lanesJ = diag || (bj1 - bj0) >= (bi1 - bi0);
-                const uint32_t p0 = lanesJ ? bj0 : bi0, p1 = lanesJ ? bj1 : bi1;   // lane list
-                const uint32_t q0 = lanesJ ? bi0 : bj0, q1 = lanesJ ? bi1 : bj1;   // loop list
-                const uint32_t sP = lanesJ ? sJ : sI, sQ = lanesJ ? sI : sJ;
-                const uint32_t mulP = lanesJ ? 1u : (uint32_t)MID_PITCH, mulQ = lanesJ ? (uint32_t)MID_PITCH : 1u;
-                for (uint32_t l0 = p0; __any_sync(0xffffffffu, l0 < p1); l0 += 8) {
-                    const uint32_t l = l0 + gl;
-                    const bool lv = l < p1;
-                    const uint32_t offe = lv ? (P.ts[bb + l] - sP) * mulP : 0u;
-                    const uint32_t qe = lv ? mid_q(P.tv[bb + l], P.qscale) : 0u;
-                    const uint32_t kend = diag ? (l0 + 8 < q1 ? l0 + 8 : q1) : q1;     // diag: only k < l
-                    for (uint32_t kb = q0; __any_sync(0xffffffffu, kb < kend); kb += 8) {
-                        const uint32_t kk = kb + gl;
-                        uint32_t offf = 0, qf = 0;
-                        if (kk < kend) { offf = (P.ts[bb + kk] - sQ) * mulQ; qf = mid_q(P.tv[bb + kk], P.qscale); }
+                for (int u = 0; u < 4; ++u) { f[u] = make_uint2(0u, 0u); if (l + u < jC1) f[u] = __ldg(P.pk + l + u); }
 #pragma unroll
-                        for (int t = 0; t < 8; ++t) {
-                            const uint32_t of = __shfl_sync(0xffffffffu, offf, gbase + t);
-                            const uint32_t qv = __shfl_sync(0xffffffffu, qf, gbase + t);
-                            if (lv && kb + t < kend && (!diag || kb + t < l)) atomicAdd(&macc[offe + of], qe < qv ? qe : qv);
-                        }
-                    }
-                }
+                for (int u = 0; u < 4; ++u)
+                    if (l + u < jC1) atomicAdd(arow + (f[u].x & 127u), qa < f[u].y ? qa : f[u].y);
+                l += 4;
             }
         }
         __syncthreads();
         // ---- epilogue: add the tile pair's fixed-point sums to the condensed matrix (exclusive owner)
+        const uint32_t sI = (uint32_t)ij.x * TILE, sJ = (uint32_t)ij.y * TILE;
         for (int e = threadIdx.x; e < TILE * TILE; e += MID_THREADS) {
             const int a = e >> 7, b = e & 127;
             const uint32_t q = macc[a * MID_PITCH + b];

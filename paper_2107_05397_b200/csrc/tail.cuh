@@ -94,13 +94,13 @@ __global__ void k_mark_class(int n, const uint8_t* __restrict__ cls, uint8_t whi
 //   c2_mid <= C(n_v,2) < c2_head   -> mid   (pair contributions accumulated per 128 x 128 tile pair in shared memory, mid.cuh)
 //   C(n_v,2) < c2_mid              -> tail  (pair contributions scattered with global RED.ADD, k_tail_scatter)
 // mid and tail branches share one list format; tcnt[v] = n_v for both (0 for head rows), scanned into the
-// list offsets.  counters[0..5] = head rows, tail rows, tail pair updates, list entries (all rows that keep a list), mid rows, mid pair updates.
+// list offsets.  counters[0..5] = head rows, tail rows, tail pair updates, list entries (all rows that keep a list), mid rows, mid pair updates; counters[9] = entries of the mid rows.
 __global__ void k_classify(int n, const uint32_t* __restrict__ nv, const uint32_t* __restrict__ ne, int all_rows,
                            double c2_head, double c2_mid, uint32_t force,
                            uint8_t* __restrict__ cls, uint32_t* __restrict__ tcnt, unsigned long long* __restrict__ counters)
 {
     int v = blockIdx.x * blockDim.x + threadIdx.x;
-    unsigned long long h = 0, t = 0, tu = 0, te = 0, m = 0, mu = 0;
+    unsigned long long h = 0, t = 0, tu = 0, te = 0, m = 0, mu = 0, me = 0;
     if (v < n) {
         unsigned long long k = nv[v];
         uint8_t c = CLS_NONE;
@@ -108,7 +108,7 @@ __global__ void k_classify(int n, const uint32_t* __restrict__ nv, const uint32_
             double c2 = 0.5 * (double)k * (double)(k - 1);
             c = force == 2 ? CLS_TAIL : force == 1 ? CLS_HEAD : c2 >= c2_head ? CLS_HEAD : c2 >= c2_mid ? CLS_MID : CLS_TAIL;
             if (c == CLS_TAIL) { t = 1; tu = k * (k - 1) / 2; }
-            else if (c == CLS_MID) { m = 1; mu = k * (k - 1) / 2; }
+            else if (c == CLS_MID) { m = 1; mu = k * (k - 1) / 2; me = k; }
             else h = 1;
         }
         cls[v] = c;
@@ -122,10 +122,11 @@ __global__ void k_classify(int n, const uint32_t* __restrict__ nv, const uint32_
         h += __shfl_xor_sync(0xffffffffu, h, o);  t += __shfl_xor_sync(0xffffffffu, t, o);
         tu += __shfl_xor_sync(0xffffffffu, tu, o); te += __shfl_xor_sync(0xffffffffu, te, o);
         m += __shfl_xor_sync(0xffffffffu, m, o);  mu += __shfl_xor_sync(0xffffffffu, mu, o);
+        me += __shfl_xor_sync(0xffffffffu, me, o);
     }
     if ((threadIdx.x & 31) == 0 && (h | t | m)) {
         atomicAdd(&counters[0], h); atomicAdd(&counters[1], t); atomicAdd(&counters[2], tu); atomicAdd(&counters[3], te);
-        atomicAdd(&counters[4], m); atomicAdd(&counters[5], mu);
+        atomicAdd(&counters[4], m); atomicAdd(&counters[5], mu); atomicAdd(&counters[9], me);
     }
 }
 

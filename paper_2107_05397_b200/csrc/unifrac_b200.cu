@@ -212,13 +212,18 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     const int n_tiles = cdiv(N, TILE);
     const double Pd = 0.5 * (double)N * (double)(N - 1), n_tp = 0.5 * (double)n_tiles * (n_tiles + 1);
     auto envd = [](const char* k, double d) { const char* e = getenv(k); return e ? atof(e) : d; };
-    const double R_tail = envd("UNIFRAC_B200_R_TAIL", 1.6e11), R_mid = envd("UNIFRAC_B200_R_MID", 6e11);
+    const double R_tail = envd("UNIFRAC_B200_R_TAIL", 1.6e11), R_mid = envd("UNIFRAC_B200_R_MID", 1.2e12);
     const double R_head = envd("UNIFRAC_B200_R_HEAD", 1.07e13), gram_Bps = envd("UNIFRAC_B200_GRAM_BPS", 6.0e12);
-    const double c_row = envd("UNIFRAC_B200_MID_ROW_S", 1e-10);          // seconds per (mid row, tile pair) visit
+    const double c_ent = envd("UNIFRAC_B200_MID_ENT_S", 3e-12);         // seconds per (mid entry, tile pair) visit of the join kernel
     const double head_s = gram ? n_tp * 512.0 / gram_Bps : Pd / R_head;  // seconds per head branch
     double c2_head, c2_mid;
-    if (mid_ok) { c2_head = head_s * R_mid; c2_mid = n_tp * c_row / (1.0 / R_tail - 1.0 / R_mid); if (c2_mid > c2_head) c2_mid = c2_head; }
-    else { c2_head = head_s * R_tail; c2_mid = INFINITY; }
+    if (mid_ok) {
+        // mid row: n_v entries, each visited once per tile J >= its own tile (~ n_tiles / 2 visits) + C(n_v,2) / R_mid;
+        // tail row: C(n_v,2) / R_tail  =>  mid wins for n_v > 1 + n_tiles * c_ent / (1/R_tail - 1/R_mid)
+        const double nstar = 1.0 + (double)n_tiles * c_ent / (1.0 / R_tail - 1.0 / R_mid);
+        c2_head = head_s * R_mid; c2_mid = 0.5 * nstar * (nstar - 1.0);
+        if (c2_mid > c2_head) c2_mid = c2_head;
+    } else { c2_head = head_s * R_tail; c2_mid = INFINITY; }
     uint32_t force = 0;
     if (flags & (UNIFRAC_FLAG_NO_TAIL | UNIFRAC_FLAG_ABSDIFF | UNIFRAC_FLAG_LITERAL)) force = 1;   // NO_TAIL + Gram = dense GEMM over every branch
     else if (flags & UNIFRAC_FLAG_ALL_TAIL) force = 2;
@@ -232,11 +237,11 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         k_tip_mark<<<cdiv(n, TB), TB, 0, st>>>(n, child_count, ne, tipc, work + 16); CU_LAUNCH(); ++launches;
         k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>(n, tipc, cptr); CU_LAUNCH(); ++launches;
     }
-    unsigned long long h_work[17];
+    unsigned long long h_work[18];
     CU(cudaMemcpyAsync(h_work, work, sizeof(h_work), cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
     const unsigned long long head_rows = h_work[8], tail_rows = h_work[9], tail_updates = h_work[10], tail_entries = h_work[11];
-    const unsigned long long mid_rows = h_work[12], mid_updates = h_work[13], nnz_pos = h_work[16];
+    const unsigned long long mid_rows = h_work[12], mid_updates = h_work[13], nnz_pos = h_work[16], mid_entries = h_work[17];
     if (tail_entries >= (1ull << 32) || nnz_pos >= (1ull << 32)) throw StatusFail{UNIFRAC_ERR_UNSUPPORTED};
     uint32_t* ts = A.get_n<uint32_t>(tail_entries ? tail_entries : 1);
     T* tv = A.get_n<T>(tail_entries ? tail_entries : 1);
@@ -387,27 +392,36 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             uint32_t* mcur = A.get_n<uint32_t>((size_t)N + 2);
             int32_t* mrows = A.get_n<int32_t>(n_mid);
             uint32_t* mbase = A.get_n<uint32_t>(n_mid);
+            uint32_t* mlen = A.get_n<uint32_t>(n_mid);
             CU(cudaMemsetAsync(mhist, 0, sizeof(uint32_t) * ((size_t)N + 2), st));
             k_mid_hist<<<cdiv(n, TB), TB, 0, st>>>(n, cls, nv, mhist); CU_LAUNCH(); ++launches;
             k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>(N + 1, mhist, mcur); CU_LAUNCH(); ++launches;
-            k_mid_rows<<<cdiv(n, TB), TB, 0, st>>>(n, cls, nv, mcur, tptr, mrows, mbase); CU_LAUNCH(); ++launches;
+            k_mid_rows<<<cdiv(n, TB), TB, 0, st>>>(n, cls, nv, mcur, tptr, mrows, mbase, mlen); CU_LAUNCH(); ++launches;
             uint32_t* mseg = A.get_n<uint32_t>((size_t)(n_tiles + 1) * n_mid);
             k_mid_seg<<<cdiv((long long)(n_tiles + 1) * n_mid, TB), TB, 0, st>>>(n_mid, mrows, tptr, ts, n_tiles, mseg); CU_LAUNCH(); ++launches;
+            uint32_t* moff = A.get_n<uint32_t>((size_t)n_tiles * ((size_t)n_mid + 1));
+            uint32_t* ttot = A.get_n<uint32_t>(n_tiles);
+            uint32_t* tbase = A.get_n<uint32_t>((size_t)n_tiles + 1);
+            k_mid_off<<<n_tiles, 1024, 0, st>>>(n_mid, mseg, moff, ttot); CU_LAUNCH(); ++launches;
+            k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>(n_tiles, ttot, tbase); CU_LAUNCH(); ++launches;
             unsigned long long* smax = work + 15;
             k_max_positive<<<cdiv((long long)n_tiles * TILE, TB), TB, 0, st>>>(n_tiles * TILE, sums, smax); CU_LAUNCH(); ++launches;
             unsigned long long h_smax = 0;
             CU(cudaMemcpyAsync(&h_smax, smax, sizeof(h_smax), cudaMemcpyDeviceToHost, st));
-            std::vector<int2> h_mp = blocked_pairs(n_tiles, 12);
+            std::vector<int2> h_mp = blocked_pairs(n_tiles, 8);
             int2* mpairs = A.get_n<int2>(h_mp.size());
             CU(cudaMemcpyAsync(mpairs, h_mp.data(), sizeof(int2) * h_mp.size(), cudaMemcpyHostToDevice, st));
             CU(cudaStreamSynchronize(st));
             double sm; memcpy(&sm, &h_smax, sizeof(sm));
             int ex = 0; frexp(sm > 0 ? sm : 1.0, &ex);          // sm < 2^ex
             mid_F = 30 - ex;                                     // acc <= min(R_a, R_b) * 2^F < 2^30 (+ rounding slack)
+            uint2* pk = A.get_n<uint2>(mid_entries ? mid_entries : 1);
+            k_mid_pack<<<cdiv((long long)n_mid * 32, TB), TB, 0, st>>>(n_mid, mbase, mlen, ts, reinterpret_cast<const float*>(tv), mseg, moff, tbase,
+                                                                      ldexpf(1.0f, mid_F), pk); CU_LAUNCH(); ++launches;
             MidParams M{};
             M.pairs = mpairs; M.n_pairs = (uint32_t)h_mp.size(); M.counter = reinterpret_cast<unsigned int*>(work + 7);
-            M.n_mid = n_mid; M.mbase = mbase; M.seg = mseg; M.ts = ts; M.tv = reinterpret_cast<const float*>(tv);
-            M.n_samples = N; M.out = reinterpret_cast<float*>(out); M.qscale = ldexpf(1.0f, mid_F); M.inv_qscale = ldexp(1.0, -mid_F);
+            M.n_mid = n_mid; M.off = moff; M.tbase = tbase; M.pk = pk;
+            M.n_samples = N; M.out = reinterpret_cast<float*>(out); M.inv_qscale = ldexp(1.0, -mid_F);
             CU(cudaFuncSetAttribute(k_mid, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MID_SMEM));
             int occ = 0, dev2 = 0, n_sm2 = 0;
             CU(cudaGetDevice(&dev2));
