@@ -61,6 +61,8 @@ typedef enum {
 #define UNIFRAC_FLAG_ALL_TAIL        32u  /* debug: every branch goes through the sparse tail scatter       */
 #define UNIFRAC_FLAG_NO_MID         128u  /* fp32: no shared-memory fixed-point "mid" kernel; branches are split into
                                              head and tail only                                            */
+#define UNIFRAC_FLAG_SPARSE_STRIPE   256u  /* head branches on the sparse-aware compact-row stripe kernel (row flags, quarter masks)
+                                             instead of the dense min-GEMM kernel                          */
 #define UNIFRAC_FLAG_NO_TENSOR       64u  /* unweighted + fp32: head branches on the CUDA-core stripe kernel
                                              instead of the tensor-core Gram kernel                        */
 
@@ -148,13 +150,14 @@ typedef struct {
     uint32_t gram;               /* 1 if the head branches went through the tcgen05 int8 Gram kernel    */
     uint32_t gram_k;             /* K (head branches, padded to 64) of that GEMM                       */
     uint32_t gram_q;             /* fixed-point scale: L_v = round(len_v * 2^q)                        */
+    uint32_t dense;              /* 1 if the head branches went through the dense CUDA-core kernel (k_dense) */
     float ms_plan, ms_embed, ms_tail, ms_mid, ms_stripe, ms_total;
 } unifrac_stats_t;
 int unifrac_last_stats(unifrac_stats_t *out);
 
 const char *unifrac_status_string(int status);
 const char *unifrac_last_cuda_error(void);   /* text of the last CUDA error seen by this thread  */
-int unifrac_abi_version(void);               /* 2                                                */
+int unifrac_abi_version(void);               /* 3                                                */
 
 #ifdef __cplusplus
 }

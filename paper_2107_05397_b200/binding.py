@@ -17,7 +17,7 @@ from . import build as _build
 UNWEIGHTED, WEIGHTED_NORMALIZED = 0, 1
 FP32, FP64 = 0, 1
 FLAG_LITERAL, FLAG_TENSOR_GRAM, FLAG_SKIP_VALIDATION, FLAG_ABSDIFF = 1, 2, 4, 8
-FLAG_NO_TAIL, FLAG_ALL_TAIL, FLAG_NO_TENSOR, FLAG_NO_MID = 16, 32, 64, 128
+FLAG_NO_TAIL, FLAG_ALL_TAIL, FLAG_NO_TENSOR, FLAG_NO_MID, FLAG_SPARSE_STRIPE = 16, 32, 64, 128, 256
 
 OK = 0
 ERR_INVALID_ARG, ERR_INVALID_TREE, ERR_INVALID_TABLE, ERR_EMPTY_SAMPLE = -1, -2, -3, -4
@@ -39,7 +39,7 @@ class Stats(C.Structure):
                 ("rows_staged", C.c_uint64),
                 ("embed_rows", C.c_uint64), ("workspace_bytes", C.c_uint64), ("n_tile_pairs", C.c_uint32),
                 ("n_levels", C.c_uint32), ("stripe_launches", C.c_uint32), ("tail_launches", C.c_uint32),
-                ("kernel_launches", C.c_uint32), ("mid_launches", C.c_uint32), ("mid_F", C.c_uint32), ("gram", C.c_uint32), ("gram_k", C.c_uint32), ("gram_q", C.c_uint32),
+                ("kernel_launches", C.c_uint32), ("mid_launches", C.c_uint32), ("mid_F", C.c_uint32), ("gram", C.c_uint32), ("gram_k", C.c_uint32), ("gram_q", C.c_uint32), ("dense", C.c_uint32),
                 ("ms_plan", C.c_float), ("ms_embed", C.c_float), ("ms_tail", C.c_float), ("ms_mid", C.c_float), ("ms_stripe", C.c_float),
                 ("ms_total", C.c_float)]
 

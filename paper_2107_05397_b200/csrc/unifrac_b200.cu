@@ -9,6 +9,7 @@
 #include "stripe.cuh"
 #include "gram.cuh"
 #include "mid.cuh"
+#include "dense.cuh"
 
 #include <cstdio>
 #include <cstdlib>
@@ -66,7 +67,8 @@ inline int cdiv(long long a, long long b) { return (int)((a + b - 1) / b); }
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-CUtensorMap make_u8_rowmajor_map(void* base, uint64_t cols, uint64_t rows, uint32_t box_cols, uint32_t box_rows)
+CUtensorMap make_rowmajor_map(void* base, CUtensorMapDataType dt, size_t esz, uint64_t cols, uint64_t rows, uint32_t box_cols,
+                              uint32_t box_rows, CUtensorMapSwizzle swz)
 {
     static EncodeTiledFn fn = nullptr;
     if (!fn) {
@@ -78,13 +80,17 @@ CUtensorMap make_u8_rowmajor_map(void* base, uint64_t cols, uint64_t rows, uint3
     }
     CUtensorMap m;
     cuuint64_t dims[2] = {cols, rows};
-    cuuint64_t strides[1] = {cols};              // bytes, dimension 1
+    cuuint64_t strides[1] = {cols * esz};        // bytes, dimension 1
     cuuint32_t box[2] = {box_cols, box_rows};
     cuuint32_t estr[2] = {1, 1};
-    CUresult r = fn(&m, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                    CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    CUresult r = fn(&m, dt, 2, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, swz,
+                    CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) throw CudaFail{cudaErrorInvalidValue, "cuTensorMapEncodeTiled", __LINE__};
     return m;
+}
+CUtensorMap make_u8_rowmajor_map(void* base, uint64_t cols, uint64_t rows, uint32_t box_cols, uint32_t box_rows)
+{
+    return make_rowmajor_map(base, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, cols, rows, box_cols, box_rows, CU_TENSOR_MAP_SWIZZLE_128B);
 }
 
 // tile pairs (I <= J) in BLK x BLK blocks of tiles, so that CTAs working on consecutive pairs share operand tiles in L2
@@ -248,13 +254,15 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
 
     // ------------------------------------------------------------------ tensor-core Gram path: u8 operand matrices from the bits
     bool use_gram = gram && head_rows > 0 && head_rows < (1ull << 23);
+    // CUDA-core head path: dense min-GEMM kernel (dense.cuh) unless a debug form needs the sparse-aware compact-row kernel
+    const bool dense_head = !use_gram && !(flags & (UNIFRAC_FLAG_ABSDIFF | UNIFRAC_FLAG_LITERAL | UNIFRAC_FLAG_NO_TAIL | UNIFRAC_FLAG_SPARSE_STRIPE));
     double* uval = nullptr;
     uint8_t* XG[4] = {nullptr, nullptr, nullptr, nullptr};
     uint32_t K_pad = 0;
     int gram_q = 0;
     uint32_t* hrank = nullptr;                                 // head rank of every node (exclusive scan of the head marks)
     int32_t* hrows = nullptr;                                  // head rank -> node id
-    if (head_rows > 0 && (use_gram || weighted)) {
+    if (head_rows > 0 && (use_gram || weighted || dense_head)) {
         uint32_t* is_head = A.get_n<uint32_t>(n);
         hrank = A.get_n<uint32_t>((size_t)n + 1);
         k_mark_class<<<cdiv(n, TB), TB, 0, st>>>(n, cls, CLS_HEAD, is_head); CU_LAUNCH(); ++launches;
@@ -317,7 +325,29 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     uint32_t* rflags = nullptr; uint32_t* rrank = nullptr;
     T** tileE = nullptr; uint8_t** tileQ = nullptr;
     uint64_t embed_rows = 0;
-    if (!use_gram) {
+    T* Edense = nullptr;
+    const size_t Npad = (size_t)n_tiles * TILE;
+    uint32_t Kd_pad = 0;
+    if (dense_head) {
+        constexpr int BK = DenseCfg<T>::BK;
+        Kd_pad = (uint32_t)((head_rows + BK - 1) / BK * BK);
+        if (Kd_pad == 0) Kd_pad = BK;
+        Edense = A.get_n<T>((size_t)Kd_pad * Npad);
+        CU(cudaMemsetAsync(Edense + (size_t)head_rows * Npad, 0, sizeof(T) * (Kd_pad - (size_t)head_rows) * Npad, st));
+        if (head_rows > 0) {
+            hrows = A.get_n<int32_t>(head_rows);
+            k_head_rows<<<cdiv(n, TB), TB, 0, st>>>(n, cls, hrank, hrows); CU_LAUNCH(); ++launches;
+            uint32_t* hpref = nullptr;
+            if (weighted) {
+                hpref = A.get_n<uint32_t>((size_t)head_rows * n_tiles);
+                k_head_pref<<<cdiv((long long)head_rows * 32, TB), TB, 0, st>>>((uint32_t)head_rows, hrows, bits, NW, n_tiles, hpref); CU_LAUNCH(); ++launches;
+            }
+            k_head_dense<T><<<cdiv((long long)head_rows * n_tiles * 32, TB), TB, 0, st>>>((uint32_t)head_rows, hrows, len, bits, NW, n_tiles, tptr, hpref,
+                                                                                         weighted ? tv : nullptr, Edense, Npad);
+            CU_LAUNCH(); ++launches;
+            embed_rows = head_rows * (uint64_t)n_tiles;
+        }
+    } else if (!use_gram) {
         rflags = A.get_n<uint32_t>((size_t)n_tiles * nwords);
         rrank = A.get_n<uint32_t>((size_t)n_tiles * nwords);
         uint32_t* rows = A.get_n<uint32_t>(n_tiles);
@@ -460,6 +490,23 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             k_gram<<<grid, GRAM_THREADS, GRAM_SMEM, st>>>(tmA, tmB0, tmB1, tmB2, G); CU_LAUNCH(); ++launches; ++stripe_launches;
             CU(cudaStreamSynchronize(st));       // h_pairs staging copy done before it goes out of scope
         }
+    } else if (dense_head) {
+        std::vector<int2> h_pairs = blocked_pairs(n_tiles, 12);
+        n_pairs = (uint32_t)h_pairs.size();
+        int2* pairs = A.get_n<int2>(n_pairs);
+        CU(cudaMemcpyAsync(pairs, h_pairs.data(), sizeof(int2) * n_pairs, cudaMemcpyHostToDevice, st));
+        constexpr bool f32 = std::is_same<T, float>::value;
+        CUtensorMap tmE = make_rowmajor_map(Edense, f32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, sizeof(T), Npad, Kd_pad,
+                                            TILE, DenseCfg<T>::BK, CU_TENSOR_MAP_SWIZZLE_NONE);
+        DenseParams D{};
+        D.pairs = pairs; D.n_pairs = n_pairs; D.K_pad = Kd_pad; D.sums = sums; D.n_samples = N; D.weighted = weighted; D.out = out;
+        D.add_out = (tail_rows || mid_rows) ? 1 : 0;
+        const size_t smem = dense_smem_bytes<T>();
+        CU(cudaFuncSetAttribute(k_dense<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        unsigned grid = (unsigned)std::min<long long>(n_sm, n_pairs);
+        D.scratch = A.get_n<double>((size_t)grid * 64 * 256);
+        k_dense<T><<<grid, DENSE_THREADS, smem, st>>>(tmE, D); CU_LAUNCH(); ++launches; ++stripe_launches;
+        CU(cudaStreamSynchronize(st));           // h_pairs staging copy done before it goes out of scope
     } else {
     std::vector<int2> h_pairs;
     h_pairs.reserve((size_t)n_tiles * (n_tiles + 1) / 2);
@@ -511,7 +558,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     g_stats.head_rows = head_rows; g_stats.tail_rows = tail_rows; g_stats.tail_updates = tail_updates; g_stats.tail_entries = tail_entries;
     g_stats.tail_launches = tail_launches;
     g_stats.mid_rows = mid_rows; g_stats.mid_updates = mid_updates; g_stats.mid_launches = mid_launches; g_stats.mid_F = (uint32_t)mid_F;
-    g_stats.gram = use_gram ? 1u : 0u; g_stats.gram_k = K_pad; g_stats.gram_q = (uint32_t)gram_q;
+    g_stats.gram = use_gram ? 1u : 0u; g_stats.dense = dense_head ? 1u : 0u; g_stats.gram_k = K_pad; g_stats.gram_q = (uint32_t)gram_q;
     g_stats.n_tile_pairs = n_pairs;
     g_stats.n_levels = (uint32_t)n_levels;
     g_stats.stripe_launches = stripe_launches;
@@ -534,7 +581,7 @@ int guarded(int32_t n_nodes, const int32_t* parent, const double* len, const int
     if (variant != UNIFRAC_UNWEIGHTED && variant != UNIFRAC_WEIGHTED_NORMALIZED) return UNIFRAC_ERR_INVALID_ARG;
     if (precision != UNIFRAC_FP32 && precision != UNIFRAC_FP64) return UNIFRAC_ERR_INVALID_ARG;
     if (flags & ~(UNIFRAC_FLAG_LITERAL | UNIFRAC_FLAG_TENSOR_GRAM | UNIFRAC_FLAG_SKIP_VALIDATION | UNIFRAC_FLAG_ABSDIFF |
-                  UNIFRAC_FLAG_NO_TAIL | UNIFRAC_FLAG_ALL_TAIL | UNIFRAC_FLAG_NO_TENSOR | UNIFRAC_FLAG_NO_MID))
+                  UNIFRAC_FLAG_NO_TAIL | UNIFRAC_FLAG_ALL_TAIL | UNIFRAC_FLAG_NO_TENSOR | UNIFRAC_FLAG_NO_MID | UNIFRAC_FLAG_SPARSE_STRIPE))
         return UNIFRAC_ERR_INVALID_ARG;
     if ((long long)N > (1ll << 23)) return UNIFRAC_ERR_UNSUPPORTED;
     Arena A{alloc, user, st};
@@ -616,7 +663,7 @@ int unifrac_last_stats(unifrac_stats_t* out)
     if (g_stats_pending) {
         if (cudaEventSynchronize(g_stats_event) != cudaSuccess) { cudaGetLastError(); return UNIFRAC_ERR_CUDA; }
         g_stats.updates_executed_head = g_stats_pinned[0] * 2048ull;    // one (warp,row) = 32 x 64 pair updates
-        if (g_stats.gram) g_stats.updates_executed_head = g_stats.head_rows * ((uint64_t)g_stats.updates_dense / (g_stats.branches_embedded ? g_stats.branches_embedded : 1));
+        if (g_stats.gram || g_stats.dense) g_stats.updates_executed_head = g_stats.head_rows * ((uint64_t)g_stats.updates_dense / (g_stats.branches_embedded ? g_stats.branches_embedded : 1));
         g_stats.updates_executed = g_stats.updates_executed_head + g_stats.tail_updates + g_stats.mid_updates;
         g_stats.rows_staged = g_stats_pinned[1];
         g_stats_pending = false;
@@ -641,6 +688,6 @@ const char* unifrac_status_string(int status)
 }
 
 const char* unifrac_last_cuda_error(void) { return g_cuda_err.c_str(); }
-int unifrac_abi_version(void) { return 2; }
+int unifrac_abi_version(void) { return 3; }
 
 }  // extern "C"

@@ -27,7 +27,7 @@ def test_header_symbols_are_exported_and_bound():
 
 
 def test_version_and_status_strings_without_gpu():
-    assert binding.unifrac_abi_version() == 2
+    assert binding.unifrac_abi_version() == 3
     assert binding.unifrac_status_string(0) == "ok"
     assert "tree" in binding.unifrac_status_string(binding.ERR_INVALID_TREE)
 
