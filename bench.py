@@ -32,6 +32,7 @@ METRIC = "unifrac_dense_equivalent_pair_branch_updates_per_s"
 UNIT = "updates/s"
 SM_COUNT, FP32_LANES, SM_MAX_GHZ = 148, 128, 1.965        # B200_PROFILING.md / MEASURED_PEAKS.json
 ALU_PEAK_TFLOPS = SM_COUNT * FP32_LANES * SM_MAX_GHZ / 1e3    # FADD/FMNMX-class lane-ops (not FMA-doubled)
+MID_ATOMS_PER_CLK_SM = 32.0     # one conflict-free shared-memory wavefront (32 banks) per clock per SM
 
 WORKLOADS = {   # name -> (variants, precision)    BASELINE.json:7-11
     "tiny": ((0, 1), 1), "small": ((0, 1), 1), "medium": ((0,), 0), "emp": ((0, 1), 0), "large": ((0, 1), 0),
@@ -238,15 +239,16 @@ def main():
     src = "measured" if peaks else "fallback"
     step_s = ms * 1e-3
     rl = []
-    # (1) k_stripe: CUDA-core register-tile kernel (head branches; weighted, fp64, or NO_TENSOR)
+    # (1) k_dense (default) / k_stripe (debug forms): CUDA-core register-tile kernel (head branches; weighted, fp64, or NO_TENSOR)
     ss = [s for s in flat if not s["gram"]]
     if ss:
+        kname = "k_dense" if all(s["dense"] for s in ss) else "k_stripe"
         t = sum(s["ms_stripe"] for s in ss) * 1e-3
         w_exec = sum(s["updates_executed_head"] for s in ss)
         nl = sum(s["stripe_launches"] for s in ss)
         ach = 2.0 * w_exec / t / 1e12 if t > 0 else 0.0
         rl.append(dict(bound="alu", achieved=ach, peak=ALU_PEAK_TFLOPS, unit="TFLOP/s", frac=ach / ALU_PEAK_TFLOPS, traffic=None,
-                       kernel="k_stripe", launches=nl, ms_per_launch=1e3 * t / max(1, nl),
+                       kernel=kname, launches=nl, ms_per_launch=1e3 * t / max(1, nl),
                        executed_updates_per_launch=w_exec / max(1, nl), seconds=t, share_of_step=t / step_s,
                        peak_source=f"{SM_COUNT} SMs x {FP32_LANES} FP32 lanes x {SM_MAX_GHZ} GHz (sm_max_mhz of MEASURED_PEAKS.json, {src}); "
                                    "2 FP32-pipe lane-ops (FMNMX+FADD) per (pair, branch) update"))
@@ -275,6 +277,17 @@ def main():
                        frac=reds / t / RED_PEAK if t > 0 else 0.0, traffic=None, kernel="k_tail_scatter", launches=nl,
                        ms_per_launch=1e3 * t / max(1, nl), seconds=t, share_of_step=t / step_s,
                        peak_source="micro-benchmark of scattered RED.ADD.F32 into an L2-resident footprint, same GPU pool"))
+    # (4) k_mid: tile-pair join with native shared-memory integer atomics (ATOMS.ADD), one per (pair, branch) update
+    t = sum(s["ms_mid"] for s in flat) * 1e-3
+    mu = sum(s["mid_updates"] for s in flat)
+    nl = sum(s["mid_launches"] for s in flat)
+    if nl:
+        ATOMS_PEAK = MID_ATOMS_PER_CLK_SM * SM_COUNT * SM_MAX_GHZ * 1e9
+        rl.append(dict(bound="smem_atomic", achieved=mu / t / 1e9 if t > 0 else 0.0, peak=ATOMS_PEAK / 1e9, unit="GATOM/s",
+                       frac=mu / t / ATOMS_PEAK if t > 0 else 0.0, traffic=None, kernel="k_mid", launches=nl,
+                       ms_per_launch=1e3 * t / max(1, nl), seconds=t, share_of_step=t / step_s,
+                       note="ms_mid also covers the mid list preparation kernels (k_mid_seg/off/pack)",
+                       peak_source=f"{MID_ATOMS_PER_CLK_SM} ATOMS.ADD lane-ops/clk/SM x {SM_COUNT} SMs x {SM_MAX_GHZ} GHz (DESIGN.md 'k_mid')"))
     rl.sort(key=lambda r: -r["seconds"])
     roofline = dict(rl[0])
     roofline["others"] = rl[1:]

@@ -16,13 +16,15 @@
 #pragma once
 #include "common.cuh"
 #include "tail.cuh"
+#include "stripe.cuh"   // smem_u32
 
 namespace ufb {
 
 constexpr int MID_THREADS = 384;
 constexpr int MID_MINB = 3;                         // CTAs per SM (3 x 66 KB of accumulators)
-constexpr int MID_PITCH = TILE + 1;                 // accumulator row pitch: bank = (a + b) mod 32
-constexpr size_t MID_SMEM = (size_t)TILE * MID_PITCH * sizeof(uint32_t);
+// accumulator cell (a, b) lives at word a * 128 + (b ^ (a & 31)): bank = (a ^ b) mod 32, and the byte address is
+// one LOP3 away from the packed entry word:  (row_base(a) | (a & 31) << 2) ^ (b << 2)
+constexpr size_t MID_SMEM = (size_t)TILE * TILE * sizeof(uint32_t) + 512 /*alignment*/;
 
 // mid rows ordered by n_v (counting sort: histogram, scan, scatter) so that the rows a warp handles together
 // have similar list lengths; mbase[r] = list offset of row r.  The order inside a bucket is arbitrary --
@@ -93,7 +95,7 @@ k_mid_off(uint32_t n_mid, const uint32_t* __restrict__ seg, uint32_t* __restrict
     if (th == 1023) { o[n_mid] = part[1023]; ttot[t] = part[1023]; }
 }
 
-// packed tile-major entries: pk[tbase[t] + off[t][r] + k] = { r << 7 | (sample - 128 t),  round(u~ * 2^F) }
+// packed tile-major entries: pk[tbase[t] + off[t][r] + k] = { r << 9 | (sample - 128 t) << 2,  round(u~ * 2^F) }
 // One warp per mid row.
 __global__ void __launch_bounds__(256)
 k_mid_pack(uint32_t n_mid, const uint32_t* __restrict__ mbase, const uint32_t* __restrict__ mlen,
@@ -108,7 +110,7 @@ k_mid_pack(uint32_t n_mid, const uint32_t* __restrict__ mbase, const uint32_t* _
         const uint32_t s = ts[base + k];
         const uint32_t t = s >> 7;
         const uint32_t pos = tbase[t] + off[(size_t)t * (n_mid + 1) + r] + (k - seg[(size_t)t * n_mid + r]);
-        pk[pos] = make_uint2((r << 7) | (s & 127u), __float2uint_rn(tv[base + k] * qscale));
+        pk[pos] = make_uint2((r << 9) | ((s & 127u) << 2), __float2uint_rn(tv[base + k] * qscale));
     }
 }
 
@@ -127,19 +129,29 @@ struct MidParams {
 // The join: every entry (row r, sample a, q_a) of tile I meets the entries (r, b, q_b) of the same row in tile J.
 // One lane per I entry, looping over the row's J entries; chunks of 32 consecutive I entries per warp, software
 // pipelined (entry loads two chunks ahead, offset gathers one chunk ahead).
+// predicated shared-memory integer add (no branch around the ATOMS): executes iff idx < end
+__device__ __forceinline__ void mid_red_if(uint32_t addr, uint32_t v, uint32_t idx, uint32_t end) {
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.lt.u32 p, %2, %3;\n\t@p red.shared.add.u32 [%0], %1;\n\t}"
+                 ::"r"(addr), "r"(v), "r"(idx), "r"(end) : "memory");
+}
+
 __global__ void __launch_bounds__(MID_THREADS, MID_MINB)
 k_mid(const MidParams P)
 {
-    extern __shared__ uint32_t macc[];              // [128][129]
+    extern __shared__ uint32_t macc_raw[];
     __shared__ int s_pair;
+    const uint32_t raw_s = smem_u32(macc_raw);
+    const uint32_t macc_s = (raw_s + 511u) & ~511u;                    // 512-byte aligned rows: row a at macc_s + 512 a
+    uint32_t* macc = macc_raw + ((macc_s - raw_s) >> 2);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     constexpr int NWARP = MID_THREADS / 32;
     const long long N = P.n_samples;
     const size_t pitch = (size_t)P.n_mid + 1;
+    const uint2* __restrict__ pk = P.pk;
 
     for (;;) {
         if (threadIdx.x == 0) s_pair = (int)atomicAdd(P.counter, 1u);
-        for (int i = threadIdx.x; i < TILE * MID_PITCH; i += MID_THREADS) macc[i] = 0u;
+        for (int i = threadIdx.x; i < TILE * TILE; i += MID_THREADS) macc[i] = 0u;
         __syncthreads();
         const int pi = s_pair;
         if ((uint32_t)pi >= P.n_pairs) break;
@@ -156,12 +168,12 @@ k_mid(const MidParams P)
         auto load_ent = [&](uint32_t c, uint2& ent, bool& valid) {
             const uint32_t e = eI0 + c * 32u + lane;
             valid = c < nchunk && e < eI1;
-            if (valid) ent = __ldg(P.pk + e);
+            if (valid) ent = __ldg(pk + e);
         };
         auto load_range = [&](uint32_t c, const uint2& ent, bool valid, uint32_t& j0, uint32_t& j1) {
             j0 = j1 = 0;
             if (valid) {
-                const uint32_t r = ent.x >> 7;
+                const uint32_t r = ent.x >> 9;
                 j1 = eJ0 + offJ[r + 1];
                 j0 = diag ? (eI0 + c * 32u + lane + 1u) : (eJ0 + offJ[r]);       // diag: only the row's later entries (a < b)
             }
@@ -175,16 +187,17 @@ k_mid(const MidParams P)
             entB = entA; vB = vA;
             load_range(c + NWARP, entB, vB, jB0, jB1);
             load_ent(c + 2 * NWARP, entA, vA);
-            uint32_t* arow = macc + (entC.x & 127u) * MID_PITCH;
+            const uint32_t a4 = entC.x & 0x1fcu;                                  // 4 a
+            const uint32_t arow = (macc_s + (a4 << 7)) | (a4 & 0x7cu);            // row base | (a & 31) << 2
             const uint32_t qa = entC.y;
             uint32_t l = jC0;
             while (__any_sync(0xffffffffu, l < jC1)) {
                 uint2 f[4];
 #pragma unroll
-                for (int u = 0; u < 4; ++u) { f[u] = make_uint2(0u, 0u); if (l + u < jC1) f[u] = __ldg(P.pk + l + u); }
+                for (int u = 0; u < 4; ++u) if (l + u < jC1) f[u] = __ldg(pk + l + u);
 #pragma unroll
                 for (int u = 0; u < 4; ++u)
-                    if (l + u < jC1) atomicAdd(arow + (f[u].x & 127u), qa < f[u].y ? qa : f[u].y);
+                    mid_red_if(arow ^ (f[u].x & 0x1fcu), min(qa, f[u].y), l + u, jC1);
                 l += 4;
             }
         }
@@ -192,8 +205,8 @@ k_mid(const MidParams P)
         // ---- epilogue: add the tile pair's fixed-point sums to the condensed matrix (exclusive owner)
         const uint32_t sI = (uint32_t)ij.x * TILE, sJ = (uint32_t)ij.y * TILE;
         for (int e = threadIdx.x; e < TILE * TILE; e += MID_THREADS) {
-            const int a = e >> 7, b = e & 127;
-            const uint32_t q = macc[a * MID_PITCH + b];
+            const int a = e >> 7, b = (e & 127) ^ (a & 31);
+            const uint32_t q = macc[e];
             if (q) {
                 const long long gi = (long long)sI + a, gj = (long long)sJ + b;
                 if (gi < gj && gj < N) {

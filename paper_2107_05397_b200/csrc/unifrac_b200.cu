@@ -417,6 +417,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     int mid_F = 0;
     if (mid_rows) {
         if constexpr (std::is_same<T, float>::value) {
+            if (mid_rows >= (1ull << 23)) throw StatusFail{UNIFRAC_ERR_UNSUPPORTED};     // packed entries keep the row in 23 bits
             const uint32_t n_mid = (uint32_t)mid_rows;
             uint32_t* mhist = A.get_n<uint32_t>((size_t)N + 2);
             uint32_t* mcur = A.get_n<uint32_t>((size_t)N + 2);
