@@ -81,7 +81,7 @@ k_mid_off(uint32_t n_mid, const uint32_t* __restrict__ seg, uint32_t* __restrict
     if (lo > n_mid) lo = n_mid;
     if (hi > n_mid) hi = n_mid;
     uint32_t s = 0;
-    for (uint32_t r = lo; r < hi; ++r) s += s1[r] - s0[r];
+    for (uint32_t r = lo; r < hi; ++r) s += (s1[r] - s0[r] + 1u) & ~1u;      // every (row, tile) list padded to an even length
     part[th] = s;
     __syncthreads();
     for (int k = 1; k < 1024; k <<= 1) {
@@ -91,7 +91,7 @@ k_mid_off(uint32_t n_mid, const uint32_t* __restrict__ seg, uint32_t* __restrict
         __syncthreads();
     }
     uint32_t run = th ? part[th - 1] : 0;
-    for (uint32_t r = lo; r < hi; ++r) { o[r] = run; run += s1[r] - s0[r]; }
+    for (uint32_t r = lo; r < hi; ++r) { o[r] = run; run += (s1[r] - s0[r] + 1u) & ~1u; }
     if (th == 1023) { o[n_mid] = part[1023]; ttot[t] = part[1023]; }
 }
 
@@ -109,8 +109,11 @@ k_mid_pack(uint32_t n_mid, const uint32_t* __restrict__ mbase, const uint32_t* _
     for (uint32_t k = lane; k < m; k += 32) {
         const uint32_t s = ts[base + k];
         const uint32_t t = s >> 7;
-        const uint32_t pos = tbase[t] + off[(size_t)t * (n_mid + 1) + r] + (k - seg[(size_t)t * n_mid + r]);
-        pk[pos] = make_uint2((r << 9) | ((s & 127u) << 2), __float2uint_rn(tv[base + k] * qscale));
+        const uint32_t g0 = seg[(size_t)t * n_mid + r], g1 = seg[(size_t)(t + 1) * n_mid + r];
+        const uint32_t pos = tbase[t] + off[(size_t)t * (n_mid + 1) + r] + (k - g0);
+        const uint32_t x = (r << 9) | ((s & 127u) << 2);
+        pk[pos] = make_uint2(x, __float2uint_rn(tv[base + k] * qscale));
+        if (k + 1 == g1 && ((g1 - g0) & 1u)) pk[pos + 1] = make_uint2(x, 0u);    // padding entry: adds 0 to a valid cell
     }
 }
 
@@ -129,10 +132,8 @@ struct MidParams {
 // The join: every entry (row r, sample a, q_a) of tile I meets the entries (r, b, q_b) of the same row in tile J.
 // One lane per I entry, looping over the row's J entries; chunks of 32 consecutive I entries per warp, software
 // pipelined (entry loads two chunks ahead, offset gathers one chunk ahead).
-// predicated shared-memory integer add (no branch around the ATOMS): executes iff idx < end
-__device__ __forceinline__ void mid_red_if(uint32_t addr, uint32_t v, uint32_t idx, uint32_t end) {
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.lt.u32 p, %2, %3;\n\t@p red.shared.add.u32 [%0], %1;\n\t}"
-                 ::"r"(addr), "r"(v), "r"(idx), "r"(end) : "memory");
+__device__ __forceinline__ void mid_red(uint32_t addr, uint32_t v) {
+    asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
 }
 
 __global__ void __launch_bounds__(MID_THREADS, MID_MINB)
@@ -156,7 +157,6 @@ k_mid(const MidParams P)
         const int pi = s_pair;
         if ((uint32_t)pi >= P.n_pairs) break;
         const int2 ij = P.pairs[pi];
-        const bool diag = ij.x == ij.y;
         const uint32_t eI0 = P.tbase[ij.x], eI1 = P.tbase[ij.x + 1], eJ0 = P.tbase[ij.y];
         const uint32_t* offJ = P.off + (size_t)ij.y * pitch;
         const uint32_t nchunk = (eI1 - eI0 + 31u) >> 5;
@@ -170,34 +170,36 @@ k_mid(const MidParams P)
             valid = c < nchunk && e < eI1;
             if (valid) ent = __ldg(pk + e);
         };
-        auto load_range = [&](uint32_t c, const uint2& ent, bool valid, uint32_t& j0, uint32_t& j1) {
+        auto load_range = [&](const uint2& ent, bool valid, uint32_t& j0, uint32_t& j1) {
             j0 = j1 = 0;
-            if (valid) {
+            if (valid && ent.y != 0u) {                      // q = 0 (padding entries) contributes nothing
                 const uint32_t r = ent.x >> 9;
+                j0 = eJ0 + offJ[r];                          // both even: 16-byte aligned pairs of entries
                 j1 = eJ0 + offJ[r + 1];
-                j0 = diag ? (eI0 + c * 32u + lane + 1u) : (eJ0 + offJ[r]);       // diag: only the row's later entries (a < b)
             }
         };
+        // The diagonal tile pair (I == J) walks the row's full list as well: cells with a >= b receive sums that the
+        // epilogue never reads (it keeps gi < gj only).
         uint32_t c = warp;
         load_ent(c, entB, vB);
-        load_range(c, entB, vB, jB0, jB1);
+        load_range(entB, vB, jB0, jB1);
         load_ent(c + NWARP, entA, vA);
         for (; c < nchunk; c += NWARP) {
             entC = entB; jC0 = jB0; jC1 = jB1;
             entB = entA; vB = vA;
-            load_range(c + NWARP, entB, vB, jB0, jB1);
+            load_range(entB, vB, jB0, jB1);
             load_ent(c + 2 * NWARP, entA, vA);
             const uint32_t a4 = entC.x & 0x1fcu;                                  // 4 a
             const uint32_t arow = (macc_s + (a4 << 7)) | (a4 & 0x7cu);            // row base | (a & 31) << 2
             const uint32_t qa = entC.y;
             uint32_t l = jC0;
             while (__any_sync(0xffffffffu, l < jC1)) {
-                uint2 f[4];
-#pragma unroll
-                for (int u = 0; u < 4; ++u) if (l + u < jC1) f[u] = __ldg(pk + l + u);
-#pragma unroll
-                for (int u = 0; u < 4; ++u)
-                    mid_red_if(arow ^ (f[u].x & 0x1fcu), min(qa, f[u].y), l + u, jC1);
+                uint4 f0, f1;
+                const bool p0 = l < jC1, p1 = l + 2u < jC1;
+                if (p0) f0 = __ldg(reinterpret_cast<const uint4*>(pk + l));
+                if (p1) f1 = __ldg(reinterpret_cast<const uint4*>(pk + l + 2));
+                if (p0) { mid_red(arow ^ (f0.x & 0x1fcu), min(qa, f0.y)); mid_red(arow ^ (f0.z & 0x1fcu), min(qa, f0.w)); }
+                if (p1) { mid_red(arow ^ (f1.x & 0x1fcu), min(qa, f1.y)); mid_red(arow ^ (f1.z & 0x1fcu), min(qa, f1.w)); }
                 l += 4;
             }
         }

@@ -439,6 +439,8 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             k_max_positive<<<cdiv((long long)n_tiles * TILE, TB), TB, 0, st>>>(n_tiles * TILE, sums, smax); CU_LAUNCH(); ++launches;
             unsigned long long h_smax = 0;
             CU(cudaMemcpyAsync(&h_smax, smax, sizeof(h_smax), cudaMemcpyDeviceToHost, st));
+            uint32_t h_pk_total = 0;                            // packed entries incl. the even-length padding
+            CU(cudaMemcpyAsync(&h_pk_total, tbase + n_tiles, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
             std::vector<int2> h_mp = blocked_pairs(n_tiles, 8);
             int2* mpairs = A.get_n<int2>(h_mp.size());
             CU(cudaMemcpyAsync(mpairs, h_mp.data(), sizeof(int2) * h_mp.size(), cudaMemcpyHostToDevice, st));
@@ -446,7 +448,8 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             double sm; memcpy(&sm, &h_smax, sizeof(sm));
             int ex = 0; frexp(sm > 0 ? sm : 1.0, &ex);          // sm < 2^ex
             mid_F = 30 - ex;                                     // acc <= min(R_a, R_b) * 2^F < 2^30 (+ rounding slack)
-            uint2* pk = A.get_n<uint2>(mid_entries ? mid_entries : 1);
+            (void)mid_entries;
+            uint2* pk = A.get_n<uint2>(h_pk_total ? h_pk_total : 1);
             k_mid_pack<<<cdiv((long long)n_mid * 32, TB), TB, 0, st>>>(n_mid, mbase, mlen, ts, reinterpret_cast<const float*>(tv), mseg, moff, tbase,
                                                                       ldexpf(1.0f, mid_F), pk); CU_LAUNCH(); ++launches;
             MidParams M{};
