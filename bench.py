@@ -123,7 +123,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=2)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default=os.environ.get("UNIFRAC_BENCH_WORKLOAD", "emp"))
+    ap.add_argument("--workload", default=os.environ.get("UNIFRAC_BENCH_WORKLOAD", "large"))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--seed", type=int, default=0)
     ap.add_argument("--flags", type=int, default=0)

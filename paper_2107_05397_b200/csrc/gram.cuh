@@ -143,7 +143,23 @@ struct GramParams {
     float* out;                   // condensed fp32
     int add_out;
     int q;                        // fixed-point scale
+    // producer pacing (keeps the CTAs' K positions within two epochs of each other so that operand tiles shared by
+    // the tile pairs of a block are still L2-resident when the slower CTAs reach them)
+    unsigned int* epoch_cnt;      // [steps_per_cta >> epoch_shift + 1], zeroed per launch; NULL = no pacing
+    uint32_t steps_per_cta;       // ceil(n_pairs / grid) * (K_pad / GRAM_BK): the same for every CTA
+    uint32_t epoch_shift;         // epoch = 2^epoch_shift k-blocks
 };
+
+// arrive at epoch e; before starting it, wait until every CTA has started epoch e - 1 (bounded spin: pacing only)
+__device__ __forceinline__ void gram_epoch_sync(unsigned int* cnt, uint32_t e, uint32_t n_cta) {
+    atomicAdd(cnt + e, 1u);
+    if (e == 0) return;
+    const volatile unsigned int* prev = cnt + (e - 1);
+    for (uint32_t spin = 0; spin < (1u << 20); ++spin) {
+        if (*prev >= n_cta) break;
+        __nanosleep(64);
+    }
+}
 
 __global__ void __launch_bounds__(GRAM_THREADS, 1)
 k_gram(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB0,
@@ -178,10 +194,12 @@ k_gram(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensor
     if (warp == 0) {
         // ======================================================= TMA producer
         if (lane == 0) {
-            uint32_t stage = 0, phase = 0;
+            uint32_t stage = 0, phase = 0, g = 0;
+            const uint32_t emask = (1u << P.epoch_shift) - 1u;
             for (uint32_t pi = blockIdx.x; pi < P.n_pairs; pi += gridDim.x) {
                 const int2 ij = P.pairs[pi];
-                for (uint32_t kb = 0; kb < n_k; ++kb) {
+                for (uint32_t kb = 0; kb < n_k; ++kb, ++g) {
+                    if (P.epoch_cnt && (g & emask) == 0u) gram_epoch_sync(P.epoch_cnt, g >> P.epoch_shift, gridDim.x);
                     mbar_wait(empty(stage), phase ^ 1u);
                     const uint32_t dst = base + stage * GRAM_STAGE_BYTES;
                     mbar_arrive_expect_tx(full(stage), GRAM_STAGE_BYTES);
@@ -193,6 +211,10 @@ k_gram(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensor
                     if (++stage == GRAM_STAGES) { stage = 0; phase ^= 1u; }
                 }
             }
+            // CTAs with one tile pair fewer still arrive at the remaining epochs
+            if (P.epoch_cnt)
+                for (; g < P.steps_per_cta; ++g)
+                    if ((g & emask) == 0u) atomicAdd(P.epoch_cnt + (g >> P.epoch_shift), 1u);
         }
     } else if (warp == 1) {
         // ======================================================= MMA issuer

@@ -218,8 +218,11 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     const int n_tiles = cdiv(N, TILE);
     const double Pd = 0.5 * (double)N * (double)(N - 1), n_tp = 0.5 * (double)n_tiles * (n_tiles + 1);
     auto envd = [](const char* k, double d) { const char* e = getenv(k); return e ? atof(e) : d; };
-    const double R_tail = envd("UNIFRAC_B200_R_TAIL", 1.6e11), R_mid = envd("UNIFRAC_B200_R_MID", 1.2e12);
-    const double R_head = envd("UNIFRAC_B200_R_HEAD", 1.07e13), gram_Bps = envd("UNIFRAC_B200_GRAM_BPS", 6.0e12);
+    const double R_tail = envd("UNIFRAC_B200_R_TAIL", 1.6e11), R_mid = envd("UNIFRAC_B200_R_MID", 1.6e12);
+    const double R_head = envd("UNIFRAC_B200_R_HEAD", std::is_same<T, float>::value ? 1.4e13 : 3.3e12), gram_Bps = envd("UNIFRAC_B200_GRAM_BPS", 1.15e13);
+    // the rows that compete with the Gram kernel are sparse (a few entries per tile), where k_mid's per-entry overhead
+    // halves its update rate (measured 5.9e11 /s at Large against 1.3e12 - 1.6e12 /s for the denser rows of the weighted variant)
+    const double R_mid_head = gram ? envd("UNIFRAC_B200_R_MID_SPARSE", 5.5e11) : R_mid;
     const double c_ent = envd("UNIFRAC_B200_MID_ENT_S", 3e-12);         // seconds per (mid entry, tile pair) visit of the join kernel
     const double head_s = gram ? n_tp * 512.0 / gram_Bps : Pd / R_head;  // seconds per head branch
     double c2_head, c2_mid;
@@ -227,7 +230,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         // mid row: n_v entries, each visited once per tile J >= its own tile (~ n_tiles / 2 visits) + C(n_v,2) / R_mid;
         // tail row: C(n_v,2) / R_tail  =>  mid wins for n_v > 1 + n_tiles * c_ent / (1/R_tail - 1/R_mid)
         const double nstar = 1.0 + (double)n_tiles * c_ent / (1.0 / R_tail - 1.0 / R_mid);
-        c2_head = head_s * R_mid; c2_mid = 0.5 * nstar * (nstar - 1.0);
+        c2_head = head_s * R_mid_head; c2_mid = 0.5 * nstar * (nstar - 1.0);
         if (c2_mid > c2_head) c2_mid = c2_head;
     } else { c2_head = head_s * R_tail; c2_mid = INFINITY; }
     uint32_t force = 0;
@@ -491,6 +494,14 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             G.out = reinterpret_cast<float*>(out); G.add_out = (tail_rows || mid_rows) ? 1 : 0; G.q = gram_q;
             CU(cudaFuncSetAttribute(k_gram, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GRAM_SMEM));
             unsigned grid = (unsigned)std::min<long long>(n_sm, n_pairs);
+            const int eshift = (int)envd("UNIFRAC_B200_GRAM_EPOCH_SHIFT", 5);
+            if (eshift >= 0) {
+                G.steps_per_cta = (uint32_t)((n_pairs + grid - 1) / grid) * (K_pad / GRAM_BK);
+                G.epoch_shift = (uint32_t)eshift;
+                const size_t n_ep = ((size_t)G.steps_per_cta >> eshift) + 2;
+                G.epoch_cnt = A.get_n<unsigned int>(n_ep);
+                CU(cudaMemsetAsync(G.epoch_cnt, 0, sizeof(unsigned int) * n_ep, st));
+            }
             k_gram<<<grid, GRAM_THREADS, GRAM_SMEM, st>>>(tmA, tmB0, tmB1, tmB2, G); CU_LAUNCH(); ++launches; ++stripe_launches;
             CU(cudaStreamSynchronize(st));       // h_pairs staging copy done before it goes out of scope
         }
