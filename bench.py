@@ -34,6 +34,10 @@ SM_COUNT, FP32_LANES, SM_MAX_GHZ = 148, 128, 1.965        # B200_PROFILING.md / 
 ALU_PEAK_TFLOPS = SM_COUNT * FP32_LANES * SM_MAX_GHZ / 1e3    # FADD/FMNMX-class lane-ops (not FMA-doubled)
 MID_ATOMS_PER_CLK_SM = 32.0     # one conflict-free shared-memory wavefront (32 banks) per clock per SM
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full captures of profiles/r01_summary.md
+# (default flags, seed 0; k_mid: mean of the unweighted and the weighted launch); other workloads: null
+NCU_TRAFFIC_BYTES = {"large": {"k_dense": 237.7e9, "k_gram": 300.1e9, "k_mid": 191.8e9, "k_tail_scatter": 0.227e9}}
+
 WORKLOADS = {   # name -> (variants, precision)    BASELINE.json:7-11
     "tiny": ((0, 1), 1), "small": ((0, 1), 1), "medium": ((0,), 0), "emp": ((0, 1), 0), "large": ((0, 1), 0),
 }
@@ -288,6 +292,9 @@ def main():
                        ms_per_launch=1e3 * t / max(1, nl), seconds=t, share_of_step=t / step_s,
                        note="ms_mid also covers the mid list preparation kernels (k_mid_seg/off/pack)",
                        peak_source=f"{MID_ATOMS_PER_CLK_SM} ATOMS.ADD lane-ops/clk/SM x {SM_COUNT} SMs x {SM_MAX_GHZ} GHz (DESIGN.md 'k_mid')"))
+    for r in rl:
+        if a.flags == 0 and a.seed == 0:
+            r["traffic"] = NCU_TRAFFIC_BYTES.get(a.workload, {}).get(r["kernel"])
     rl.sort(key=lambda r: -r["seconds"])
     roofline = dict(rl[0])
     roofline["others"] = rl[1:]

@@ -20,7 +20,7 @@
 
 namespace ufb {
 
-constexpr int MID_THREADS = 384;
+constexpr int MID_THREADS = 512;
 constexpr int MID_MINB = 3;                         // CTAs per SM (3 x 64.5 KB of accumulators)
 // accumulator cell (a, b) lives at word a * 128 + (b ^ (a & 31)): bank = (a ^ b) mod 32, and the byte address is
 // one LOP3 away from the packed entry word:  (row_base(a) | (a & 31) << 2) ^ (b << 2)
