@@ -47,22 +47,24 @@ __global__ void k_mid_rows(int n, const uint8_t* __restrict__ cls, const uint32_
     }
 }
 
-// seg[t][r] for t = 0..n_tiles (thread per (t, r), r fastest)
-__global__ void k_mid_seg(uint32_t n_mid, const int32_t* __restrict__ mrows, const uint32_t* __restrict__ tptr,
-                          const uint32_t* __restrict__ ts, int n_tiles, uint32_t* __restrict__ seg)
+// seg[t][r] for t = 0..n_tiles = number of entries of row r with sample < 128 t.  One warp per mid row walks the row's
+// sorted sample list; the lane that sees the first entry of a new tile fills the boundaries up to that tile.
+__global__ void __launch_bounds__(256)
+k_mid_seg(uint32_t n_mid, const int32_t* __restrict__ mrows, const uint32_t* __restrict__ tptr,
+          const uint32_t* __restrict__ ts, int n_tiles, uint32_t* __restrict__ seg)
 {
-    long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    uint32_t t = (uint32_t)(gid / n_mid), r = (uint32_t)(gid - (long long)t * n_mid);
-    if (t > (uint32_t)n_tiles) return;
+    const uint32_t r = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (r >= n_mid) return;
     const int v = mrows[r];
-    const uint32_t lo0 = tptr[v], hi0 = tptr[v + 1];
-    uint32_t lo = lo0, hi = hi0;
-    const uint32_t key = t * (uint32_t)TILE;
-    while (lo < hi) {
-        uint32_t mid = lo + ((hi - lo) >> 1);
-        if (ts[mid] < key) lo = mid + 1; else hi = mid;
+    const uint32_t base = tptr[v], m = tptr[v + 1] - base;
+    for (uint32_t k = lane; k < m; k += 32) {
+        const int t1 = (int)(ts[base + k] >> 7);
+        const int t0 = k ? (int)(ts[base + k - 1] >> 7) : -1;
+        for (int t = t0 + 1; t <= t1; ++t) seg[(size_t)t * n_mid + r] = k;
     }
-    seg[(size_t)t * n_mid + r] = lo - lo0;
+    const int tl = m ? (int)(ts[base + m - 1] >> 7) : -1;
+    for (int t = tl + 1 + lane; t <= n_tiles; t += 32) seg[(size_t)t * n_mid + r] = m;
 }
 
 // off[t][r], r = 0..n_mid: offset (within tile t's packed entries) of row r's first entry in tile t;

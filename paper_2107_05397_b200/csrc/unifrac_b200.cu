@@ -432,7 +432,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>(N + 1, mhist, mcur); CU_LAUNCH(); ++launches;
             k_mid_rows<<<cdiv(n, TB), TB, 0, st>>>(n, cls, nv, mcur, tptr, mrows, mbase, mlen); CU_LAUNCH(); ++launches;
             uint32_t* mseg = A.get_n<uint32_t>((size_t)(n_tiles + 1) * n_mid);
-            k_mid_seg<<<cdiv((long long)(n_tiles + 1) * n_mid, TB), TB, 0, st>>>(n_mid, mrows, tptr, ts, n_tiles, mseg); CU_LAUNCH(); ++launches;
+            k_mid_seg<<<cdiv((long long)n_mid * 32, TB), TB, 0, st>>>(n_mid, mrows, tptr, ts, n_tiles, mseg); CU_LAUNCH(); ++launches;
             uint32_t* moff = A.get_n<uint32_t>((size_t)n_tiles * ((size_t)n_mid + 1));
             uint32_t* ttot = A.get_n<uint32_t>(n_tiles);
             uint32_t* tbase = A.get_n<uint32_t>((size_t)n_tiles + 1);
