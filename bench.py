@@ -134,6 +134,9 @@ def main():
     ap.add_argument("--cpu-budget-s", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--shard", action="store_true",
+                    help="N > 1: the ranks compute disjoint shards of ONE matrix (unifrac_dm_shard, strong scaling) "
+                         "instead of independent replicas (default, weak scaling)")
     a = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -164,7 +167,8 @@ def main():
         return 0
 
     # ---------------------------------------------------------------- our arm
-    p = synth.make_config(a.workload, seed=rank_seed(a.seed, rank))       # generated before CUDA is touched (fork pool)
+    shard = (rank, world) if (a.shard and world > 1) else None
+    p = synth.make_config(a.workload, seed=a.seed if shard else rank_seed(a.seed, rank))   # generated before CUDA is touched (fork pool)
     os.environ["UNIFRAC_B200_TIMING"] = "1"
     import torch
     from paper_2107_05397_b200 import binding
@@ -180,7 +184,7 @@ def main():
     def step():
         stats = []
         for v in variants:
-            binding.unifrac_dm(*args, p.n_samples, v, precision, out=outs[v], flags=a.flags)
+            binding.unifrac_dm(*args, p.n_samples, v, precision, out=outs[v], flags=a.flags, shard=shard)
             stats.append(binding.unifrac_last_stats())     # waits for the call's stripe kernel (stats event)
         return stats
 
@@ -206,12 +210,15 @@ def main():
     stop.set()
     th.join(timeout=3)
     flat = [s for st in all_stats for s in st]
-    ms, upd_all = reduce_over_ranks(e0.elapsed_time(e1), float(sum(s["updates_dense"] for s in flat)), world, dev)
+    upd_local = float(sum(s["updates_dense"] for s in flat))
+    if shard:
+        upd_local /= world               # the ranks share one matrix: its updates are counted once
+    ms, upd_all = reduce_over_ranks(e0.elapsed_time(e1), upd_local, world, dev)
     value = upd_all / (ms * 1e-3)
 
     # ---------------- end to end through the host-buffer C-ABI call (H2D + D2H inside the timed region)
     e2e = None
-    if not a.no_e2e:
+    if not a.no_e2e and not shard:      # the host-buffer entry point computes whole matrices
         pin = lambda arr: torch.from_numpy(np.ascontiguousarray(arr)).pin_memory().numpy()
         hp = [pin(x) for x in (p.parent, p.branch_len, p.postorder, p.indptr, p.indices, p.counts)]
         hout = torch.empty(p.n_pairs, dtype=torch.float32 if precision == 0 else torch.float64).pin_memory().numpy()
@@ -327,9 +334,10 @@ def main():
             branches_embedded=ss[0]["branches_embedded"], workspace_gb=ss[0]["workspace_bytes"] / 2**30)
 
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=a.steps, warmup=a.warmup, ms_per_step=ms / a.steps,
-                higher_is_better=True, scaling="weak", vs_baseline=None, dtype=dtype, data="synthetic",
+                higher_is_better=True, scaling="strong" if shard else "weak", vs_baseline=None, dtype=dtype, data="synthetic",
                 config=dict(workload=a.workload, n_samples=p.n_samples, n_nodes=p.n_nodes, nnz=p.nnz, seed=a.seed,
-                            variants=list(variants), precision=dtype, flags=a.flags, parallelism=f"replicas x{world}",
+                            variants=list(variants), precision=dtype, flags=a.flags,
+                            parallelism=f"shards x{world} (disjoint tile-pair blocks, no collective)" if shard else f"replicas x{world}",
                             l2="inputs larger than L2 (compact embedding >> 126 MB)"),
                 clocks=summarize_clocks(lines), e2e=e2e, gpu_launches=int(sum(s["kernel_launches"] for s in flat)),
                 roofline=roofline, cpu_baseline=cpu, wall=per_variant)

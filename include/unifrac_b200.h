@@ -111,6 +111,27 @@ int unifrac_dm(int32_t n_nodes, const int32_t *tree_parent, const double *branch
                unifrac_alloc_fn alloc, void *alloc_user, uint32_t flags, void *stream);
 
 /*
+ * unifrac_dm_shard -- one shard of the same computation, for one process per GPU (the paper's "set of stripes" split,
+ * independent pieces of the matrix, merged afterwards).  The upper triangle is cut into blocks of
+ * UNIFRAC_SHARD_BLOCK x UNIFRAC_SHARD_BLOCK sample tiles (128 samples each) that are dealt round-robin to the shards:
+ * block (bi <= bj) belongs to shard (bj*(bj+1)/2 + bi) % shard_count  (see unifrac_shard_of_pair).  Every shard
+ * embeds the whole table (cheap) and runs step a-5 / a-6 only for its own blocks: no data-path communication.
+ * On return (after the stream work completes) `out_condensed` holds the distances of the pairs this shard owns and
+ * 0 everywhere else, so the full matrix is the element-wise SUM (or an all-gather by owner) of the shards' buffers.
+ * shard_count = 1 is unifrac_dm.  0 <= shard_index < shard_count <= 255, else UNIFRAC_ERR_INVALID_ARG.
+ * The debug flags LITERAL / ABSDIFF / SPARSE_STRIPE / NO_TAIL are not available in shard mode (UNIFRAC_ERR_INVALID_ARG).
+ */
+#define UNIFRAC_SHARD_BLOCK 12
+int unifrac_dm_shard(int32_t n_nodes, const int32_t *tree_parent, const double *branch_len,
+                     const int32_t *postorder, unifrac_csr_t table, int32_t n_samples,
+                     unifrac_variant_t variant, unifrac_precision_t precision, void *out_condensed,
+                     unifrac_alloc_fn alloc, void *alloc_user, uint32_t flags, void *stream,
+                     int32_t shard_index, int32_t shard_count);
+
+/* owner shard of the pair of samples (i, j), i != j  (host helper, no CUDA) */
+int32_t unifrac_shard_of_pair(int32_t i, int32_t j, int32_t shard_count);
+
+/*
  * unifrac_dm_host -- same computation with HOST buffers (pageable or pinned).  The library
  * allocates device memory itself (cudaMalloc), copies the inputs in, runs unifrac_dm on an
  * internal stream, copies the condensed result out to `out_condensed_host`, frees everything
@@ -157,7 +178,7 @@ int unifrac_last_stats(unifrac_stats_t *out);
 
 const char *unifrac_status_string(int status);
 const char *unifrac_last_cuda_error(void);   /* text of the last CUDA error seen by this thread  */
-int unifrac_abi_version(void);               /* 3                                                */
+int unifrac_abi_version(void);               /* 4                                                */
 
 #ifdef __cplusplus
 }

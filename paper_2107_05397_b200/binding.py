@@ -23,7 +23,7 @@ OK = 0
 ERR_INVALID_ARG, ERR_INVALID_TREE, ERR_INVALID_TABLE, ERR_EMPTY_SAMPLE = -1, -2, -3, -4
 ERR_WORKSPACE, ERR_CUDA, ERR_UNSUPPORTED = -5, -6, -7
 
-EXPORTS = ("unifrac_dm", "unifrac_dm_host", "unifrac_last_stats", "unifrac_status_string",
+EXPORTS = ("unifrac_dm", "unifrac_dm_shard", "unifrac_shard_of_pair", "unifrac_dm_host", "unifrac_last_stats", "unifrac_status_string",
            "unifrac_last_cuda_error", "unifrac_abi_version")
 
 
@@ -74,6 +74,10 @@ def load(build_if_missing: bool = True) -> C.CDLL:
     lib.unifrac_dm.restype = C.c_int
     lib.unifrac_dm.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, CSR, C.c_int32, C.c_int, C.c_int,
                                C.c_void_p, ALLOC_FN, C.c_void_p, C.c_uint32, C.c_void_p]
+    lib.unifrac_dm_shard.restype = C.c_int
+    lib.unifrac_dm_shard.argtypes = lib.unifrac_dm.argtypes + [C.c_int32, C.c_int32]
+    lib.unifrac_shard_of_pair.restype = C.c_int32
+    lib.unifrac_shard_of_pair.argtypes = [C.c_int32, C.c_int32, C.c_int32]
     lib.unifrac_dm_host.restype = C.c_int
     lib.unifrac_dm_host.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, CSR, C.c_int32, C.c_int, C.c_int,
                                     C.c_void_p, C.c_uint32]
@@ -96,8 +100,8 @@ def _check(lib, rc: int):
 
 
 def unifrac_dm(tree_parent, branch_len, postorder, indptr, indices, counts, n_samples: int, variant: int,
-               precision: int, out=None, flags: int = 0, stream=None):
-    """Device entry point.  All inputs are CUDA torch tensors (int32 / float64 / int32 / int64 / int32 /
+               precision: int, out=None, flags: int = 0, stream=None, shard=None):
+    """Device entry point (`shard=(index, count)` calls unifrac_dm_shard: this shard's blocks, 0 elsewhere).  All inputs are CUDA torch tensors (int32 / float64 / int32 / int64 / int32 /
     int32); returns the condensed matrix as a CUDA tensor (float32 or float64).  Asynchronous on
     `stream` (default: torch's current stream) after the plan/embedding steps."""
     import torch
@@ -124,10 +128,13 @@ def unifrac_dm(tree_parent, branch_len, postorder, indptr, indices, counts, n_sa
     with torch.cuda.device(dev):
         s = stream if stream is not None else torch.cuda.current_stream(dev)
         with torch.cuda.stream(s):
-            rc = lib.unifrac_dm(int(tree_parent.shape[0]), tree_parent.data_ptr(), branch_len.data_ptr(),
-                                postorder.data_ptr(), CSR(indptr.data_ptr(), indices.data_ptr(), counts.data_ptr()),
-                                n, int(variant), int(precision), out.data_ptr(), cb, None, int(flags),
-                                C.c_void_p(s.cuda_stream))
+            common = (int(tree_parent.shape[0]), tree_parent.data_ptr(), branch_len.data_ptr(),
+                      postorder.data_ptr(), CSR(indptr.data_ptr(), indices.data_ptr(), counts.data_ptr()),
+                      n, int(variant), int(precision), out.data_ptr(), cb, None, int(flags), C.c_void_p(s.cuda_stream))
+            if shard is None:
+                rc = lib.unifrac_dm(*common)
+            else:
+                rc = lib.unifrac_dm_shard(*common, int(shard[0]), int(shard[1]))
     # workspace tensors were allocated under `s`; dropping them here is stream-ordered safe
     del held
     _check(lib, rc)
@@ -157,6 +164,10 @@ def unifrac_last_stats() -> dict:
     s = Stats()
     _check(lib, lib.unifrac_last_stats(C.byref(s)))
     return {k: getattr(s, k) for k, _ in Stats._fields_}
+
+
+def unifrac_shard_of_pair(i: int, j: int, shard_count: int) -> int:
+    return int(load().unifrac_shard_of_pair(int(i), int(j), int(shard_count)))
 
 
 def unifrac_status_string(status: int) -> str:

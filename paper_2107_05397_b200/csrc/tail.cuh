@@ -166,7 +166,17 @@ struct TailParams {
     long long N;
     void* out;
     unsigned int* counter;  // dynamic chunk queue (one word per launch)
+    const uint8_t* owner;   // shard mode: owner[bj*(bj+1)/2 + bi] of every SHARD_BLOCK x SHARD_BLOCK block of tiles; NULL = all
+    int shard;              // this shard's index
 };
+
+constexpr int SHARD_BLOCK = 12;          // == UNIFRAC_SHARD_BLOCK of the C header
+// does this shard own the pair of samples a < b ?  (owner table lookups hit L1)
+__device__ __forceinline__ bool tail_owns(const TailParams& P, long long a, long long b) {
+    if (!P.owner) return true;
+    const uint32_t bi = ((uint32_t)a >> 7) / SHARD_BLOCK, bj = ((uint32_t)b >> 7) / SHARD_BLOCK;
+    return P.owner[bj * (bj + 1) / 2 + bi] == (uint8_t)P.shard;
+}
 
 constexpr int TAIL_SMALL = 8;
 
@@ -203,7 +213,8 @@ k_tail_scatter(const TailParams P)
                 const long long rowoff = a * (2 * N - a - 1) / 2 - a - 1;
                 for (uint32_t l = diag ? k + 1 : j0; l < j1; ++l) {
                     const T vb = tv[base + l];
-                    red_add(out + rowoff + P.ts[base + l], va < vb ? va : vb);
+                    const long long b = P.ts[base + l];
+                    if (tail_owns(P, a, b)) red_add(out + rowoff + b, va < vb ? va : vb);
                 }
             }
         }
@@ -228,7 +239,7 @@ k_tail_scatter(const TailParams P)
                 for (uint32_t k = q0; k < kend; ++k) {
                     const long long sf = P.ts[bb + k];        // warp-uniform (broadcast) loads
                     const T vf = tv[bb + k];
-                    if (lv && (!diag || k < l)) {
+                    if (lv && (!diag || k < l) && (lanesJ ? tail_owns(P, sf, se) : tail_owns(P, se, sf))) {
                         const T m = ve < vf ? ve : vf;
                         if (lanesJ) red_add(out + (sf * (2 * N - sf - 1) / 2 - sf - 1) + se, m);
                         else        red_add(out + rowoff_e + sf, m);

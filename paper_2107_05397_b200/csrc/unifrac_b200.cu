@@ -94,14 +94,21 @@ CUtensorMap make_u8_rowmajor_map(void* base, uint64_t cols, uint64_t rows, uint3
 }
 
 // tile pairs (I <= J) in BLK x BLK blocks of tiles, so that CTAs working on consecutive pairs share operand tiles in L2
-std::vector<int2> blocked_pairs(int n_tiles, int BLK)
+// owner shard of the tile pair (I <= J): blocks of SHARD_BLOCK x SHARD_BLOCK tiles dealt round-robin (unifrac_b200.h)
+inline int shard_of_tiles(int I, int J, int n_shards)
+{
+    const long long bi = I / SHARD_BLOCK, bj = J / SHARD_BLOCK;
+    return (int)((bj * (bj + 1) / 2 + bi) % n_shards);
+}
+std::vector<int2> blocked_pairs(int n_tiles, int BLK, int shard = 0, int n_shards = 1)
 {
     std::vector<int2> v;
-    v.reserve((size_t)n_tiles * (n_tiles + 1) / 2);
+    v.reserve((size_t)n_tiles * (n_tiles + 1) / 2 / n_shards + 1);
     for (int bi = 0; bi < n_tiles; bi += BLK)
         for (int bj = bi; bj < n_tiles; bj += BLK)
             for (int i = bi; i < std::min(n_tiles, bi + BLK); ++i)
-                for (int j = std::max(i, bj); j < std::min(n_tiles, bj + BLK); ++j) v.push_back(make_int2(i, j));
+                for (int j = std::max(i, bj); j < std::min(n_tiles, bj + BLK); ++j)
+                    if (n_shards == 1 || shard_of_tiles(i, j, n_shards) == shard) v.push_back(make_int2(i, j));
     return v;
 }
 
@@ -115,7 +122,7 @@ struct Timer {
 
 template <typename T>
 void run(int32_t n, const int32_t* parent, const double* len, const int32_t* postorder, unifrac_csr_t tab,
-         int32_t N, int weighted, void* out, Arena& A, uint32_t flags, cudaStream_t st)
+         int32_t N, int weighted, void* out, Arena& A, uint32_t flags, cudaStream_t st, int shard, int n_shards)
 {
     const bool validate = !(flags & UNIFRAC_FLAG_SKIP_VALIDATION);
     const bool timing = getenv("UNIFRAC_B200_TIMING") && atoi(getenv("UNIFRAC_B200_TIMING")) != 0;
@@ -388,7 +395,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
 
     // ------------------------------------------------------------------ a-5 (tail branches): scatter into the condensed matrix
     unsigned tail_launches = 0;
-    if (tail_rows || mid_rows) CU(cudaMemsetAsync(out, 0, sizeof(T) * ((size_t)N * (N - 1) / 2), st));
+    if (tail_rows || mid_rows || n_shards > 1) CU(cudaMemsetAsync(out, 0, sizeof(T) * ((size_t)N * (N - 1) / 2), st));
     if (tail_rows) {
         // super tiles: SUP x SUP samples whose condensed row segments (SUP * SUP * sizeof(T)) stay L2-resident
         size_t l2_budget = (size_t)48 << 20;
@@ -405,6 +412,16 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         CU(cudaGetDevice(&dev));
         CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
         TailParams TP{};
+        if (n_shards > 1) {
+            const int nb = cdiv(n_tiles, SHARD_BLOCK);
+            std::vector<uint8_t> h_owner((size_t)nb * (nb + 1) / 2);
+            for (int bj = 0; bj < nb; ++bj)
+                for (int bi = 0; bi <= bj; ++bi) h_owner[(size_t)bj * (bj + 1) / 2 + bi] = (uint8_t)(((long long)bj * (bj + 1) / 2 + bi) % n_shards);
+            uint8_t* owner = A.get_n<uint8_t>(h_owner.size());
+            CU(cudaMemcpyAsync(owner, h_owner.data(), h_owner.size(), cudaMemcpyHostToDevice, st));
+            CU(cudaStreamSynchronize(st));
+            TP.owner = owner; TP.shard = shard;
+        }
         TP.tptr = tptr; TP.seg = seg; TP.ts = ts; TP.tv = tv; TP.cls = cls; TP.n = n; TP.nsup = nsup; TP.N = N; TP.out = out;
         int li = 0;
         for (int si = 0; si < nsup; ++si)
@@ -444,7 +461,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             CU(cudaMemcpyAsync(&h_smax, smax, sizeof(h_smax), cudaMemcpyDeviceToHost, st));
             uint32_t h_pk_total = 0;                            // packed entries incl. the even-length padding
             CU(cudaMemcpyAsync(&h_pk_total, tbase + n_tiles, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
-            std::vector<int2> h_mp = blocked_pairs(n_tiles, 8);
+            std::vector<int2> h_mp = blocked_pairs(n_tiles, 8, shard, n_shards);
             int2* mpairs = A.get_n<int2>(h_mp.size());
             CU(cudaMemcpyAsync(mpairs, h_mp.data(), sizeof(int2) * h_mp.size(), cudaMemcpyHostToDevice, st));
             CU(cudaStreamSynchronize(st));
@@ -465,8 +482,10 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             CU(cudaDeviceGetAttribute(&n_sm2, cudaDevAttrMultiProcessorCount, dev2));
             CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_mid, MID_THREADS, MID_SMEM));
             if (occ < 1) occ = 1;
-            k_mid<<<(unsigned)std::min<long long>((long long)n_sm2 * occ, (long long)h_mp.size()), MID_THREADS, MID_SMEM, st>>>(M);
-            CU_LAUNCH(); ++launches; ++mid_launches;
+            if (!h_mp.empty()) {                                  // a shard may own no tile pair of a small problem
+                k_mid<<<(unsigned)std::min<long long>((long long)n_sm2 * occ, (long long)h_mp.size()), MID_THREADS, MID_SMEM, st>>>(M);
+                CU_LAUNCH(); ++launches; ++mid_launches;
+            }
         }
     }
     tm.mark();
@@ -480,7 +499,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
     if (use_gram) {
         if constexpr (std::is_same<T, float>::value) {
-            std::vector<int2> h_pairs = blocked_pairs(n_tiles, 12);
+            std::vector<int2> h_pairs = blocked_pairs(n_tiles, 12, shard, n_shards);
             n_pairs = (uint32_t)h_pairs.size();
             int2* pairs = A.get_n<int2>(n_pairs);
             CU(cudaMemcpyAsync(pairs, h_pairs.data(), sizeof(int2) * n_pairs, cudaMemcpyHostToDevice, st));
@@ -495,18 +514,18 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             CU(cudaFuncSetAttribute(k_gram, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GRAM_SMEM));
             unsigned grid = (unsigned)std::min<long long>(n_sm, n_pairs);
             const int eshift = (int)envd("UNIFRAC_B200_GRAM_EPOCH_SHIFT", 5);
-            if (eshift >= 0) {
+            if (eshift >= 0 && grid) {
                 G.steps_per_cta = (uint32_t)((n_pairs + grid - 1) / grid) * (K_pad / GRAM_BK);
                 G.epoch_shift = (uint32_t)eshift;
                 const size_t n_ep = ((size_t)G.steps_per_cta >> eshift) + 2;
                 G.epoch_cnt = A.get_n<unsigned int>(n_ep);
                 CU(cudaMemsetAsync(G.epoch_cnt, 0, sizeof(unsigned int) * n_ep, st));
             }
-            k_gram<<<grid, GRAM_THREADS, GRAM_SMEM, st>>>(tmA, tmB0, tmB1, tmB2, G); CU_LAUNCH(); ++launches; ++stripe_launches;
+            if (grid) { k_gram<<<grid, GRAM_THREADS, GRAM_SMEM, st>>>(tmA, tmB0, tmB1, tmB2, G); CU_LAUNCH(); ++launches; ++stripe_launches; }
             CU(cudaStreamSynchronize(st));       // h_pairs staging copy done before it goes out of scope
         }
     } else if (dense_head) {
-        std::vector<int2> h_pairs = blocked_pairs(n_tiles, 12);
+        std::vector<int2> h_pairs = blocked_pairs(n_tiles, 12, shard, n_shards);
         n_pairs = (uint32_t)h_pairs.size();
         int2* pairs = A.get_n<int2>(n_pairs);
         CU(cudaMemcpyAsync(pairs, h_pairs.data(), sizeof(int2) * n_pairs, cudaMemcpyHostToDevice, st));
@@ -520,7 +539,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         CU(cudaFuncSetAttribute(k_dense<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         unsigned grid = (unsigned)std::min<long long>(n_sm, n_pairs);
         D.scratch = A.get_n<double>((size_t)grid * 64 * 256);
-        k_dense<T><<<grid, DENSE_THREADS, smem, st>>>(tmE, D); CU_LAUNCH(); ++launches; ++stripe_launches;
+        if (grid) { k_dense<T><<<grid, DENSE_THREADS, smem, st>>>(tmE, D); CU_LAUNCH(); ++launches; ++stripe_launches; }
         CU(cudaStreamSynchronize(st));           // h_pairs staging copy done before it goes out of scope
     } else {
     std::vector<int2> h_pairs;
@@ -589,8 +608,11 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
 
 int guarded(int32_t n_nodes, const int32_t* parent, const double* len, const int32_t* postorder, unifrac_csr_t tab,
             int32_t N, unifrac_variant_t variant, unifrac_precision_t precision, void* out, unifrac_alloc_fn alloc,
-            void* user, uint32_t flags, cudaStream_t st)
+            void* user, uint32_t flags, cudaStream_t st, int shard = 0, int n_shards = 1)
 {
+    if (n_shards < 1 || n_shards > 255 || shard < 0 || shard >= n_shards) return UNIFRAC_ERR_INVALID_ARG;
+    if (n_shards > 1 && (flags & (UNIFRAC_FLAG_LITERAL | UNIFRAC_FLAG_ABSDIFF | UNIFRAC_FLAG_SPARSE_STRIPE | UNIFRAC_FLAG_NO_TAIL)))
+        return UNIFRAC_ERR_INVALID_ARG;
     if (!parent || !len || !postorder || !tab.indptr || !tab.indices || !tab.counts || !out) return UNIFRAC_ERR_INVALID_ARG;
     if (n_nodes < 2 || N < 2) return UNIFRAC_ERR_INVALID_ARG;
     if (variant != UNIFRAC_UNWEIGHTED && variant != UNIFRAC_WEIGHTED_NORMALIZED) return UNIFRAC_ERR_INVALID_ARG;
@@ -602,8 +624,8 @@ int guarded(int32_t n_nodes, const int32_t* parent, const double* len, const int
     Arena A{alloc, user, st};
     int rc = UNIFRAC_OK;
     try {
-        if (precision == UNIFRAC_FP32) run<float>(n_nodes, parent, len, postorder, tab, N, variant == UNIFRAC_WEIGHTED_NORMALIZED, out, A, flags, st);
-        else run<double>(n_nodes, parent, len, postorder, tab, N, variant == UNIFRAC_WEIGHTED_NORMALIZED, out, A, flags, st);
+        if (precision == UNIFRAC_FP32) run<float>(n_nodes, parent, len, postorder, tab, N, variant == UNIFRAC_WEIGHTED_NORMALIZED, out, A, flags, st, shard, n_shards);
+        else run<double>(n_nodes, parent, len, postorder, tab, N, variant == UNIFRAC_WEIGHTED_NORMALIZED, out, A, flags, st, shard, n_shards);
     } catch (const CudaFail& f) {
         char buf[512];
         snprintf(buf, sizeof(buf), "%s: %s (unifrac_b200.cu:%d)", f.what, cudaGetErrorString(f.e), f.line);
@@ -627,6 +649,22 @@ int unifrac_dm(int32_t n_nodes, const int32_t* tree_parent, const double* branch
 {
     return guarded(n_nodes, tree_parent, branch_len, postorder, table, n_samples, variant, precision, out_condensed,
                    alloc, alloc_user, flags, reinterpret_cast<cudaStream_t>(stream));
+}
+
+int unifrac_dm_shard(int32_t n_nodes, const int32_t* tree_parent, const double* branch_len, const int32_t* postorder,
+                     unifrac_csr_t table, int32_t n_samples, unifrac_variant_t variant, unifrac_precision_t precision,
+                     void* out_condensed, unifrac_alloc_fn alloc, void* alloc_user, uint32_t flags, void* stream,
+                     int32_t shard_index, int32_t shard_count)
+{
+    return guarded(n_nodes, tree_parent, branch_len, postorder, table, n_samples, variant, precision, out_condensed,
+                   alloc, alloc_user, flags, reinterpret_cast<cudaStream_t>(stream), shard_index, shard_count);
+}
+
+int32_t unifrac_shard_of_pair(int32_t i, int32_t j, int32_t shard_count)
+{
+    if (shard_count < 1 || i < 0 || j < 0 || i == j) return -1;
+    const int a = i < j ? i : j, b = i < j ? j : i;
+    return shard_of_tiles(a / TILE, b / TILE, shard_count);
 }
 
 int unifrac_dm_host(int32_t n_nodes, const int32_t* tree_parent, const double* branch_len, const int32_t* postorder,
@@ -703,6 +741,6 @@ const char* unifrac_status_string(int status)
 }
 
 const char* unifrac_last_cuda_error(void) { return g_cuda_err.c_str(); }
-int unifrac_abi_version(void) { return 3; }
+int unifrac_abi_version(void) { return 4; }
 
 }  // extern "C"

@@ -27,7 +27,7 @@ def test_header_symbols_are_exported_and_bound():
 
 
 def test_version_and_status_strings_without_gpu():
-    assert binding.unifrac_abi_version() == 3
+    assert binding.unifrac_abi_version() == 4
     assert binding.unifrac_status_string(0) == "ok"
     assert "tree" in binding.unifrac_status_string(binding.ERR_INVALID_TREE)
 
@@ -46,3 +46,13 @@ def test_library_is_built_for_sm_100a_with_bulk_copies():
     sass = subprocess.run(["cuobjdump", "-sass", build.LIB], capture_output=True, text=True).stdout
     assert "sm_100a" in sass
     assert "UBLKCP" in sass            # cp.async.bulk (TMA bulk copy) in the stripe kernel
+
+
+def test_shard_of_pair_is_a_partition_by_blocks_of_12_tiles():
+    """unifrac_shard_of_pair (host helper): symmetric, constant on 1536 x 1536 sample blocks, round-robin over blocks."""
+    f = binding.unifrac_shard_of_pair
+    assert f(0, 1, 1) == 0 and f(5, 5, 4) == -1
+    assert f(3, 7, 4) == f(7, 3, 4) == 0                     # block (0, 0)
+    assert f(0, 1535, 4) == 0 and f(0, 1536, 4) == 1         # block (0, 1) = linear index 1
+    assert f(1536, 3071, 4) == 2 and f(0, 3072, 4) == 3      # (1, 1) -> 2, (0, 2) -> 3
+    assert f(1536, 3072, 4) == 0 and f(3072, 3073, 4) == 1   # (1, 2) -> 4 % 4, (2, 2) -> 5 % 4

@@ -46,3 +46,44 @@ def test_single_rank_is_identity():
     sys.path.insert(0, ROOT)
     import bench
     assert bench.reduce_over_ranks(3.5, 7.0, 1) == (3.5, 7.0)
+
+
+def _shard_worker(rank, world, port, q):
+    """Shard mode (unifrac_dm_shard): every pair is owned by exactly one rank, so summing the ranks' buffers (the
+    merge of the paper's stripe pieces) reproduces the whole condensed matrix.  The owner map is the
+    library's host helper; the stand-in 'distance' of pair k is k + 1."""
+    sys.path.insert(0, ROOT)
+    from paper_2107_05397_b200 import binding, synth
+    import numpy as np
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    n = 3300                                             # 26 tiles = 3 block rows of 12 tiles
+    rng = np.random.default_rng(0)
+    i = rng.integers(0, n - 1, size=4000)
+    j = rng.integers(i + 1, n)
+    pairs = np.unique(np.stack([i, j], 1), axis=0)
+    own = np.array([binding.unifrac_shard_of_pair(int(a), int(b), world) for a, b in pairs])
+    buf = torch.zeros(len(pairs), dtype=torch.float64)
+    mine = torch.from_numpy(own == rank)
+    buf[mine] = torch.arange(1, len(pairs) + 1, dtype=torch.float64)[mine]
+    dist.all_reduce(buf, op=dist.ReduceOp.SUM)
+    ok = bool(torch.equal(buf, torch.arange(1, len(pairs) + 1, dtype=torch.float64)))
+    q.put((rank, ok, int(mine.sum()), len(pairs)))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_two_rank_shard_merge_by_sum():
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 30100 + (os.getpid() % 500)
+    procs = [ctx.Process(target=_shard_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in range(2))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    (_, ok0, n0, tot), (_, ok1, n1, _) = res
+    assert ok0 and ok1
+    assert n0 + n1 == tot and n0 > 0 and n1 > 0      # disjoint, complete, both ranks own something

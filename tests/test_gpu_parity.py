@@ -232,3 +232,37 @@ def test_stats_work_counters_match_definitions(B):
     st = B.unifrac_last_stats()
     assert st["head_rows"] == 0 and st["tail_updates"] == int((tail * (tail - 1) // 2).sum())
     assert st["tail_entries"] == int(tail.sum()) and st["updates_executed"] == st["tail_updates"]
+
+
+@pytest.mark.parametrize("variant,precision", [(U, 0), (W, 0), (W, 1)])
+def test_shards_partition_the_matrix(B, O, variant, precision):
+    """unifrac_dm_shard: the shards' buffers are disjoint (a pair is non-zero only in the shard
+    unifrac_shard_of_pair names) and their sum is the matrix -- checked against the oracle on sampled pairs and
+    against the unsharded call.  26 tiles = 3 block rows of 12 tiles, ragged last tile."""
+    import torch
+    cfg = synth.CONFIGS["small"]
+    p = synth.make_problem(3000, 3300, 0.1, 1.1, cfg[4], cfg[5], seed=3)
+    n, S = p.n_samples, 4
+    pairs = np.concatenate([synth.sample_pairs(n, 6000, seed=1),
+                            np.array([[0, 1], [0, n - 1], [n - 2, n - 1], [1535, 1536], [0, 1536], [1536, 3072],
+                                      [3071, 3072], [1535, 3299]], dtype=np.int32)])
+    idx = synth.condensed_index(n, pairs[:, 0], pairs[:, 1])
+    want = O.pair_list(p.parent, p.branch_len, p.indptr, p.indices, p.counts, variant, pairs)
+    args = B.to_device(p)
+    full = B.unifrac_dm(*args, n, variant, precision)
+    total = torch.zeros_like(full)
+    owners = np.array([B.unifrac_shard_of_pair(int(i), int(j), S) for i, j in pairs])
+    assert set(owners.tolist()) == set(range(S))
+    for s in range(S):
+        part = B.unifrac_dm(*args, n, variant, precision, shard=(s, S))
+        torch.cuda.synchronize()
+        got = part[torch.from_numpy(idx).cuda()].cpu().numpy().astype(np.float64)
+        assert np.all(got[owners != s] == 0.0)
+        check(got[owners == s], want[owners == s], precision)
+        assert int(torch.count_nonzero(part)) <= int(torch.count_nonzero(full))
+        total += part
+    torch.cuda.synchronize()
+    a, b = total.cpu().numpy().astype(np.float64), full.cpu().numpy().astype(np.float64)
+    assert np.allclose(a, b, rtol=2e-6 if precision == 0 else 1e-12, atol=1e-7 if precision == 0 else 1e-13)
+    with pytest.raises(B.UnifracError):
+        B.unifrac_dm(*args, n, variant, precision, shard=(4, 4))
