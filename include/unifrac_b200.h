@@ -133,9 +133,11 @@ int32_t unifrac_shard_of_pair(int32_t i, int32_t j, int32_t shard_count);
 
 /*
  * unifrac_dm_host -- same computation with HOST buffers (pageable or pinned).  The library
- * allocates device memory itself (cudaMalloc), copies the inputs in, runs unifrac_dm on an
- * internal stream, copies the condensed result out to `out_condensed_host`, frees everything
- * and returns after completion (synchronous).  `nnz` is read from indptr[n_samples].
+ * allocates device memory itself from the device's default stream-ordered pool (cudaMallocAsync), copies the
+ * inputs in, runs unifrac_dm on an internal stream, copies the condensed result out to `out_condensed_host`,
+ * returns every buffer to the pool and returns after completion (synchronous).  The pool's release threshold is
+ * raised so that the memory stays mapped for the next call (cudaMemPoolTrimTo(pool, 0) gives it back).
+ * `nnz` is read from indptr[n_samples].
  */
 int unifrac_dm_host(int32_t n_nodes, const int32_t *tree_parent, const double *branch_len,
                     const int32_t *postorder, unifrac_csr_t table_host, int32_t n_samples,

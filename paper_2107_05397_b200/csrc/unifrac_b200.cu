@@ -683,10 +683,20 @@ int unifrac_dm_host(int32_t n_nodes, const int32_t* tree_parent, const double* b
     int rc = UNIFRAC_OK;
     auto ok = [&](cudaError_t e) { if (e != cudaSuccess && rc == UNIFRAC_OK) { g_cuda_err = cudaGetErrorString(e); cudaGetLastError(); rc = e == cudaErrorMemoryAllocation ? UNIFRAC_ERR_WORKSPACE : UNIFRAC_ERR_CUDA; } return rc == UNIFRAC_OK; };
     ok(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
-    ok(cudaMalloc(&d_parent, sizeof(int32_t) * n_nodes)) && ok(cudaMalloc(&d_len, sizeof(double) * n_nodes)) &&
-    ok(cudaMalloc(&d_post, sizeof(int32_t) * n_nodes)) && ok(cudaMalloc(&d_indptr, sizeof(int64_t) * ((size_t)N + 1))) &&
-    ok(cudaMalloc(&d_idx, sizeof(int32_t) * (size_t)(nnz ? nnz : 1))) && ok(cudaMalloc(&d_cnt, sizeof(int32_t) * (size_t)(nnz ? nnz : 1))) &&
-    ok(cudaMalloc(&d_out, esz * n_out));
+    // All device memory of this call (inputs, output, workspace) comes from the device's stream-ordered pool; the pool keeps
+    // what it has mapped between calls (release threshold = max), so repeated calls do not pay for mapping ~20 GB again.
+    {
+        int dev = 0; cudaMemPool_t pool = nullptr;
+        if (ok(cudaGetDevice(&dev)) && ok(cudaDeviceGetDefaultMemPool(&pool, dev))) {
+            uint64_t keep = UINT64_MAX;
+            ok(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
+        }
+    }
+    auto dalloc = [&](void** p, size_t bytes) { return ok(cudaMallocAsync(p, bytes ? bytes : 256, st)); };
+    dalloc(&d_parent, sizeof(int32_t) * n_nodes) && dalloc(&d_len, sizeof(double) * n_nodes) &&
+    dalloc(&d_post, sizeof(int32_t) * n_nodes) && dalloc(&d_indptr, sizeof(int64_t) * ((size_t)N + 1)) &&
+    dalloc(&d_idx, sizeof(int32_t) * (size_t)nnz) && dalloc(&d_cnt, sizeof(int32_t) * (size_t)nnz) &&
+    dalloc(&d_out, esz * n_out);
     if (rc == UNIFRAC_OK) {
         ok(cudaMemcpyAsync(d_parent, tree_parent, sizeof(int32_t) * n_nodes, cudaMemcpyHostToDevice, st));
         ok(cudaMemcpyAsync(d_len, branch_len, sizeof(double) * n_nodes, cudaMemcpyHostToDevice, st));
@@ -702,11 +712,9 @@ int unifrac_dm_host(int32_t n_nodes, const int32_t* tree_parent, const double* b
     }
     if (rc == UNIFRAC_OK) {
         ok(cudaMemcpyAsync(out_host, d_out, esz * n_out, cudaMemcpyDeviceToHost, st));
-        ok(cudaStreamSynchronize(st));
     }
-    if (st) cudaStreamSynchronize(st);
-    cudaFree(d_parent); cudaFree(d_len); cudaFree(d_post); cudaFree(d_indptr); cudaFree(d_idx); cudaFree(d_cnt); cudaFree(d_out);
-    if (st) cudaStreamDestroy(st);
+    for (void* p : {d_parent, d_len, d_post, d_indptr, d_idx, d_cnt, d_out}) if (p && st) cudaFreeAsync(p, st);
+    if (st) { ok(cudaStreamSynchronize(st)); cudaStreamDestroy(st); }
     return rc;
 }
 
