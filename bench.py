@@ -32,7 +32,9 @@ METRIC = "unifrac_dense_equivalent_pair_branch_updates_per_s"
 UNIT = "updates/s"
 SM_COUNT, FP32_LANES, SM_MAX_GHZ = 148, 128, 1.965        # B200_PROFILING.md / MEASURED_PEAKS.json
 ALU_PEAK_TFLOPS = SM_COUNT * FP32_LANES * SM_MAX_GHZ / 1e3    # FADD/FMNMX-class lane-ops (not FMA-doubled)
-MID_ATOMS_PER_CLK_SM = 32.0     # one conflict-free shared-memory wavefront (32 banks) per clock per SM
+# fallbacks when unifrac_measure_rates is not run (values it measured on this pool's B200: 8.84 shared-memory atomic
+# lane-ops/clk/SM, independent of bank conflicts; 1.94e11 L2-resident scattered fp32 REDs/s)
+SMEM_ATOMIC_PER_S, L2_RED_PER_S = 8.84 * SM_COUNT * SM_MAX_GHZ * 1e9, 1.94e11
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full captures of profiles/r01_summary.md
 # (default flags, seed 0; k_mid: mean of the unweighted and the weighted launch); other workloads: null
@@ -245,7 +247,16 @@ def main():
             dist.destroy_process_group()
         return 0
 
-    # ---------------- rooflines of the three a-5 kernels; the one with the most time in the step is "roofline"
+    # ---------------- device rates of the atomic units (peaks of the k_mid / k_tail_scatter rooflines), measured live
+    rates = dict(smem_atomic_random_per_s=SMEM_ATOMIC_PER_S, l2_red_random_per_s=L2_RED_PER_S)
+    rates_src = "fallback constants (bench.py)"
+    try:
+        rates = binding.unifrac_measure_rates()
+        rates_src = "measured live by unifrac_measure_rates on this GPU"
+    except Exception as e:                                   # noqa: BLE001 - the probe is not on the data path
+        rates_src += f" [probe failed: {e}]"
+
+    # ---------------- rooflines of the a-5 kernels; the one with the most time in the step is "roofline"
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
@@ -287,22 +298,23 @@ def main():
     reds = sum(s["tail_updates"] for s in flat)
     nl = sum(s["tail_launches"] for s in flat)
     if nl:
-        RED_PEAK = 1.93e11      # measured on this pool's B200: random fp32 RED.ADD into a 64 MB footprint (profiles/r01_ubench_red.txt)
+        RED_PEAK = rates["l2_red_random_per_s"]
         rl.append(dict(bound="l2_atomic", achieved=reds / t / 1e9 if t > 0 else 0.0, peak=RED_PEAK / 1e9, unit="GRED/s",
                        frac=reds / t / RED_PEAK if t > 0 else 0.0, traffic=None, kernel="k_tail_scatter", launches=nl,
                        ms_per_launch=1e3 * t / max(1, nl), seconds=t, share_of_step=t / step_s,
-                       peak_source="micro-benchmark of scattered RED.ADD.F32 into an L2-resident footprint, same GPU pool"))
+                       peak_source=f"scattered RED.ADD.F32 into a 48 MB L2-resident footprint, {rates_src}"))
     # (4) k_mid: tile-pair join with native shared-memory integer atomics (ATOMS.ADD), one per (pair, branch) update
     t = sum(s["ms_mid"] for s in flat) * 1e-3
     mu = sum(s["mid_updates"] for s in flat)
     nl = sum(s["mid_launches"] for s in flat)
     if nl:
-        ATOMS_PEAK = MID_ATOMS_PER_CLK_SM * SM_COUNT * SM_MAX_GHZ * 1e9
+        ATOMS_PEAK = rates["smem_atomic_random_per_s"]
         rl.append(dict(bound="smem_atomic", achieved=mu / t / 1e9 if t > 0 else 0.0, peak=ATOMS_PEAK / 1e9, unit="GATOM/s",
                        frac=mu / t / ATOMS_PEAK if t > 0 else 0.0, traffic=None, kernel="k_mid", launches=nl,
                        ms_per_launch=1e3 * t / max(1, nl), seconds=t, share_of_step=t / step_s,
                        note="ms_mid also covers the mid list preparation kernels (k_mid_seg/off/pack)",
-                       peak_source=f"{MID_ATOMS_PER_CLK_SM} ATOMS.ADD lane-ops/clk/SM x {SM_COUNT} SMs x {SM_MAX_GHZ} GHz (DESIGN.md 'k_mid')"))
+                       peak_source=f"shared-memory u32 atomic adds on random cells of a 128 x 128 tile, 3 CTAs/SM x 512 threads "
+                                   f"(= {ATOMS_PEAK / SM_COUNT / SM_MAX_GHZ / 1e9:.2f} lane-ops/clk/SM; same rate conflict-free), {rates_src}"))
     for r in rl:
         if a.flags == 0 and a.seed == 0:
             r["traffic"] = NCU_TRAFFIC_BYTES.get(a.workload, {}).get(r["kernel"])

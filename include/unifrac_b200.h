@@ -178,6 +178,18 @@ typedef struct {
 } unifrac_stats_t;
 int unifrac_last_stats(unifrac_stats_t *out);
 
+/* Device-rate probes (not on the data path): what this GPU retires per second of the two atomic units of work the
+ * sparse kernels are made of; they are the constants of the head / mid / tail cost model and the `peak` of the
+ * k_mid / k_tail_scatter rooflines in bench.py.  Runs ~20 ms of probe kernels on `stream` and synchronises it. */
+typedef struct {
+    double smem_atomic_conflict_free_per_s;  /* shared-memory u32 atomic adds, 32 lanes on 32 different banks        */
+    double smem_atomic_random_per_s;         /* ... on pseudo-random cells of a 128 x 128 tile (k_mid's access pattern) */
+    double l2_red_random_per_s;              /* fp32 RED.ADD on pseudo-random words of a 48 MB (L2-resident) footprint */
+    int32_t sm_count;
+    int32_t sm_clock_khz;                    /* cudaDevAttrClockRate                                               */
+} unifrac_rates_t;
+int unifrac_measure_rates(unifrac_rates_t *out, void *stream);
+
 const char *unifrac_status_string(int status);
 const char *unifrac_last_cuda_error(void);   /* text of the last CUDA error seen by this thread  */
 int unifrac_abi_version(void);               /* 4                                                */

@@ -23,7 +23,7 @@ OK = 0
 ERR_INVALID_ARG, ERR_INVALID_TREE, ERR_INVALID_TABLE, ERR_EMPTY_SAMPLE = -1, -2, -3, -4
 ERR_WORKSPACE, ERR_CUDA, ERR_UNSUPPORTED = -5, -6, -7
 
-EXPORTS = ("unifrac_dm", "unifrac_dm_shard", "unifrac_shard_of_pair", "unifrac_dm_host", "unifrac_last_stats", "unifrac_status_string",
+EXPORTS = ("unifrac_dm", "unifrac_dm_shard", "unifrac_shard_of_pair", "unifrac_dm_host", "unifrac_measure_rates", "unifrac_last_stats", "unifrac_status_string",
            "unifrac_last_cuda_error", "unifrac_abi_version")
 
 
@@ -42,6 +42,11 @@ class Stats(C.Structure):
                 ("kernel_launches", C.c_uint32), ("mid_launches", C.c_uint32), ("mid_F", C.c_uint32), ("gram", C.c_uint32), ("gram_k", C.c_uint32), ("gram_q", C.c_uint32), ("dense", C.c_uint32),
                 ("ms_plan", C.c_float), ("ms_embed", C.c_float), ("ms_tail", C.c_float), ("ms_mid", C.c_float), ("ms_stripe", C.c_float),
                 ("ms_total", C.c_float)]
+
+
+class Rates(C.Structure):
+    _fields_ = [("smem_atomic_conflict_free_per_s", C.c_double), ("smem_atomic_random_per_s", C.c_double),
+                ("l2_red_random_per_s", C.c_double), ("sm_count", C.c_int32), ("sm_clock_khz", C.c_int32)]
 
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
@@ -81,6 +86,8 @@ def load(build_if_missing: bool = True) -> C.CDLL:
     lib.unifrac_dm_host.restype = C.c_int
     lib.unifrac_dm_host.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, CSR, C.c_int32, C.c_int, C.c_int,
                                     C.c_void_p, C.c_uint32]
+    lib.unifrac_measure_rates.restype = C.c_int
+    lib.unifrac_measure_rates.argtypes = [C.POINTER(Rates), C.c_void_p]
     lib.unifrac_last_stats.restype = C.c_int
     lib.unifrac_last_stats.argtypes = [C.POINTER(Stats)]
     lib.unifrac_status_string.restype = C.c_char_p
@@ -164,6 +171,16 @@ def unifrac_last_stats() -> dict:
     s = Stats()
     _check(lib, lib.unifrac_last_stats(C.byref(s)))
     return {k: getattr(s, k) for k, _ in Stats._fields_}
+
+
+def unifrac_measure_rates(stream=None) -> dict:
+    """Device-rate probes (shared-memory atomics, L2 REDs) on torch's current stream."""
+    import torch
+    lib = load()
+    r = Rates()
+    s = stream if stream is not None else torch.cuda.current_stream()
+    _check(lib, lib.unifrac_measure_rates(C.byref(r), C.c_void_p(s.cuda_stream)))
+    return {k: getattr(r, k) for k, _ in Rates._fields_}
 
 
 def unifrac_shard_of_pair(i: int, j: int, shard_count: int) -> int:

@@ -6,8 +6,9 @@
 // 128 x 128 tile pair (I, J) only the n_I x n_J pairs of samples present on BOTH sides contribute
 // min(u~_a, u~_b) to M_ab (identities I3 / I5).  One CTA owns the tile pair's 128 x 128 accumulators in
 // shared memory as 32-bit FIXED-POINT integers and adds the contributions with native shared-memory
-// integer atomics (ATOMS.ADD; measured 8.4 /clk/SM = 2.4e12 /s against 2.6 /clk/SM for the fp32 CAS loop
-// and 1.9e11 /s for global RED.ADD, profiles/r01_ubench_atomics.txt).  Integer addition commutes, so the
+// integer atomics (ATOMS.ADD: 8.84 lane-ops/clk/SM = 2.57e12 /s on B200, the same for conflict-free and for random
+// cells -- unifrac_measure_rates, rates.cuh -- against 2.6 /clk/SM for an fp32 CAS loop and 1.9e11 /s for global
+// RED.ADD).  Integer addition commutes, so the
 // result does not depend on the order in which warps reach a cell.
 //   u_q = round(u~ * 2^F),  F = 30 - ceil(log2(max_s R_s))   =>   acc <= min(R_a, R_b) * 2^F < 2^31
 //   epilogue: out[idx(a,b)] += acc * 2^-F      (exclusive owner of the tile pair; tail REDs ran before)

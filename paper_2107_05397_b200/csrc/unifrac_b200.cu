@@ -10,6 +10,7 @@
 #include "gram.cuh"
 #include "mid.cuh"
 #include "dense.cuh"
+#include "rates.cuh"
 
 #include <cstdio>
 #include <cstdlib>
@@ -731,6 +732,57 @@ int unifrac_last_stats(unifrac_stats_t* out)
     }
     *out = g_stats;
     return UNIFRAC_OK;
+}
+
+int unifrac_measure_rates(unifrac_rates_t* out, void* stream)
+{
+    if (!out) return UNIFRAC_ERR_INVALID_ARG;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    int rc = UNIFRAC_OK;
+    float* buf = nullptr; unsigned int* sink = nullptr;
+    cudaEvent_t e[2] = {nullptr, nullptr};
+    try {
+        int dev = 0, n_sm = 0, khz = 0;
+        CU(cudaGetDevice(&dev));
+        CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+        CU(cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, dev));
+        const uint32_t cells = (48u << 20) / 4u;
+        CU(cudaMallocAsync(reinterpret_cast<void**>(&buf), (size_t)cells * 4, st));
+        CU(cudaMallocAsync(reinterpret_cast<void**>(&sink), 256, st));
+        CU(cudaMemsetAsync(buf, 0, (size_t)cells * 4, st));
+        CU(cudaMemsetAsync(sink, 0, 256, st));
+        CU(cudaEventCreate(&e[0])); CU(cudaEventCreate(&e[1]));
+        const size_t smem = 128 * 128 * 4;
+        CU(cudaFuncSetAttribute(k_rate_atoms, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        auto timed = [&](auto&& launch) {
+            launch();                                        // warm-up
+            CU(cudaEventRecord(e[0], st));
+            launch();
+            CU(cudaEventRecord(e[1], st));
+            CU(cudaEventSynchronize(e[1]));
+            float ms = 0; CU(cudaEventElapsedTime(&ms, e[0], e[1]));
+            return (double)ms * 1e-3;
+        };
+        const int it_a = 4096, it_r = 512;
+        const unsigned ga = (unsigned)n_sm * 3, gr = (unsigned)n_sm * 8;
+        double t0 = timed([&] { k_rate_atoms<<<ga, 512, smem, st>>>(0, it_a, sink); CU_LAUNCH(); });
+        double t1 = timed([&] { k_rate_atoms<<<ga, 512, smem, st>>>(1, it_a, sink); CU_LAUNCH(); });
+        double t2 = timed([&] { k_rate_red<<<gr, 256, 0, st>>>(buf, cells, it_r); CU_LAUNCH(); });
+        out->smem_atomic_conflict_free_per_s = (double)ga * 512 * it_a * 8 / t0;
+        out->smem_atomic_random_per_s = (double)ga * 512 * it_a * 8 / t1;
+        out->l2_red_random_per_s = (double)gr * 256 * it_r * 4 / t2;
+        out->sm_count = n_sm; out->sm_clock_khz = khz;
+    } catch (const CudaFail& f) {
+        char b[512];
+        snprintf(b, sizeof(b), "%s: %s (unifrac_b200.cu:%d)", f.what, cudaGetErrorString(f.e), f.line);
+        g_cuda_err = b; cudaGetLastError(); rc = UNIFRAC_ERR_CUDA;
+    } catch (...) { rc = UNIFRAC_ERR_CUDA; g_cuda_err = "unexpected C++ exception"; }
+    if (e[0]) cudaEventDestroy(e[0]);
+    if (e[1]) cudaEventDestroy(e[1]);
+    if (buf) cudaFreeAsync(buf, st);
+    if (sink) cudaFreeAsync(sink, st);
+    cudaStreamSynchronize(st);
+    return rc;
 }
 
 const char* unifrac_status_string(int status)
