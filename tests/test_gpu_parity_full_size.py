@@ -44,3 +44,44 @@ def test_full_size_sampled_pairs(name, n_pairs):
         assert ok.all(), f"{name} variant {variant}: max rel err {rel.max():.3e}"
         print(f"{name} variant {variant}: max rel err {rel.max():.3e}, p99.99 {np.quantile(rel, 0.9999):.3e}, "
               f"min d {want.min():.4f}, pairs {len(want)}")
+
+
+def _permute_samples(p, perm):
+    """Problem with sample k of the result = sample perm[k] of p (CSR rows reordered; nothing else changes)."""
+    import copy
+    lens = np.diff(p.indptr)[perm]
+    indptr = np.concatenate([[0], np.cumsum(lens)]).astype(p.indptr.dtype)
+    take = np.concatenate([np.arange(p.indptr[s], p.indptr[s + 1]) for s in perm]) if len(perm) else np.zeros(0, np.int64)
+    q = copy.copy(p)
+    q.indptr, q.indices, q.counts = indptr, p.indices[take], p.counts[take]
+    return q
+
+
+@pytest.mark.parametrize("name", ["medium", "emp"])
+def test_full_size_sample_permutation_property(name):
+    """A property that holds at any size (no oracle needed): permuting the samples permutes the matrix.  The permuted run
+    puts every pair into a different tile pair / shared-memory cell / TMEM lane and sums in a different order, so agreement
+    on 5e6 random pairs per variant checks the tiling, the condensed indexing and the head / mid / tail split against
+    themselves at BASELINE.json's sizes (tolerance: twice the fp32 parity tolerance, both runs carry rounding)."""
+    import torch
+    from paper_2107_05397_b200 import binding as B
+    p = synth.make_config(name, seed=0)
+    n = p.n_samples
+    rng = np.random.default_rng(11)
+    perm = rng.permutation(n)
+    q = _permute_samples(p, perm)
+    inv = np.empty(n, dtype=np.int64)
+    inv[perm] = np.arange(n)                                  # sample s of p is sample inv[s] of q
+    pairs = synth.sample_pairs(n, 5_000_000, seed=5).astype(np.int64)
+    a, b = inv[pairs[:, 0]], inv[pairs[:, 1]]
+    idx_p = torch.from_numpy(synth.condensed_index(n, pairs[:, 0], pairs[:, 1])).cuda()
+    idx_q = torch.from_numpy(synth.condensed_index(n, np.minimum(a, b), np.maximum(a, b))).cuda()
+    args_p, args_q = B.to_device(p), B.to_device(q)
+    for variant in ((0,) if name == "medium" else (0, 1)):
+        dp = B.unifrac_dm(*args_p, n, variant, B.FP32)[idx_p].double()
+        dq = B.unifrac_dm(*args_q, n, variant, B.FP32)[idx_q].double()
+        torch.cuda.synchronize()
+        err = (dp - dq).abs()
+        ok = (err <= 2e-5 * dp.abs()) | (err <= 2e-7)
+        assert bool(ok.all()), f"{name} variant {variant}: max rel diff {float((err / dp.abs().clamp_min(1e-30)).max()):.3e}"
+        print(f"{name} variant {variant}: permuted run max rel diff {float((err / dp.abs().clamp_min(1e-30)).max()):.3e}")
