@@ -23,8 +23,8 @@
 namespace ufb {
 
 template <typename T> struct DenseCfg;
-template <> struct DenseCfg<float>  { static constexpr int BK = 32, STAGES = 4, FLUSH_STAGES = 16; };
-template <> struct DenseCfg<double> { static constexpr int BK = 16, STAGES = 4, FLUSH_STAGES = 1 << 30; };
+template <> struct DenseCfg<float>  { static constexpr int BK = 32, STAGES = 4, FLUSH_STAGES = 16, LAST_EVERY_STAGE = 8; };
+template <> struct DenseCfg<double> { static constexpr int BK = 16, STAGES = 4, FLUSH_STAGES = 1 << 30, LAST_EVERY_STAGE = 0; };
 
 constexpr int DENSE_THREADS = 288;       // 8 consumer warps + 1 producer warp
 
@@ -167,7 +167,9 @@ k_dense(const __grid_constant__ CUtensorMap tmE, const DenseParams P)
             __syncwarp();
             if (lane == 0) mbar_arrive(empty(stage));
             if (++stage == STAGES) { stage = 0; phase ^= 1u; }
-            if (++since_flush >= Cfg::FLUSH_STAGES && kb + 1 < n_k) {
+            // the last LAST_EVERY_STAGE stages hold the branches with the largest n_v (rows are in ascending n_v order):
+            // their values are orders of magnitude above the rest and are folded after every stage
+            if ((++since_flush >= Cfg::FLUSH_STAGES || kb + Cfg::LAST_EVERY_STAGE + 1 >= n_k) && kb + 1 < n_k) {
                 // blocked summation: fold the fp32 partial sums into fp64 (per-thread slots, L2-resident)
 #pragma unroll
                 for (int a = 0; a < 8; ++a)

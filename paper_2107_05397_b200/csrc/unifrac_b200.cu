@@ -18,6 +18,7 @@
 #include <string>
 #include <type_traits>
 #include <vector>
+#include <algorithm>
 
 using namespace ufb;
 
@@ -348,6 +349,19 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         if (head_rows > 0) {
             hrows = A.get_n<int32_t>(head_rows);
             k_head_rows<<<cdiv(n, TB), TB, 0, st>>>(n, cls, hrank, hrows); CU_LAUNCH(); ++launches;
+            {
+                // fp32 accuracy: K order = ascending n_v (stable), so the few root-adjacent branches whose u~ is O(0.1) for every
+                // sample come last and are folded into fp64 stage by stage (k_dense) instead of swamping the fp32 partial
+                // sums that the thousands of small terms are added to
+                std::vector<int32_t> h_rows(head_rows);
+                std::vector<uint32_t> h_nv(n);
+                CU(cudaMemcpyAsync(h_rows.data(), hrows, sizeof(int32_t) * head_rows, cudaMemcpyDeviceToHost, st));
+                CU(cudaMemcpyAsync(h_nv.data(), nv, sizeof(uint32_t) * n, cudaMemcpyDeviceToHost, st));
+                CU(cudaStreamSynchronize(st));
+                std::stable_sort(h_rows.begin(), h_rows.end(), [&](int32_t a, int32_t b) { return h_nv[a] < h_nv[b]; });
+                CU(cudaMemcpyAsync(hrows, h_rows.data(), sizeof(int32_t) * head_rows, cudaMemcpyHostToDevice, st));
+                CU(cudaStreamSynchronize(st));
+            }
             uint32_t* hpref = nullptr;
             if (weighted) {
                 hpref = A.get_n<uint32_t>((size_t)head_rows * n_tiles);
