@@ -136,6 +136,9 @@ def main():
     ap.add_argument("--cpu-budget-s", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--mantel-perms", type=int, default=9,
+                    help="after the timed region: Mantel / Pearson test between the unweighted and the weighted matrix with this "
+                         "many permutations (0 = skip); reported under \"mantel\", not part of the step")
     ap.add_argument("--shard", action="store_true",
                     help="N > 1: the ranks compute disjoint shards of ONE matrix (unifrac_dm_shard, strong scaling) "
                          "instead of independent replicas (default, weak scaling)")
@@ -217,6 +220,24 @@ def main():
         upd_local /= world               # the ranks share one matrix: its updates are counted once
     ms, upd_all = reduce_over_ranks(e0.elapsed_time(e1), upd_local, world, dev)
     value = upd_all / (ms * 1e-3)
+
+    # ---------------- next row: Mantel / Pearson between the two variants' matrices, still resident in HBM
+    mantel = None
+    if len(variants) == 2 and a.mantel_perms > 0 and not shard:
+        g = torch.Generator(device=dev).manual_seed(a.seed)
+        perms = torch.stack([torch.randperm(p.n_samples, device=dev, generator=g) for _ in range(a.mantel_perms)]).to(torch.int32).contiguous()
+        binding.unifrac_mantel_pearson(outs[variants[0]], outs[variants[1]], p.n_samples, perms)      # warm-up
+        barrier()
+        m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        m0.record()
+        mo = binding.unifrac_mantel_pearson(outs[variants[0]], outs[variants[1]], p.n_samples, perms)
+        m1.record()
+        barrier()
+        m_ms = m0.elapsed_time(m1)
+        alg = (a.mantel_perms + 1) * 2.0 * p.n_pairs * 4            # both condensed matrices once per (permuted) statistic
+        mantel = dict(n_samples=p.n_samples, permutations=a.mantel_perms, ms=m_ms, ms_per_permutation=m_ms / (a.mantel_perms + 1),
+                      r=float(mo[0]), p_two_sided=float(mo[1]), algorithmic_gbs=alg / m_ms / 1e6)
+        del perms, mo
 
     # ---------------- end to end through the host-buffer C-ABI call (H2D + D2H inside the timed region)
     e2e = None
@@ -357,6 +378,11 @@ def main():
                             l2="inputs larger than L2 (compact embedding >> 126 MB)"),
                 clocks=summarize_clocks(lines), e2e=e2e, gpu_launches=int(sum(s["kernel_launches"] for s in flat)),
                 roofline=roofline, cpu_baseline=cpu, wall=per_variant)
+    if mantel:
+        hbm = peaks.get("hbm_gbs", 6550.0)
+        mantel.update(bound="hbm", peak_gbs=hbm, frac=mantel["algorithmic_gbs"] / hbm,
+                      note="algorithmic bytes = 2 x N(N-1)/2 x 4 B per statistic; the kernel moves ~1.5x that (full rows of the square copy)")
+        line["mantel"] = mantel
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -178,6 +178,21 @@ typedef struct {
 } unifrac_stats_t;
 int unifrac_last_stats(unifrac_stats_t *out);
 
+/*
+ * unifrac_mantel_pearson -- Mantel test with Pearson's correlation between two distance matrices that are already resident
+ * in HBM (the test itself is the standard one).  x, y: condensed upper triangles (the
+ * layout unifrac_dm writes) of two symmetric hollow n x n matrices; perms: n_perms permutations of 0..n-1, row-major
+ * [n_perms][n], supplied by the caller (the library draws no random numbers).  With X^pi[i][j] = X[pi(i)][pi(j)]:
+ *     out[0] = r = Pearson(x, y);   out[4 + k] = r_k = Pearson(condensed(X^pi_k), y),  k = 0 .. n_perms-1
+ *     out[1], out[2], out[3] = p-values (count + 1) / (n_perms + 1) with count = #{|r_k| >= |r|}, #{r_k >= r}, #{r_k <= r}
+ * All pointers are DEVICE pointers; out has 4 + n_perms doubles; precision selects float / double inputs; sums are fp64.
+ * Workspace (the square copy of X, n*n elements) comes from `alloc` (NULL: cudaMallocAsync).  A constant matrix (zero variance)
+ * gives r = 0.  n < 3: UNIFRAC_ERR_INVALID_ARG.  Permutations are not validated.  Asynchronous on `stream`.
+ */
+int unifrac_mantel_pearson(int32_t n_samples, const void *x_condensed, const void *y_condensed,
+                           unifrac_precision_t precision, const int32_t *perms, int32_t n_perms, double *out,
+                           unifrac_alloc_fn alloc, void *alloc_user, void *stream);
+
 /* Device-rate probes (not on the data path): what this GPU retires per second of the two atomic units of work the
  * sparse kernels are made of; they are the constants of the head / mid / tail cost model and the `peak` of the
  * k_mid / k_tail_scatter rooflines in bench.py.  Runs ~20 ms of probe kernels on `stream` and synchronises it. */

@@ -23,7 +23,7 @@ OK = 0
 ERR_INVALID_ARG, ERR_INVALID_TREE, ERR_INVALID_TABLE, ERR_EMPTY_SAMPLE = -1, -2, -3, -4
 ERR_WORKSPACE, ERR_CUDA, ERR_UNSUPPORTED = -5, -6, -7
 
-EXPORTS = ("unifrac_dm", "unifrac_dm_shard", "unifrac_shard_of_pair", "unifrac_dm_host", "unifrac_measure_rates", "unifrac_last_stats", "unifrac_status_string",
+EXPORTS = ("unifrac_dm", "unifrac_dm_shard", "unifrac_shard_of_pair", "unifrac_dm_host", "unifrac_mantel_pearson", "unifrac_measure_rates", "unifrac_last_stats", "unifrac_status_string",
            "unifrac_last_cuda_error", "unifrac_abi_version")
 
 
@@ -86,6 +86,9 @@ def load(build_if_missing: bool = True) -> C.CDLL:
     lib.unifrac_dm_host.restype = C.c_int
     lib.unifrac_dm_host.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, CSR, C.c_int32, C.c_int, C.c_int,
                                     C.c_void_p, C.c_uint32]
+    lib.unifrac_mantel_pearson.restype = C.c_int
+    lib.unifrac_mantel_pearson.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_int32, C.c_void_p,
+                                           ALLOC_FN, C.c_void_p, C.c_void_p]
     lib.unifrac_measure_rates.restype = C.c_int
     lib.unifrac_measure_rates.argtypes = [C.POINTER(Rates), C.c_void_p]
     lib.unifrac_last_stats.restype = C.c_int
@@ -171,6 +174,42 @@ def unifrac_last_stats() -> dict:
     s = Stats()
     _check(lib, lib.unifrac_last_stats(C.byref(s)))
     return {k: getattr(s, k) for k, _ in Stats._fields_}
+
+
+def unifrac_mantel_pearson(x_condensed, y_condensed, n_samples: int, perms, stream=None):
+    """Mantel test (Pearson) on two condensed CUDA tensors (both float32 or both float64); perms: CUDA int32 [K, n].
+    Returns a CUDA float64 tensor [4 + K]: r, p two-sided, p greater, p less, r_1 .. r_K.  Asynchronous on the stream."""
+    import torch
+    lib = load()
+    dev = x_condensed.device
+    n = int(n_samples)
+    assert dev.type == "cuda" and y_condensed.device == dev and perms.device == dev
+    assert x_condensed.dtype == y_condensed.dtype and x_condensed.dtype in (torch.float32, torch.float64)
+    assert x_condensed.is_contiguous() and y_condensed.is_contiguous() and perms.is_contiguous() and perms.dtype == torch.int32
+    assert x_condensed.numel() == n * (n - 1) // 2 == y_condensed.numel()
+    K = int(perms.numel() // n) if perms.numel() else 0
+    out = torch.empty(4 + K, dtype=torch.float64, device=dev)
+    held = []
+
+    def _alloc(nbytes, _user):
+        try:
+            t = torch.empty(int(nbytes), dtype=torch.uint8, device=dev)
+        except Exception:
+            return None
+        held.append(t)
+        return t.data_ptr()
+
+    cb = ALLOC_FN(_alloc)
+    with torch.cuda.device(dev):
+        s = stream if stream is not None else torch.cuda.current_stream(dev)
+        with torch.cuda.stream(s):
+            rc = lib.unifrac_mantel_pearson(n, x_condensed.data_ptr(), y_condensed.data_ptr(),
+                                            FP32 if x_condensed.dtype == torch.float32 else FP64,
+                                            perms.data_ptr() if K else None, K, out.data_ptr(), cb, None,
+                                            C.c_void_p(s.cuda_stream))
+    del held
+    _check(lib, rc)
+    return out
 
 
 def unifrac_measure_rates(stream=None) -> dict:

@@ -11,6 +11,7 @@
 #include "mid.cuh"
 #include "dense.cuh"
 #include "rates.cuh"
+#include "mantel.cuh"
 
 #include <cstdio>
 #include <cstdlib>
@@ -654,6 +655,40 @@ int guarded(int32_t n_nodes, const int32_t* parent, const double* len, const int
     return rc;
 }
 
+template <typename T>
+void run_mantel(int32_t N, const T* x, const T* y, const int32_t* perms, int32_t K, double* out, Arena& A, cudaStream_t st)
+{
+    const unsigned long long P = (unsigned long long)N * (N - 1) / 2;
+    double* mom = A.get_n<double>(8);
+    double* S = A.get_n<double>((size_t)K + 1);
+    const long long pitch = ((long long)N + 3) & ~3ll;                      // rows start 16-byte aligned (bulk copies)
+    T* Xs = A.get_n<T>((size_t)N * pitch);
+    CU(cudaMemsetAsync(mom, 0, sizeof(double) * 8, st));
+    CU(cudaMemsetAsync(S, 0, sizeof(double) * ((size_t)K + 1), st));
+    CU(cudaMemsetAsync(Xs, 0, sizeof(T) * (size_t)N * pitch, st));         // pitch padding
+    int dev = 0, n_sm = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    k_mantel_moments<T><<<n_sm * 8, 256, 0, st>>>(x, y, P, mom); CU_LAUNCH();
+    const unsigned nb = (unsigned)cdiv(N, 32);
+    k_mantel_square<T><<<dim3(nb, nb), dim3(32, 8), 0, st>>>(x, N, pitch, Xs); CU_LAUNCH();
+    // two ring buffers of one column segment each: as few segments as fit in ~208 KB
+    const size_t budget = (size_t)208 * 1024 / 2 / sizeof(T);              // elements per buffer
+    const int n_split = cdiv(pitch, (long long)budget);
+    const int seg = (int)(((pitch + n_split - 1) / n_split + 3) & ~3ll);
+    const size_t smem = 2 * (size_t)seg * sizeof(T);
+    CU(cudaFuncSetAttribute(k_mantel_perm<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    for (int k0 = 0; k0 <= K; k0 += 65535) {                              // grid.y limit
+        const int kn = std::min(65535, K + 1 - k0);
+        int G = std::max(8, cdiv(2 * n_sm, kn));                           // row-strided CTAs per permutation
+        if (G > N - 1) G = N - 1;
+        k_mantel_perm<T><<<dim3((unsigned)G, (unsigned)kn), MANTEL_THREADS, smem, st>>>(
+            Xs, pitch, y, perms, N, seg, n_split, k0, S);
+        CU_LAUNCH();
+    }
+    k_mantel_final<<<1, 256, 0, st>>>(mom, S, K, (double)P, out); CU_LAUNCH();
+    A.release();
+}
 }  // namespace
 
 extern "C" {
@@ -746,6 +781,28 @@ int unifrac_last_stats(unifrac_stats_t* out)
     }
     *out = g_stats;
     return UNIFRAC_OK;
+}
+
+int unifrac_mantel_pearson(int32_t N, const void* x, const void* y, unifrac_precision_t precision, const int32_t* perms,
+                           int32_t K, double* out, unifrac_alloc_fn alloc, void* user, void* stream)
+{
+    if (!x || !y || !out || K < 0 || (K > 0 && !perms) || N < 3) return UNIFRAC_ERR_INVALID_ARG;
+    if (precision != UNIFRAC_FP32 && precision != UNIFRAC_FP64) return UNIFRAC_ERR_INVALID_ARG;
+    if ((long long)N > (1ll << 23)) return UNIFRAC_ERR_UNSUPPORTED;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    Arena A{alloc, user, st};
+    int rc = UNIFRAC_OK;
+    try {
+        if (precision == UNIFRAC_FP32) run_mantel<float>(N, reinterpret_cast<const float*>(x), reinterpret_cast<const float*>(y), perms, K, out, A, st);
+        else run_mantel<double>(N, reinterpret_cast<const double*>(x), reinterpret_cast<const double*>(y), perms, K, out, A, st);
+    } catch (const CudaFail& f) {
+        char b[512];
+        snprintf(b, sizeof(b), "%s: %s (unifrac_b200.cu:%d)", f.what, cudaGetErrorString(f.e), f.line);
+        g_cuda_err = b; cudaGetLastError(); rc = UNIFRAC_ERR_CUDA;
+    } catch (const WorkspaceFail&) { rc = UNIFRAC_ERR_WORKSPACE; }
+    catch (...) { rc = UNIFRAC_ERR_CUDA; g_cuda_err = "unexpected C++ exception"; }
+    if (rc != UNIFRAC_OK) A.release();
+    return rc;
 }
 
 int unifrac_measure_rates(unifrac_rates_t* out, void* stream)

@@ -266,3 +266,17 @@ def test_shards_partition_the_matrix(B, O, variant, precision):
     assert np.allclose(a, b, rtol=2e-6 if precision == 0 else 1e-12, atol=1e-7 if precision == 0 else 1e-13)
     with pytest.raises(B.UnifracError):
         B.unifrac_dm(*args, n, variant, precision, shard=(4, 4))
+
+
+@pytest.mark.parametrize("seed", [1, 2])
+@pytest.mark.parametrize("variant", [U, W])
+def test_other_seeds_six_tiles_all_pairs_fp32_and_fp64(B, O, variant, seed):
+    """DESIGN.md reading Q16: seeds 1 and 2 as extra parity runs.  700 samples = 6 tiles (ragged last one), 8,000 tips:
+    all 244,650 pairs against the oracle's all-pairs driver, default split (head + mid + tail all non-empty in fp32)."""
+    cfg = synth.CONFIGS["small"]
+    p = synth.make_problem(8000, 700, 0.05, 1.05, cfg[4], cfg[5], seed=seed)
+    want = O.all_pairs(p.parent, p.branch_len, p.indptr, p.indices, p.counts, variant)
+    check(gpu_dm(B, p, variant, 1), want, 1)
+    check(gpu_dm(B, p, variant, 0), want, 0)
+    st = B.unifrac_last_stats()
+    assert st["head_rows"] > 0 and st["tail_rows"] > 0
