@@ -680,8 +680,14 @@ void run_mantel(int32_t N, const T* x, const T* y, const int32_t* perms, int32_t
     CU(cudaFuncSetAttribute(k_mantel_perm<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     for (int k0 = 0; k0 <= K; k0 += 65535) {                              // grid.y limit
         const int kn = std::min(65535, K + 1 - k0);
-        int G = std::max(8, cdiv(2 * n_sm, kn));                           // row-strided CTAs per permutation
-        if (G > N - 1) G = N - 1;
+        // row-strided CTAs per permutation: G * kn CTAs (one per SM at a time) should fill whole waves of n_sm
+        int G = 1; double best = 0.0;
+        for (int m = 1; m <= 8; ++m) {
+            const int g = std::min<long long>(N - 1, (long long)n_sm * m / kn);
+            if (g < 1) continue;
+            const double fill = (double)g * kn / ((double)n_sm * cdiv((long long)g * kn, n_sm));
+            if (fill > best + 1e-9) { best = fill; G = g; }
+        }
         k_mantel_perm<T><<<dim3((unsigned)G, (unsigned)kn), MANTEL_THREADS, smem, st>>>(
             Xs, pitch, y, perms, N, seg, n_split, k0, S);
         CU_LAUNCH();
