@@ -280,3 +280,12 @@ def test_other_seeds_six_tiles_all_pairs_fp32_and_fp64(B, O, variant, seed):
     check(gpu_dm(B, p, variant, 0), want, 0)
     st = B.unifrac_last_stats()
     assert st["head_rows"] > 0 and st["tail_rows"] > 0
+
+
+def test_measure_rates_probe(B):
+    """unifrac_measure_rates (the peaks of the k_mid / k_tail_scatter rooflines): positive, plausible, repeatable to 10 %."""
+    a, b = B.unifrac_measure_rates(), B.unifrac_measure_rates()
+    for k in ("smem_atomic_conflict_free_per_s", "smem_atomic_random_per_s", "l2_red_random_per_s"):
+        assert a[k] > 1e10 and abs(a[k] - b[k]) <= 0.1 * a[k]
+    assert a["sm_count"] > 0 and a["sm_clock_khz"] > 0
+    assert a["smem_atomic_random_per_s"] <= a["sm_count"] * a["sm_clock_khz"] * 1e3 * 32     # at most one full wavefront per clock
