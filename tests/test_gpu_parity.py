@@ -289,3 +289,22 @@ def test_measure_rates_probe(B):
         assert a[k] > 1e10 and abs(a[k] - b[k]) <= 0.1 * a[k]
     assert a["sm_count"] > 0 and a["sm_clock_khz"] > 0
     assert a["smem_atomic_random_per_s"] <= a["sm_count"] * a["sm_clock_khz"] * 1e3 * 32     # at most one full wavefront per clock
+
+
+@pytest.mark.parametrize("case", range(8))
+def test_randomized_shapes_all_pairs(B, O, case):
+    """Seeded random shapes (tips 50..6000, samples 2..900, the count / richness recipes, branch-length scale and Zipf
+    exponent varied): all pairs, both variants, fp32 and fp64, default split and head + tail only."""
+    rng = np.random.default_rng(1000 + case)
+    n_tips = int(rng.integers(50, 6000))
+    n = int(rng.integers(2, 900))
+    # the richer recipes need enough tips (the generator draws features until k of them are distinct)
+    names = ["tiny"] if n_tips < 500 else ["tiny", "small"] if n_tips < 3000 else ["tiny", "small", "medium"]
+    cfg = synth.CONFIGS[names[int(rng.integers(0, len(names)))]]
+    p = synth.make_problem(n_tips, n, float(rng.choice([0.05, 0.1, 1.0])), float(rng.choice([1.05, 1.1, 1.3])), cfg[4], cfg[5],
+                           seed=int(rng.integers(0, 10**6)))
+    for variant in (U, W):
+        want = O.all_pairs(p.parent, p.branch_len, p.indptr, p.indices, p.counts, variant)
+        for precision in (0, 1):
+            for flags in (0, 128):
+                check(gpu_dm(B, p, variant, precision, flags), want, precision)
