@@ -298,7 +298,8 @@ def main():
                        kernel=kname, launches=nl, ms_per_launch=1e3 * t / max(1, nl),
                        executed_updates_per_launch=w_exec / max(1, nl), seconds=t, share_of_step=t / step_s,
                        peak_source=f"{SM_COUNT} SMs x {FP32_LANES} FP32 lanes x {SM_MAX_GHZ} GHz (sm_max_mhz of MEASURED_PEAKS.json, {src}); "
-                                   "2 FP32-pipe lane-ops (FMNMX+FADD) per (pair, branch) update"))
+                                   "2 FP32-pipe lane-ops (FMNMX+FADD) per (pair, branch) update",
+                       measured_fmnmx_fadd_tflops=rates.get("fmnmx_fadd_per_s", 0.0) / 1e12 or None))
     # (2) k_gram: tcgen05 kind::i8 Gram kernel (head branches, unweighted fp32): 3 u8 digit MACs per update
     gs = [s for s in flat if s["gram"]]
     if gs:

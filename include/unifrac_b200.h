@@ -200,6 +200,9 @@ typedef struct {
     double smem_atomic_conflict_free_per_s;  /* shared-memory u32 atomic adds, 32 lanes on 32 different banks        */
     double smem_atomic_random_per_s;         /* ... on pseudo-random cells of a 128 x 128 tile (k_mid's access pattern) */
     double l2_red_random_per_s;              /* fp32 RED.ADD on pseudo-random words of a 48 MB (L2-resident) footprint */
+    double fmnmx_per_s;                      /* FP32 min lane-ops (the half-rate ALU pipe), register chains            */
+    double fadd_per_s;                       /* FP32 add lane-ops (the FMA pipe)                                      */
+    double fmnmx_fadd_per_s;                 /* lane-ops of interleaved min + add pairs (one k_dense update = 2)       */
     int32_t sm_count;
     int32_t sm_clock_khz;                    /* cudaDevAttrClockRate                                               */
 } unifrac_rates_t;

@@ -46,7 +46,8 @@ class Stats(C.Structure):
 
 class Rates(C.Structure):
     _fields_ = [("smem_atomic_conflict_free_per_s", C.c_double), ("smem_atomic_random_per_s", C.c_double),
-                ("l2_red_random_per_s", C.c_double), ("sm_count", C.c_int32), ("sm_clock_khz", C.c_int32)]
+                ("l2_red_random_per_s", C.c_double), ("fmnmx_per_s", C.c_double), ("fadd_per_s", C.c_double),
+                ("fmnmx_fadd_per_s", C.c_double), ("sm_count", C.c_int32), ("sm_clock_khz", C.c_int32)]
 
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)

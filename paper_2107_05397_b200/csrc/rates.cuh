@@ -52,4 +52,31 @@ k_rate_red(float* __restrict__ buf, uint32_t cells, int iters)
     }
 }
 
+// FP32-pipe probes behind the `"bound": "alu"` roofline of k_dense: 8 independent register chains per thread of
+// mode 0: FMNMX (min.f32, the half-rate ALU pipe);  1: FADD (the FMA pipe);  2: FMNMX + FADD pairs (k_dense's update)
+template <int mode>
+__global__ void __launch_bounds__(256)
+k_rate_alu(int iters, float* __restrict__ sink)
+{
+    float a[8], b[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) { a[k] = 1.0f + threadIdx.x * 1e-3f + k; b[k] = 0.5f + k * 1e-2f + blockIdx.x * 1e-6f; }
+#pragma unroll 4
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            if (mode == 0) {                                    // min / max alternate so that the chain is not idempotent
+                if (it & 1) asm volatile("min.f32 %0, %0, %1;" : "+f"(a[k]) : "f"(b[k]));
+                else        asm volatile("max.f32 %0, %0, %1;" : "+f"(a[k]) : "f"(b[(k + 1) & 7]));
+            }
+            else if (mode == 1) asm volatile("add.f32 %0, %0, %1;" : "+f"(a[k]) : "f"(b[k]));
+            else { float m; asm volatile("min.f32 %0, %1, %2;" : "=f"(m) : "f"(a[k]), "f"(b[k])); asm volatile("add.f32 %0, %0, %1;" : "+f"(b[k]) : "f"(m)); }
+        }
+    }
+    float t = 0.f;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) t += a[k] + b[k];
+    if (t == 12345.678f) sink[0] = t;
+}
+
 }  // namespace ufb

@@ -848,6 +848,15 @@ int unifrac_measure_rates(unifrac_rates_t* out, void* stream)
         out->smem_atomic_conflict_free_per_s = (double)ga * 512 * it_a * 8 / t0;
         out->smem_atomic_random_per_s = (double)ga * 512 * it_a * 8 / t1;
         out->l2_red_random_per_s = (double)gr * 256 * it_r * 4 / t2;
+        const int it_f = 8192;
+        const unsigned gf = (unsigned)n_sm * 8;
+        float* fsink = buf;
+        double t3 = timed([&] { k_rate_alu<0><<<gf, 256, 0, st>>>(it_f, fsink); CU_LAUNCH(); });
+        double t4 = timed([&] { k_rate_alu<1><<<gf, 256, 0, st>>>(it_f, fsink); CU_LAUNCH(); });
+        double t5 = timed([&] { k_rate_alu<2><<<gf, 256, 0, st>>>(it_f, fsink); CU_LAUNCH(); });
+        out->fmnmx_per_s = (double)gf * 256 * it_f * 8 / t3;
+        out->fadd_per_s = (double)gf * 256 * it_f * 8 / t4;
+        out->fmnmx_fadd_per_s = (double)gf * 256 * it_f * 16 / t5;
         out->sm_count = n_sm; out->sm_clock_khz = khz;
     } catch (const CudaFail& f) {
         char b[512];
