@@ -218,4 +218,131 @@ k_dense(const __grid_constant__ CUtensorMap tmE, const DenseParams P)
     }
 }
 
+// ------------------------------------------------------------------ fp32 variant with 16 consumer warps
+// Same pipeline and arithmetic as k_dense<float>, but the 128 x 128 tile pair is owned by 16 consumer warps (4 x 4 grid of
+// 32 x 32 sub-tiles, an 8 x 4 register tile per thread: 3 LDS.128 per 32 updates instead of 4 per 64) so that every
+// scheduler has four warps to pick from while FMNMX occupies the half-rate ALU pipe.
+constexpr int DENSE16_THREADS = 544;     // 16 consumer warps + 1 producer warp
+__global__ void __launch_bounds__(DENSE16_THREADS, 1)
+k_dense16(const __grid_constant__ CUtensorMap tmE, const DenseParams P)
+{
+    using T = float;
+    using Cfg = DenseCfg<float>;
+    constexpr int BK = Cfg::BK, STAGES = Cfg::STAGES;
+    constexpr uint32_t BOX_BYTES = BK * TILE * sizeof(T);
+
+    extern __shared__ unsigned char dsm_raw[];
+    const uint32_t raw = smem_u32(dsm_raw);
+    const uint32_t base = (raw + 127u) & ~127u;
+    T* ring = reinterpret_cast<T*>(dsm_raw + (base - raw));
+    const uint32_t bar0 = base + STAGES * 2 * BOX_BYTES;
+    auto full = [&](uint32_t s) { return bar0 + 8u * s; };
+    auto empty = [&](uint32_t s) { return bar0 + 8u * (STAGES + s); };
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < STAGES; ++s) { mbar_init(full(s), 1); mbar_init(empty(s), 16); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    const uint32_t n_k = P.K_pad / BK;
+
+    if (warp == 16) {
+        if (lane == 0) {
+            uint32_t stage = 0, phase = 0;
+            for (uint32_t pi = blockIdx.x; pi < P.n_pairs; pi += gridDim.x) {
+                const int2 ij = P.pairs[pi];
+                for (uint32_t kb = 0; kb < n_k; ++kb) {
+                    mbar_wait(empty(stage), phase ^ 1u);
+                    const uint32_t dst = base + stage * 2 * BOX_BYTES;
+                    mbar_arrive_expect_tx(full(stage), 2 * BOX_BYTES);
+                    tma_load_2d_box(dst, &tmE, ij.x * TILE, (int)(kb * BK), full(stage));
+                    tma_load_2d_box(dst + BOX_BYTES, &tmE, ij.y * TILE, (int)(kb * BK), full(stage));
+                    if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                }
+            }
+        }
+        return;
+    }
+
+    const int wi = warp >> 2, wj = warp & 3;
+    const int ty = lane >> 3, tx = lane & 7;
+    // i side: element a at local row (a/4)*16 + ty*4 + a%4 of the warp's 32 rows; j side: element b at column tx*4 + b of its 32
+    const int i_off = wi * 32 + ty * 4;
+    const int j_off = BK * TILE + wj * 32 + tx * 4;
+    double* my_scratch = P.scratch + (size_t)blockIdx.x * 64 * 256 + threadIdx.x;      // [32][512] per CTA
+
+    float acc[8][4];
+#pragma unroll
+    for (int a = 0; a < 8; ++a)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) acc[a][b] = 0.f;
+    uint32_t stage = 0, phase = 0;
+
+    for (uint32_t pi = blockIdx.x; pi < P.n_pairs; pi += gridDim.x) {
+        int since_flush = 0;
+        bool scratch_live = false;
+        for (uint32_t kb = 0; kb < n_k; ++kb) {
+            mbar_wait(full(stage), phase);
+            const float* sb = ring + (size_t)stage * 2 * BK * TILE;
+#pragma unroll 4
+            for (int r = 0; r < BK; ++r) {
+                const float* row = sb + r * TILE;
+                float ai[8], bj[4];
+                VecLd<float>::ld(row + i_off, ai);
+                VecLd<float>::ld(row + i_off + 16, ai + 4);
+                VecLd<float>::ld(row + j_off, bj);
+#pragma unroll
+                for (int a = 0; a < 8; ++a)
+#pragma unroll
+                    for (int b = 0; b < 4; ++b) acc[a][b] += fminf(ai[a], bj[b]);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty(stage));
+            if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+            if ((++since_flush >= Cfg::FLUSH_STAGES || kb + Cfg::LAST_EVERY_STAGE + 1 >= n_k) && kb + 1 < n_k) {
+#pragma unroll
+                for (int a = 0; a < 8; ++a)
+#pragma unroll
+                    for (int b = 0; b < 4; ++b) {
+                        double* s = my_scratch + (size_t)(a * 4 + b) * 512;
+                        double v = (double)acc[a][b];
+                        if (scratch_live) v += *s;
+                        *s = v;
+                        acc[a][b] = 0.f;
+                    }
+                scratch_live = true;
+                since_flush = 0;
+            }
+        }
+        // ----------------------------------------------------------- a-6 finalize (epilogue of the tile pair)
+        const int2 ij = P.pairs[pi];
+        const long long N = P.n_samples;
+        double sj[4];
+#pragma unroll
+        for (int b = 0; b < 4; ++b) sj[b] = P.sums[ij.y * TILE + wj * 32 + tx * 4 + b];
+#pragma unroll
+        for (int a = 0; a < 8; ++a) {
+            const long long gi = (long long)ij.x * TILE + wi * 32 + (a / 4) * 16 + ty * 4 + (a % 4);
+            const double si = P.sums[gi];
+            const long long rowbase = gi * (2 * N - gi - 1) / 2 - gi - 1;
+#pragma unroll
+            for (int b = 0; b < 4; ++b) {
+                double tot = (double)acc[a][b];
+                if (scratch_live) tot += my_scratch[(size_t)(a * 4 + b) * 512];
+                acc[a][b] = 0.f;
+                const long long gj = (long long)ij.y * TILE + wj * 32 + tx * 4 + b;
+                if (gi < gj && gj < N) {
+                    const double ss = si + sj[b];
+                    if (P.add_out) tot += (double)reinterpret_cast<const float*>(P.out)[rowbase + gj];
+                    double num = ss - 2.0 * tot;
+                    const double den = P.weighted ? ss : ss - tot;
+                    if (num < 0.0) num = 0.0;
+                    reinterpret_cast<float*>(P.out)[rowbase + gj] = (float)(den > 0.0 ? num / den : 0.0);
+                }
+            }
+        }
+    }
+}
+
 }  // namespace ufb

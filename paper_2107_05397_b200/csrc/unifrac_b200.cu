@@ -552,10 +552,15 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         D.pairs = pairs; D.n_pairs = n_pairs; D.K_pad = Kd_pad; D.sums = sums; D.n_samples = N; D.weighted = weighted; D.out = out;
         D.add_out = (tail_rows || mid_rows) ? 1 : 0;
         const size_t smem = dense_smem_bytes<T>();
-        CU(cudaFuncSetAttribute(k_dense<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         unsigned grid = (unsigned)std::min<long long>(n_sm, n_pairs);
         D.scratch = A.get_n<double>((size_t)grid * 64 * 256);
-        if (grid) { k_dense<T><<<grid, DENSE_THREADS, smem, st>>>(tmE, D); CU_LAUNCH(); ++launches; ++stripe_launches; }
+        if (f32 && envd("UNIFRAC_B200_DENSE16", 1) != 0) {       // fp32: 16 consumer warps
+            CU(cudaFuncSetAttribute(k_dense16, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            if (grid) { k_dense16<<<grid, DENSE16_THREADS, smem, st>>>(tmE, D); CU_LAUNCH(); ++launches; ++stripe_launches; }
+        } else {
+            CU(cudaFuncSetAttribute(k_dense<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            if (grid) { k_dense<T><<<grid, DENSE_THREADS, smem, st>>>(tmE, D); CU_LAUNCH(); ++launches; ++stripe_launches; }
+        }
         CU(cudaStreamSynchronize(st));           // h_pairs staging copy done before it goes out of scope
     } else {
     std::vector<int2> h_pairs;
