@@ -38,7 +38,7 @@ SMEM_ATOMIC_PER_S, L2_RED_PER_S = 8.84 * SM_COUNT * SM_MAX_GHZ * 1e9, 1.94e11
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full captures of profiles/r01_summary.md
 # (default flags, seed 0; k_mid: mean of the unweighted and the weighted launch); other workloads: null
-NCU_TRAFFIC_BYTES = {"large": {"k_dense": 237.7e9, "k_gram": 300.1e9, "k_mid": 240.2e9, "k_tail_scatter": 0.227e9}}
+NCU_TRAFFIC_BYTES = {"large": {"k_dense16": 308.4e9, "k_gram": 300.1e9, "k_mid": 240.2e9, "k_tail_scatter": 0.227e9}}
 
 WORKLOADS = {   # name -> (variants, precision)    BASELINE.json:7-11
     "tiny": ((0, 1), 1), "small": ((0, 1), 1), "medium": ((0,), 0), "emp": ((0, 1), 0), "large": ((0, 1), 0),
@@ -289,7 +289,7 @@ def main():
     # (1) k_dense (default) / k_stripe (debug forms): CUDA-core register-tile kernel (head branches; weighted, fp64, or NO_TENSOR)
     ss = [s for s in flat if not s["gram"]]
     if ss:
-        kname = "k_dense" if all(s["dense"] for s in ss) else "k_stripe"
+        kname = ("k_dense16" if precision == 0 else "k_dense") if all(s["dense"] for s in ss) else "k_stripe"
         t = sum(s["ms_stripe"] for s in ss) * 1e-3
         w_exec = sum(s["updates_executed_head"] for s in ss)
         nl = sum(s["stripe_launches"] for s in ss)
