@@ -226,6 +226,21 @@ k_tail_scatter(const TailParams P)
             const uint32_t bi0 = __shfl_sync(0xffffffffu, i0, src), bi1 = __shfl_sync(0xffffffffu, i1, src);
             const uint32_t bj0 = __shfl_sync(0xffffffffu, j0, src), bj1 = __shfl_sync(0xffffffffu, j1, src);
             const uint32_t bb = __shfl_sync(0xffffffffu, base, src);
+            if (!diag) {
+                // off-diagonal super tile: the nI x nJ products are dealt to the lanes as one flat list (product t = lane,
+                // lane + 32, ...; (i, j) advanced incrementally), so short lists still fill the warp's RED instructions
+                const uint32_t nI2 = bi1 - bi0, nJ2 = bj1 - bj0, tot = nI2 * nJ2;
+                uint32_t i = (uint32_t)lane / nJ2, j = (uint32_t)lane - i * nJ2;
+                const uint32_t di = 32u / nJ2, dj = 32u - di * nJ2;
+                for (uint32_t t = lane; t < tot; t += 32) {
+                    const long long sa = P.ts[bb + bi0 + i], sb = P.ts[bb + bj0 + j];
+                    const T va = tv[bb + bi0 + i], vb = tv[bb + bj0 + j];
+                    if (tail_owns(P, sa, sb)) red_add(out + (sa * (2 * N - sa - 1) / 2 - sa - 1) + sb, va < vb ? va : vb);
+                    i += di; j += dj;
+                    if (j >= nJ2) { j -= nJ2; ++i; }
+                }
+                continue;
+            }
             const bool lanesJ = diag || (bj1 - bj0) >= (bi1 - bi0);       // lane entries are the b's (else the a's)
             const uint32_t p0 = lanesJ ? bj0 : bi0, p1 = lanesJ ? bj1 : bi1;   // lane list
             const uint32_t q0 = lanesJ ? bi0 : bj0, q1 = lanesJ ? bi1 : bj1;   // loop list
