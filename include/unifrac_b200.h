@@ -174,6 +174,14 @@ typedef struct {
     uint32_t gram_k;             /* K (head branches, padded to 64) of that GEMM                       */
     uint32_t gram_q;             /* fixed-point scale: L_v = round(len_v * 2^q)                        */
     uint32_t dense;              /* 1 if the head branches went through the dense CUDA-core kernel (k_dense) */
+    uint32_t guard_pairs;        /* pairs with d < 1/16 that the near-duplicate guard recomputed from the definition */
+    uint32_t guard_capacity;     /* size of the guard's pair list: min(P, max(2^22, 64 N)); pairs listed beyond it keep
+                                    their separable-form value (absolute error ~1e-7 in fp32)                           */
+    uint32_t quant_fallback;     /* 1 if the fixed-point error ratio was over budget and the call was rerun without
+                                    the fixed-point kernels (tensor-core Gram, shared-memory mid)                       */
+    float guard_theta;           /* the guard's threshold of this call: max(1/16, quant_err_ratio / 2.5e-6)            */
+    float quant_err_ratio;       /* max over samples of (|sum delta| + 3 sqrt(sum delta^2)) / (side sum), delta = fixed-point
+                                    value - value over the sample's Gram-head lengths and mid entries; over 1.25e-6 => rerun */
     float ms_plan, ms_embed, ms_tail, ms_mid, ms_stripe, ms_total;
 } unifrac_stats_t;
 int unifrac_last_stats(unifrac_stats_t *out);
@@ -203,6 +211,10 @@ typedef struct {
     double fmnmx_per_s;                      /* FP32 min lane-ops (the half-rate ALU pipe), register chains            */
     double fadd_per_s;                       /* FP32 add lane-ops (the FMA pipe)                                      */
     double fmnmx_fadd_per_s;                 /* lane-ops of interleaved min + add pairs (one k_dense update = 2)       */
+    double fadd2_per_s;                      /* FP32 add lane-ops issued as packed add.f32x2 (FADD2, two per instruction) */
+    double fmnmx2_fadd2_updates_per_s;       /* (pair, branch) updates of 2 x FMNMX + 1 x FADD2 (1.5 instructions per update) */
+    double dense16_mix_updates_per_s;        /* updates of k_dense16's instruction mix (24 min cells with packed adds + 8 direct
+                                                cells with FADD + FFMA per 32)                                              */
     int32_t sm_count;
     int32_t sm_clock_khz;                    /* cudaDevAttrClockRate                                               */
 } unifrac_rates_t;
@@ -210,7 +222,7 @@ int unifrac_measure_rates(unifrac_rates_t *out, void *stream);
 
 const char *unifrac_status_string(int status);
 const char *unifrac_last_cuda_error(void);   /* text of the last CUDA error seen by this thread  */
-int unifrac_abi_version(void);               /* 4                                                */
+int unifrac_abi_version(void);               /* 5                                                */
 
 #ifdef __cplusplus
 }

@@ -19,6 +19,7 @@ FP32, FP64 = 0, 1
 FLAG_LITERAL, FLAG_TENSOR_GRAM, FLAG_SKIP_VALIDATION, FLAG_ABSDIFF = 1, 2, 4, 8
 FLAG_NO_TAIL, FLAG_ALL_TAIL, FLAG_NO_TENSOR, FLAG_NO_MID, FLAG_SPARSE_STRIPE = 16, 32, 64, 128, 256
 
+ABI_VERSION = 5          # unifrac_abi_version() of the header this binding was written against
 OK = 0
 ERR_INVALID_ARG, ERR_INVALID_TREE, ERR_INVALID_TABLE, ERR_EMPTY_SAMPLE = -1, -2, -3, -4
 ERR_WORKSPACE, ERR_CUDA, ERR_UNSUPPORTED = -5, -6, -7
@@ -39,7 +40,7 @@ class Stats(C.Structure):
                 ("rows_staged", C.c_uint64),
                 ("embed_rows", C.c_uint64), ("workspace_bytes", C.c_uint64), ("n_tile_pairs", C.c_uint32),
                 ("n_levels", C.c_uint32), ("stripe_launches", C.c_uint32), ("tail_launches", C.c_uint32),
-                ("kernel_launches", C.c_uint32), ("mid_launches", C.c_uint32), ("mid_F", C.c_uint32), ("gram", C.c_uint32), ("gram_k", C.c_uint32), ("gram_q", C.c_uint32), ("dense", C.c_uint32),
+                ("kernel_launches", C.c_uint32), ("mid_launches", C.c_uint32), ("mid_F", C.c_uint32), ("gram", C.c_uint32), ("gram_k", C.c_uint32), ("gram_q", C.c_uint32), ("dense", C.c_uint32), ("guard_pairs", C.c_uint32), ("guard_capacity", C.c_uint32), ("quant_fallback", C.c_uint32), ("guard_theta", C.c_float), ("quant_err_ratio", C.c_float),
                 ("ms_plan", C.c_float), ("ms_embed", C.c_float), ("ms_tail", C.c_float), ("ms_mid", C.c_float), ("ms_stripe", C.c_float),
                 ("ms_total", C.c_float)]
 
@@ -47,7 +48,8 @@ class Stats(C.Structure):
 class Rates(C.Structure):
     _fields_ = [("smem_atomic_conflict_free_per_s", C.c_double), ("smem_atomic_random_per_s", C.c_double),
                 ("l2_red_random_per_s", C.c_double), ("fmnmx_per_s", C.c_double), ("fadd_per_s", C.c_double),
-                ("fmnmx_fadd_per_s", C.c_double), ("sm_count", C.c_int32), ("sm_clock_khz", C.c_int32)]
+                ("fmnmx_fadd_per_s", C.c_double), ("fadd2_per_s", C.c_double), ("fmnmx2_fadd2_updates_per_s", C.c_double),
+                ("dense16_mix_updates_per_s", C.c_double), ("sm_count", C.c_int32), ("sm_clock_khz", C.c_int32)]
 
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
@@ -71,12 +73,12 @@ def load(build_if_missing: bool = True) -> C.CDLL:
     if not os.path.exists(path) or (build_if_missing and _build.needs_build()):
         if not build_if_missing:
             raise FileNotFoundError(path)
-        try:
-            _build.build()
-        except Exception:
-            if not os.path.exists(path):
-                raise
+        _build.build()              # a failed rebuild raises: a stale library is never loaded in its place
     lib = C.CDLL(path)
+    lib.unifrac_abi_version.restype = C.c_int
+    if lib.unifrac_abi_version() != ABI_VERSION:
+        raise RuntimeError(f"{path}: ABI version {lib.unifrac_abi_version()} != {ABI_VERSION} (stale build; the Stats / "
+                           f"Rates layouts of this binding would not match)")
     lib.unifrac_dm.restype = C.c_int
     lib.unifrac_dm.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, CSR, C.c_int32, C.c_int, C.c_int,
                                C.c_void_p, ALLOC_FN, C.c_void_p, C.c_uint32, C.c_void_p]
@@ -123,8 +125,13 @@ def unifrac_dm(tree_parent, branch_len, postorder, indptr, indices, counts, n_sa
                   (indptr, torch.int64), (indices, torch.int32), (counts, torch.int32)):
         assert t.dtype == dt and t.is_contiguous() and t.device == dev
     n = int(n_samples)
+    odt = torch.float32 if precision == FP32 else torch.float64
+    assert indptr.numel() == n + 1, "indptr must have n_samples + 1 entries"
+    assert branch_len.numel() == tree_parent.numel() == postorder.numel() and indices.numel() == counts.numel()
     if out is None:
-        out = torch.empty(n * (n - 1) // 2, dtype=torch.float32 if precision == FP32 else torch.float64, device=dev)
+        out = torch.empty(n * (n - 1) // 2, dtype=odt, device=dev)
+    assert out.dtype == odt and out.device == dev and out.is_contiguous() and out.numel() == n * (n - 1) // 2, \
+        "out must be a contiguous condensed vector of n(n-1)/2 elements of the call's precision on the inputs' device"
     held = []
 
     def _alloc(nbytes, _user):

@@ -27,4 +27,22 @@ struct PlanWords {
 
 __device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31; }
 
+// Near-duplicate guard.  The separable forms finish with
+// num = S_a + S_b - 2 M, which loses relative accuracy as d -> 0 (duplicated / proportional / replicate samples,
+// PAPER.md:11 data reuse).  The finalize epilogues therefore append every pair whose distance comes out below
+// GUARD_THETA to a device list, and k_guard (guard.cuh) recomputes exactly those pairs from the definition.
+constexpr double GUARD_THETA = 0.0625;   // lowest threshold; the call raises it with the measured fixed-point error ratio
+struct GuardList {
+    uint2* pairs;            // (i, j) sample ids, i < j; NULL = guard off (debug forms)
+    unsigned int* count;     // appended so far (may exceed cap; entries beyond cap are dropped)
+    uint32_t cap;
+    float theta;             // pairs with d < theta are listed
+};
+__device__ __forceinline__ void guard_note(const GuardList& g, double num, double den, uint32_t gi, uint32_t gj) {
+    if (g.pairs && den > 0.0 && num < (double)g.theta * den) {
+        const uint32_t k = atomicAdd(g.count, 1u);
+        if (k < g.cap) g.pairs[k] = make_uint2(gi, gj);
+    }
+}
+
 }  // namespace ufb

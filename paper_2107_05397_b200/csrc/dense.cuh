@@ -42,6 +42,8 @@ struct DenseParams {
     void* out;                    // condensed, T
     int add_out;                  // out[] already holds the mid / tail branches' sum of min(u~_a, u~_b)
     double* scratch;              // [grid][64][256] fp64 partial sums
+    GuardList guard;              // pairs with d < GUARD_THETA are listed for k_guard (guard.cuh)
+    const double* hsum;           // k_dense16: [n_tiles*128] Rh_s = sum over the head rows of E_ks
 };
 
 // dense head embedding: E[h][s] for head row h (node hrows[h]); one warp per (row, tile), lane l owns samples 4l..4l+3
@@ -50,7 +52,7 @@ __global__ void __launch_bounds__(256)
 k_head_dense(uint32_t n_head, const int32_t* __restrict__ hrows, const double* __restrict__ len,
              const uint32_t* __restrict__ bits, uint32_t NW, int n_tiles, const uint32_t* __restrict__ tptr,
              const uint32_t* __restrict__ hpref, const T* __restrict__ tv /* weighted: values in rank layout; else NULL */,
-             T* __restrict__ E, size_t Npad)
+             T* __restrict__ E, size_t Npad, double* __restrict__ hsum /* per-sample sum of the head rows' values, or NULL */)
 {
     const long long gw = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
@@ -75,6 +77,10 @@ k_head_dense(uint32_t n_head, const int32_t* __restrict__ hrows, const double* _
         const T l = (T)len[v];
 #pragma unroll
         for (int j = 0; j < 4; ++j) if (m4 & (1u << j)) x[j] = l;
+    }
+    if (hsum) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) if (m4 & (1u << j)) atomicAdd(&hsum[(size_t)tile * TILE + lane * 4 + j], (double)x[j]);
     }
     Vec4<T>::store(E + (size_t)h * Npad + (size_t)tile * TILE + lane * 4, x[0], x[1], x[2], x[3]);
 }
@@ -211,6 +217,7 @@ k_dense(const __grid_constant__ CUtensorMap tmE, const DenseParams P)
                     double num = ss - 2.0 * tot;
                     const double den = P.weighted ? ss : ss - tot;
                     if (num < 0.0) num = 0.0;
+                    guard_note(P.guard, num, den, (uint32_t)gi, (uint32_t)gj);
                     reinterpret_cast<T*>(P.out)[rowbase + gj] = (T)(den > 0.0 ? num / den : 0.0);
                 }
             }
@@ -218,11 +225,26 @@ k_dense(const __grid_constant__ CUtensorMap tmE, const DenseParams P)
     }
 }
 
-// ------------------------------------------------------------------ fp32 variant with 16 consumer warps
-// Same pipeline and arithmetic as k_dense<float>, but the 128 x 128 tile pair is owned by 16 consumer warps (4 x 4 grid of
-// 32 x 32 sub-tiles, an 8 x 4 register tile per thread: 3 LDS.128 per 32 updates instead of 4 per 64) so that every
-// scheduler has four warps to pick from while FMNMX occupies the half-rate ALU pipe.
+// ------------------------------------------------------------------ fp32 variant with 16 consumer warps, mixed forms
+// Same pipeline as k_dense<float>, but the 128 x 128 tile pair is owned by 16 consumer warps (4 x 4 grid of 32 x 32
+// sub-tiles, an 8 x 4 register tile per thread: 3 LDS.128 per 32 updates) so that every scheduler has four warps to pick
+// from, and the two FP32 pipes are balanced (SURVEY 8a-5 table, rows "fp32 direct with FADD2" / "fp32 min-form"):
+//   24 of a thread's 32 cells ("min cells"):    acc += min(E_ki, E_kj)              FMNMX on the half-rate ALU pipe, the adds
+//                                               packed two per instruction (add.f32x2 -> FADD2, FMA pipe)
+//   8 cells, a >= 4 and b >= 2 ("direct cells"): acc += -0.5 * |E_ki - E_kj|         FADD + FFMA, both on the FMA pipe
+//   min(p, q) = (p + q) / 2 - |p - q| / 2, so with Rh_s = sum over the head rows of E_ks (fp64, k_head_dense) a direct cell
+//   holds M_ij - (Rh_i + Rh_j) / 2 and the epilogue adds that half-sum back.
+// A pure min-form row costs 32 ALU-pipe slots per 32 updates (that pipe's limit, 64 lanes/clk/SM); mixed, the ALU pipe
+// carries 0.75 and the FMA pipe 1.25 lane-passes per update, interleaved instruction by instruction, and the kernel is
+// bound by issue at 1.7 instructions per update instead of 2.1.
 constexpr int DENSE16_THREADS = 544;     // 16 consumer warps + 1 producer warp
+__device__ __forceinline__ constexpr bool dense16_direct_cell(int a, int b) { return a >= 4 && b >= 2; }
+
+__device__ __forceinline__ void add2(float& x0, float& x1, float m0, float m1) {
+    asm("{\n\t.reg .b64 p, q;\n\tmov.b64 p, {%0, %1};\n\tmov.b64 q, {%2, %3};\n\tadd.rn.f32x2 p, p, q;\n\tmov.b64 {%0, %1}, p;\n\t}"
+        : "+f"(x0), "+f"(x1) : "f"(m0), "f"(m1));
+}
+
 __global__ void __launch_bounds__(DENSE16_THREADS, 1)
 k_dense16(const __grid_constant__ CUtensorMap tmE, const DenseParams P)
 {
@@ -293,9 +315,15 @@ k_dense16(const __grid_constant__ CUtensorMap tmE, const DenseParams P)
                 VecLd<float>::ld(row + i_off + 16, ai + 4);
                 VecLd<float>::ld(row + j_off, bj);
 #pragma unroll
-                for (int a = 0; a < 8; ++a)
-#pragma unroll
-                    for (int b = 0; b < 4; ++b) acc[a][b] += fminf(ai[a], bj[b]);
+                for (int a = 0; a < 8; ++a) {
+                    add2(acc[a][0], acc[a][1], fminf(ai[a], bj[0]), fminf(ai[a], bj[1]));
+                    if (!dense16_direct_cell(a, 2)) {
+                        add2(acc[a][2], acc[a][3], fminf(ai[a], bj[2]), fminf(ai[a], bj[3]));
+                    } else {
+                        acc[a][2] = fmaf(fabsf(ai[a] - bj[2]), -0.5f, acc[a][2]);
+                        acc[a][3] = fmaf(fabsf(ai[a] - bj[3]), -0.5f, acc[a][3]);
+                    }
+                }
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(empty(stage));
@@ -318,17 +346,18 @@ k_dense16(const __grid_constant__ CUtensorMap tmE, const DenseParams P)
         // ----------------------------------------------------------- a-6 finalize (epilogue of the tile pair)
         const int2 ij = P.pairs[pi];
         const long long N = P.n_samples;
-        double sj[4];
+        double sj[4], hj[4];
 #pragma unroll
-        for (int b = 0; b < 4; ++b) sj[b] = P.sums[ij.y * TILE + wj * 32 + tx * 4 + b];
+        for (int b = 0; b < 4; ++b) { sj[b] = P.sums[ij.y * TILE + wj * 32 + tx * 4 + b]; hj[b] = P.hsum[ij.y * TILE + wj * 32 + tx * 4 + b]; }
 #pragma unroll
         for (int a = 0; a < 8; ++a) {
             const long long gi = (long long)ij.x * TILE + wi * 32 + (a / 4) * 16 + ty * 4 + (a % 4);
-            const double si = P.sums[gi];
+            const double si = P.sums[gi], hi = P.hsum[gi];
             const long long rowbase = gi * (2 * N - gi - 1) / 2 - gi - 1;
 #pragma unroll
             for (int b = 0; b < 4; ++b) {
                 double tot = (double)acc[a][b];
+                if (dense16_direct_cell(a, b)) tot += 0.5 * (hi + hj[b]);
                 if (scratch_live) tot += my_scratch[(size_t)(a * 4 + b) * 512];
                 acc[a][b] = 0.f;
                 const long long gj = (long long)ij.y * TILE + wj * 32 + tx * 4 + b;
@@ -338,6 +367,7 @@ k_dense16(const __grid_constant__ CUtensorMap tmE, const DenseParams P)
                     double num = ss - 2.0 * tot;
                     const double den = P.weighted ? ss : ss - tot;
                     if (num < 0.0) num = 0.0;
+                    guard_note(P.guard, num, den, (uint32_t)gi, (uint32_t)gj);
                     reinterpret_cast<float*>(P.out)[rowbase + gj] = (float)(den > 0.0 ? num / den : 0.0);
                 }
             }

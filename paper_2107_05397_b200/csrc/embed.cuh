@@ -182,11 +182,13 @@ k_values(int n, const uint32_t* __restrict__ nv, const uint32_t* __restrict__ tc
          const double* __restrict__ len, const double* __restrict__ uval, const uint32_t* __restrict__ bits, uint32_t NW,
          const uint32_t* __restrict__ cnt /* weighted: counts in rank layout at tptr; else NULL */,
          const unsigned long long* __restrict__ Tsum, uint32_t* __restrict__ ts, T* __restrict__ tv,
-         double* __restrict__ sums)
+         double* __restrict__ sums, const double* __restrict__ uerr /* per-branch (u~ - len) of the fixed point, or NULL */,
+         double* __restrict__ qerr /* [2 * samples] per-sample sum and sum of squares of it */)
 {
     const int v = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (v >= n || nv[v] == 0) return;
     const bool list = tcnt[v] != 0;
+    const double ev = uerr ? uerr[v] : 0.0;
     const uint32_t e0 = tptr[v];
     const double l = len[v];
     const T uconst = (T)(uval ? uval[v] : l);
@@ -207,6 +209,7 @@ k_values(int n, const uint32_t* __restrict__ nv, const uint32_t* __restrict__ tc
             if (cnt) val = (T)(l * ((double)cnt[e] / (double)Tsum[s]));
             if (list) { ts[e] = s; tv[e] = val; }
             atomicAdd(&sums[s], (double)val);
+            if (ev != 0.0) { atomicAdd(&qerr[2 * s], ev); atomicAdd(&qerr[2 * s + 1], ev * ev); }
             ++e;
         }
     }

@@ -2,14 +2,15 @@
 // cores (BASELINE.json:5: "Tensor cores are used only if the unweighted Gram-matrix reformulation
 // (X^T diag(len) Y) meets the stated tolerance"; identity I5 of DESIGN.md).
 //
-//   G_ab = sum_{v in head} L_v x_av x_bv ,   L_v = round(len_v * 2^q) < 2^24  (24-bit fixed point, the
-//   same number of significant bits as the fp32 embedding of the CUDA-core path),  L_v = sum_d 256^d * digit_d(v)
-//   => G = sum_d 256^d * ( X^T . (diag(digit_d) X) ) : three u8 x u8 -> s32 GEMMs, EXACT integer
-//   accumulation in TMEM (255 * K < 2^31), recombined in int64, scaled by 2^-q in fp64.
+//   G_ab = sum_{v in head} L_v x_av x_bv ,   L_v = m_v * 2^s_v ~ len_v * 2^q,  m_v < 2^24 = sum_d 256^d * digit_d(v),
+//   s_v <= 7 (a per-row shift carried by the A operand: 24 significant bits for every head branch within a factor
+//   2^7 of the longest one, fewer below that; the exact error sum is tracked per sample, see k_quant_ratio)
+//   => G = sum_d 256^d * ( (2^s X)^T . (diag(digit_d) X) ) : three u8 x u8 -> s32 GEMMs, EXACT integer
+//   accumulation in TMEM (128 * 255 * K < 2^31), recombined in int64, scaled by 2^-q in fp64.
 //   d_U = (S_a + S_b - 2 G_tot) / (S_a + S_b - G_tot),  G_tot = G + (tail branches' sum, already in out[]).
 //
 // Operands in HBM (built from the bit-packed presence matrix by k_gram_expand), row-major
-// [K_pad][N_pad] u8:  XA = x,  XB_d = digit_d * x.  One CTA = one 128 x 128 tile pair at a time
+// [K_pad][N_pad] u8:  XA = x * 2^s,  XB_d = digit_d * x.  One CTA = one 128 x 128 tile pair at a time
 // (static round-robin over a cache-blocked pair list); warp 0 lane 0 issues TMA 2D tile loads
 // (128B swizzle) into a 6-stage ring, warp 1 lane 0 issues tcgen05.mma kind::i8 (M=128; N=256 for
 // digits 0|1, N=128 for digit 2; both operands MN-major), warps 4..7 read the accumulators with
@@ -41,25 +42,36 @@ __global__ void k_gram_lenmax(int n, const uint8_t* __restrict__ cls, const doub
     if ((threadIdx.x & 31) == 0 && b) atomicMax(out_bits, b);
 }
 
-// head rank -> node id, 24-bit fixed-point length per head row, and the embedded value u~ of every branch
-// for a present sample (what the side sums and the tail lists must use so that all parts agree):
-//   head (Gram) rows: L_v * 2^-q      other rows: (double)(float)len_v
+// head rank -> node id, fixed-point length per head row, and the embedded value u~ of every branch for a present
+// sample (what the side sums and the tail lists must use so that all parts agree):
+//   head (Gram) rows: m_v * 2^(s_v - q)      other rows: (double)(float)len_v
+// Fixed point with a per-row shift: len_v * 2^q ~ m_v * 2^s_v, m_v < 2^24 (three u8 digits, the B operands), s_v <= max_shift
+// carried by the A operand (x * 2^s_v <= 128 fits its u8).  q is chosen so that the longest head branch uses s = max_shift
+// and all 24 bits of m; a branch up to 2^max_shift times shorter still keeps 24 significant bits.
+// Lq[r] = m | s << 24.
 __global__ void k_gram_quant(int n, const uint8_t* __restrict__ cls, const uint32_t* __restrict__ hrank,
-                             const double* __restrict__ len, int q, int32_t* __restrict__ hrows,
-                             uint32_t* __restrict__ Lq, double* __restrict__ uval)
+                             const double* __restrict__ len, int q, int max_shift, int32_t* __restrict__ hrows,
+                             uint32_t* __restrict__ Lq, double* __restrict__ uval, double* __restrict__ uerr)
 {
     int v = blockIdx.x * blockDim.x + threadIdx.x;
     if (v >= n) return;
     double l = len[v];
     if (cls[v] == 1) {
-        long long L = llrint(ldexp(l, q));
-        if (L > 0xffffff) L = 0xffffff;
+        const double Lf = ldexp(l, q);                       // < 2^(24 + max_shift)
+        int s = 0;
+        if (Lf >= 16777216.0) { int e; frexp(Lf, &e); s = e - 24; if (s > max_shift) s = max_shift; }
+        long long m = llrint(ldexp(Lf, -s));
+        if (m > 0xffffff) {                                  // rounded up to 2^24
+            if (s < max_shift) { ++s; m = llrint(ldexp(Lf, -s)); } else m = 0xffffff;
+        }
         uint32_t r = hrank[v];
         hrows[r] = v;
-        Lq[r] = (uint32_t)L;
-        uval[v] = ldexp((double)L, -q);
+        Lq[r] = (uint32_t)m | ((uint32_t)s << 24);
+        uval[v] = ldexp((double)m, s - q);
+        uerr[v] = uval[v] - l;                               // what the fixed point changed (0 for most rows)
     } else {
         uval[v] = (double)(float)l;
+        uerr[v] = 0.0;
     }
 }
 
@@ -73,14 +85,14 @@ __global__ void k_gram_expand(uint32_t K, uint32_t K_pad, const int32_t* __restr
     if (r >= K_pad) return;
     uint32_t word = 0, L = 0;
     if (r < K) { word = bits[(size_t)hrows[r] * NW + w]; L = Lq[r]; }
-    const uint32_t d0 = L & 255u, d1 = (L >> 8) & 255u, d2 = (L >> 16) & 255u;
+    const uint32_t d0 = L & 255u, d1 = (L >> 8) & 255u, d2 = (L >> 16) & 255u, da = 1u << (L >> 24);
     const size_t off = (size_t)r * NW * 32 + (size_t)w * 32;
     uint32_t a[8], b0[8], b1[8], b2[8];
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
         uint32_t nib = (word >> (4 * k)) & 15u;
         uint32_t m = (nib & 1u) | ((nib & 2u) << 7) | ((nib & 4u) << 14) | ((nib & 8u) << 21);   // 4 bytes of 0/1
-        a[k] = m; b0[k] = m * d0; b1[k] = m * d1; b2[k] = m * d2;
+        a[k] = m * da; b0[k] = m * d0; b1[k] = m * d1; b2[k] = m * d2;
     }
     uint4* pa = reinterpret_cast<uint4*>(XA + off);   uint4* p0 = reinterpret_cast<uint4*>(XB0 + off);
     uint4* p1 = reinterpret_cast<uint4*>(XB1 + off);  uint4* p2 = reinterpret_cast<uint4*>(XB2 + off);
@@ -148,6 +160,7 @@ struct GramParams {
     unsigned int* epoch_cnt;      // [steps_per_cta >> epoch_shift + 1], zeroed per launch; NULL = no pacing
     uint32_t steps_per_cta;       // ceil(n_pairs / grid) * (K_pad / GRAM_BK): the same for every CTA
     uint32_t epoch_shift;         // epoch = 2^epoch_shift k-blocks
+    GuardList guard;              // pairs with d < GUARD_THETA are listed for k_guard (guard.cuh)
 };
 
 // arrive at epoch e; before starting it, wait until every CTA has started epoch e - 1 (bounded spin: pacing only)
@@ -276,6 +289,7 @@ k_gram(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensor
                         const double ss = si + P.sums[gj];
                         double num = ss - 2.0 * tot, den = ss - tot;
                         if (num < 0.0) num = 0.0;
+                        guard_note(P.guard, num, den, (uint32_t)gi, (uint32_t)gj);
                         P.out[rowbase + gj] = (float)(den > 0.0 ? num / den : 0.0);
                     }
                 }

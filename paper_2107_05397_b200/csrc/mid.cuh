@@ -10,7 +10,8 @@
 // cells -- unifrac_measure_rates, rates.cuh -- against 2.6 /clk/SM for an fp32 CAS loop and 1.9e11 /s for global
 // RED.ADD).  Integer addition commutes, so the
 // result does not depend on the order in which warps reach a cell.
-//   u_q = round(u~ * 2^F),  F = 30 - ceil(log2(max_s R_s))   =>   acc <= min(R_a, R_b) * 2^F < 2^31
+//   u_q = round(u~ * 2^F),  F = 31 - ceil(log2(max_s R^mid_s)), R^mid_s = sample s's sum over the mid rows
+//   =>   acc <= min(R^mid_a, R^mid_b) * 2^F + (rounding) < 2^32   (unsigned 32-bit cells)
 //   epilogue: out[idx(a,b)] += acc * 2^-F      (exclusive owner of the tile pair; tail REDs ran before)
 // Row bookkeeping: seg[t][r] = offset (within row r's list) of the first entry with sample >= 128 t,
 // stored tile-major so that the 32 lanes of a warp (32 consecutive mid rows) read coalesced words.
@@ -98,12 +99,28 @@ k_mid_off(uint32_t n_mid, const uint32_t* __restrict__ seg, uint32_t* __restrict
     if (th == 1023) { o[n_mid] = part[1023]; ttot[t] = part[1023]; }
 }
 
-// packed tile-major entries: pk[tbase[t] + off[t][r] + k] = { r << 9 | (sample - 128 t) << 2,  round(u~ * 2^F) }
+// per-sample sums over the mid rows only (they bound the fixed-point accumulators: acc(a, b) <= min(midsum_a, midsum_b) * 2^F).
 // One warp per mid row.
+__global__ void __launch_bounds__(256)
+k_mid_sums(uint32_t n_mid, const uint32_t* __restrict__ mbase, const uint32_t* __restrict__ mlen,
+           const uint32_t* __restrict__ ts, const float* __restrict__ tv, double* __restrict__ midsum)
+{
+    const uint32_t r = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (r >= n_mid) return;
+    const uint32_t base = mbase[r], m = mlen[r];
+    for (uint32_t k = lane; k < m; k += 32) atomicAdd(&midsum[ts[base + k]], (double)tv[base + k]);
+}
+
+// packed tile-major entries: pk[tbase[t] + off[t][r] + k] = { r << 9 | (sample - 128 t) << 2,  q = round(u~ * 2^F) }
+// One warp per mid row.  The side sum of the sample is corrected by (q * 2^-F - u~), so that S_s / R_s and the pairwise
+// sums are sums of the SAME numbers (the result is then the exact distance of an embedding perturbed by <= 2^-(F+1) per
+// entry); qerr[s] collects the sum and the sum of squares of (q * 2^-F - u~) for the error-ratio check (k_quant_ratio).
 __global__ void __launch_bounds__(256)
 k_mid_pack(uint32_t n_mid, const uint32_t* __restrict__ mbase, const uint32_t* __restrict__ mlen,
            const uint32_t* __restrict__ ts, const float* __restrict__ tv, const uint32_t* __restrict__ seg,
-           const uint32_t* __restrict__ off, const uint32_t* __restrict__ tbase, float qscale, uint2* __restrict__ pk)
+           const uint32_t* __restrict__ off, const uint32_t* __restrict__ tbase, float qscale, double inv_qscale,
+           double* __restrict__ sums, double* __restrict__ qerr, uint2* __restrict__ pk)
 {
     const uint32_t r = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
@@ -115,7 +132,11 @@ k_mid_pack(uint32_t n_mid, const uint32_t* __restrict__ mbase, const uint32_t* _
         const uint32_t g0 = seg[(size_t)t * n_mid + r], g1 = seg[(size_t)(t + 1) * n_mid + r];
         const uint32_t pos = tbase[t] + off[(size_t)t * (n_mid + 1) + r] + (k - g0);
         const uint32_t x = (r << 9) | ((s & 127u) << 2);
-        pk[pos] = make_uint2(x, __float2uint_rn(tv[base + k] * qscale));
+        const float u = tv[base + k];
+        const uint32_t q = __float2uint_rn(u * qscale);
+        pk[pos] = make_uint2(x, q);
+        const double c = (double)q * inv_qscale - (double)u;
+        if (c != 0.0) { atomicAdd(&sums[s], c); atomicAdd(&qerr[2 * s], c); atomicAdd(&qerr[2 * s + 1], c * c); }
         if (k + 1 == g1 && ((g1 - g0) & 1u)) pk[pos + 1] = make_uint2(x, 0u);    // padding entry: adds 0 to a valid cell
     }
 }

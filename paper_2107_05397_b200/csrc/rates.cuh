@@ -70,7 +70,32 @@ k_rate_alu(int iters, float* __restrict__ sink)
                 else        asm volatile("max.f32 %0, %0, %1;" : "+f"(a[k]) : "f"(b[(k + 1) & 7]));
             }
             else if (mode == 1) asm volatile("add.f32 %0, %0, %1;" : "+f"(a[k]) : "f"(b[k]));
-            else { float m; asm volatile("min.f32 %0, %1, %2;" : "=f"(m) : "f"(a[k]), "f"(b[k])); asm volatile("add.f32 %0, %0, %1;" : "+f"(b[k]) : "f"(m)); }
+            else if (mode == 2) { float m; asm volatile("min.f32 %0, %1, %2;" : "=f"(m) : "f"(a[k]), "f"(b[k])); asm volatile("add.f32 %0, %0, %1;" : "+f"(b[k]) : "f"(m)); }
+        }
+        // packed adds (add.f32x2 -> FADD2): 3 = FADD2 alone (4 chains of pairs);  4 = two FMNMX + one FADD2 (the min cells of
+        // k_dense16);  5 = k_dense16's mix for 8 updates: 3 x (2 FMNMX + FADD2) + 2 x (FADD + FFMA |d| * -0.5)
+        if (mode == 3) {
+#pragma unroll
+            for (int k = 0; k < 8; k += 2)
+                asm volatile("{\n\t.reg .b64 p, q;\n\tmov.b64 p, {%0, %1};\n\tmov.b64 q, {%2, %3};\n\tadd.rn.f32x2 p, p, q;\n\tmov.b64 {%0, %1}, p;\n\t}"
+                             : "+f"(a[k]), "+f"(a[k + 1]) : "f"(b[k]), "f"(b[k + 1]));
+        } else if (mode == 4 || mode == 5) {
+#pragma unroll
+            for (int k = 0; k < 8; k += 2) {
+                if (mode == 5 && k == 6) {
+                    float d0, d1;
+                    asm volatile("sub.f32 %0, %1, %2;" : "=f"(d0) : "f"(a[k]), "f"(b[0]));
+                    asm volatile("sub.f32 %0, %1, %2;" : "=f"(d1) : "f"(a[k + 1]), "f"(b[1]));
+                    asm volatile("fma.rn.f32 %0, %1, 0fBF000000, %0;" : "+f"(b[k]) : "f"(fabsf(d0)));
+                    asm volatile("fma.rn.f32 %0, %1, 0fBF000000, %0;" : "+f"(b[k + 1]) : "f"(fabsf(d1)));
+                } else {
+                    float m0, m1;
+                    asm volatile("min.f32 %0, %1, %2;" : "=f"(m0) : "f"(a[k]), "f"(b[(k + 2) & 7]));
+                    asm volatile("min.f32 %0, %1, %2;" : "=f"(m1) : "f"(a[k + 1]), "f"(b[(k + 3) & 7]));
+                    asm volatile("{\n\t.reg .b64 p, q;\n\tmov.b64 p, {%0, %1};\n\tmov.b64 q, {%2, %3};\n\tadd.rn.f32x2 p, p, q;\n\tmov.b64 {%0, %1}, p;\n\t}"
+                                 : "+f"(b[k]), "+f"(b[k + 1]) : "f"(m0), "f"(m1));
+                }
+            }
         }
     }
     float t = 0.f;

@@ -76,6 +76,7 @@ struct StripeParams {
     unsigned long long* stats;    // [0] rows executed by consumer warps, [1] rows staged
     const void* zero_row;         // 128 zero values of T (16-byte aligned)
     int add_out;                  // min form: out[] already holds the tail branches' sum of min(u~_a,u~_b) (tail.cuh)
+    GuardList guard;              // min form: pairs with d < GUARD_THETA are listed for k_guard (guard.cuh)
 };
 
 template <typename T>
@@ -322,6 +323,7 @@ k_stripe(const StripeParams P)
                         den = P.weighted ? ss : ss + tot;
                     }
                     if (num < 0.0) num = 0.0;
+                    if (FORM == FORM_MIN) guard_note(P.guard, num, den, (uint32_t)gi, (uint32_t)gj);
                     double d = den > 0.0 ? num / den : 0.0;
                     reinterpret_cast<T*>(P.out)[rowbase + gj] = (T)d;
                 }

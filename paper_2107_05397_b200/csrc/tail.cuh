@@ -83,6 +83,25 @@ __global__ void k_max_positive(int n, const double* __restrict__ x, unsigned lon
     if ((threadIdx.x & 31) == 0 && b) atomicMax(out_bits, b);
 }
 
+// Fixed-point error ratio.  The fixed-point kernels (Gram head lengths, mid entries)
+// replace embedded values u~ by u~ + delta; the side sums use the same replaced values, so the result is the exact distance
+// of the perturbed embedding.  Per sample: B_s = sum of delta (systematic part: e.g. many branches of one length round the
+// same way), V_s = sum of delta^2 (random part).  ratio = max_s (|B_s| + 3 sqrt(V_s)) / S_s bounds the relative change of
+// any of the sample's branch-subset sums at 3 sigma; a pair with d >= 1/16 (smaller ones go through k_guard) moves by at
+// most ~32 x ratio relative.  Bit pattern of a double >= 0.
+__global__ void k_quant_ratio(int n, const double* __restrict__ qerr, const double* __restrict__ sums, unsigned long long* __restrict__ out_bits)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned long long b = 0;
+    if (i < n && qerr[2 * i + 1] > 0.0) {
+        const double e = fabs(qerr[2 * i]) + 3.0 * sqrt(qerr[2 * i + 1]);
+        const double r = sums[i] > 0.0 ? e / sums[i] : 1.0;
+        b = (unsigned long long)__double_as_longlong(r);
+    }
+    for (int o = 16; o; o >>= 1) { unsigned long long t = __shfl_xor_sync(0xffffffffu, b, o); b = t > b ? t : b; }
+    if ((threadIdx.x & 31) == 0 && b) atomicMax(out_bits, b);
+}
+
 __global__ void k_mark_class(int n, const uint8_t* __restrict__ cls, uint8_t which, uint32_t* __restrict__ mark)
 {
     int v = blockIdx.x * blockDim.x + threadIdx.x;

@@ -12,6 +12,7 @@
 #include "dense.cuh"
 #include "rates.cuh"
 #include "mantel.cuh"
+#include "guard.cuh"
 
 #include <cstdio>
 #include <cstdlib>
@@ -34,6 +35,12 @@ thread_local bool g_stats_pending = false;
 struct CudaFail { cudaError_t e; const char* what; int line; };
 struct WorkspaceFail {};
 struct StatusFail { int status; };
+struct RetryExact {};        // the fixed-point error ratio is over budget: rerun without the fixed-point kernels
+// Fixed-point error ratio r (tail.cuh: k_quant_ratio): a distance d moves by at most ~2 r / d relative, so the guard
+// threshold is raised to theta = max(1/16, r / QUANT_REL) -- every pair below it is recomputed from the definition -- and
+// the call is rerun without the fixed-point kernels when theta would pass 1/2 (r > QUANT_RATIO_BUDGET).
+constexpr double QUANT_REL = 2.5e-6;                 // 2 r / d <= 5e-6 for d >= theta
+constexpr double QUANT_RATIO_BUDGET = 0.5 * QUANT_REL;
 
 #define CU(x)                                                                                   \
     do {                                                                                        \
@@ -125,7 +132,7 @@ struct Timer {
 
 template <typename T>
 void run(int32_t n, const int32_t* parent, const double* len, const int32_t* postorder, unifrac_csr_t tab,
-         int32_t N, int weighted, void* out, Arena& A, uint32_t flags, cudaStream_t st, int shard, int n_shards)
+         int32_t N, int weighted, void* out, Arena& A, uint32_t flags, cudaStream_t st, int shard, int n_shards, bool is_retry)
 {
     const bool validate = !(flags & UNIFRAC_FLAG_SKIP_VALIDATION);
     const bool timing = getenv("UNIFRAC_B200_TIMING") && atoi(getenv("UNIFRAC_B200_TIMING")) != 0;
@@ -270,6 +277,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     // CUDA-core head path: dense min-GEMM kernel (dense.cuh) unless a debug form needs the sparse-aware compact-row kernel
     const bool dense_head = !use_gram && !(flags & (UNIFRAC_FLAG_ABSDIFF | UNIFRAC_FLAG_LITERAL | UNIFRAC_FLAG_NO_TAIL | UNIFRAC_FLAG_SPARSE_STRIPE));
     double* uval = nullptr;
+    double* uerr = nullptr;                                    // Gram path: |u~_v - len_v| of the fixed-point head lengths
     uint8_t* XG[4] = {nullptr, nullptr, nullptr, nullptr};
     uint32_t K_pad = 0;
     int gram_q = 0;
@@ -289,15 +297,18 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         CU(cudaStreamSynchronize(st));
         double lm; memcpy(&lm, &h_lmax, sizeof(lm));
         int ex = 0; frexp(lm, &ex);
-        gram_q = 24 - ex;                                   // lmax * 2^q in [2^23, 2^24)
         const uint32_t K = (uint32_t)head_rows;
         K_pad = (K + GRAM_BK - 1) / GRAM_BK * GRAM_BK;
+        int max_shift = 7;                                  // s32 accumulators: 2^shift * 255 * K_pad < 2^31
+        while (max_shift > 0 && (255ull << max_shift) * K_pad >= (1ull << 31)) --max_shift;
+        gram_q = 24 - ex + max_shift;                       // lmax * 2^q in [2^(23 + shift), 2^(24 + shift))
         const size_t Npad = (size_t)NW * 32;
         hrows = A.get_n<int32_t>(K_pad);
         uint32_t* Lq = A.get_n<uint32_t>(K_pad);
         uval = A.get_n<double>(n);
+        uerr = A.get_n<double>(n);
         for (auto& x : XG) x = A.get_n<uint8_t>((size_t)K_pad * Npad);
-        k_gram_quant<<<cdiv(n, TB), TB, 0, st>>>(n, cls, hrank, len, gram_q, hrows, Lq, uval); CU_LAUNCH(); ++launches;
+        k_gram_quant<<<cdiv(n, TB), TB, 0, st>>>(n, cls, hrank, len, gram_q, max_shift, hrows, Lq, uval, uerr); CU_LAUNCH(); ++launches;
         k_gram_expand<<<cdiv((long long)K_pad * NW, TB), TB, 0, st>>>(K, K_pad, hrows, Lq, bits, NW, XG[0], XG[1], XG[2], XG[3]);
         CU_LAUNCH(); ++launches;
     }
@@ -329,9 +340,10 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         }
     }
     // ------------------------------------------------------------------ a-3 / a-4 values, sample ids, side sums
-    double* sums = A.get_n<double>((size_t)n_tiles * TILE);
-    CU(cudaMemsetAsync(sums, 0, sizeof(double) * (size_t)n_tiles * TILE, st));
-    k_values<T><<<cdiv((long long)n * 32, TB), TB, 0, st>>>(n, nv, tcnt, tptr, len, uval, bits, NW, cnt, Tsum, ts, tv, sums); CU_LAUNCH(); ++launches;
+    double* sums = A.get_n<double>((size_t)n_tiles * TILE * 3);
+    double* qerr = sums + (size_t)n_tiles * TILE;             // [2 * samples] per-sample sum / sum of squares of the fixed-point errors
+    CU(cudaMemsetAsync(sums, 0, sizeof(double) * (size_t)n_tiles * TILE * 3, st));
+    k_values<T><<<cdiv((long long)n * 32, TB), TB, 0, st>>>(n, nv, tcnt, tptr, len, uval, bits, NW, cnt, Tsum, ts, tv, sums, uerr, qerr); CU_LAUNCH(); ++launches;
 
     // ------------------------------------------------------------------ head rows of the CUDA-core stripe kernel: compact dense per-tile rows
     const uint32_t nwords = (uint32_t)cdiv(n, 32);
@@ -341,6 +353,12 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     T* Edense = nullptr;
     const size_t Npad = (size_t)n_tiles * TILE;
     uint32_t Kd_pad = 0;
+    const bool dense16 = dense_head && std::is_same<T, float>::value && envd("UNIFRAC_B200_DENSE16", 1) != 0;   // fp32: 16 consumer warps, mixed forms
+    double* hsum = nullptr;
+    if (dense16) {
+        hsum = A.get_n<double>((size_t)n_tiles * TILE);
+        CU(cudaMemsetAsync(hsum, 0, sizeof(double) * (size_t)n_tiles * TILE, st));
+    }
     if (dense_head) {
         constexpr int BK = DenseCfg<T>::BK;
         Kd_pad = (uint32_t)((head_rows + BK - 1) / BK * BK);
@@ -369,7 +387,8 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
                 k_head_pref<<<cdiv((long long)head_rows * 32, TB), TB, 0, st>>>((uint32_t)head_rows, hrows, bits, NW, n_tiles, hpref); CU_LAUNCH(); ++launches;
             }
             k_head_dense<T><<<cdiv((long long)head_rows * n_tiles * 32, TB), TB, 0, st>>>((uint32_t)head_rows, hrows, len, bits, NW, n_tiles, tptr, hpref,
-                                                                                         weighted ? tv : nullptr, Edense, Npad);
+                                                                                         weighted ? tv : nullptr, Edense, Npad,
+                                                                                         hsum);
             CU_LAUNCH(); ++launches;
             embed_rows = head_rows * (uint64_t)n_tiles;
         }
@@ -451,6 +470,18 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     // ------------------------------------------------------------------ a-5 (mid branches): per tile pair, fixed point in shared memory
     unsigned mid_launches = 0;
     int mid_F = 0;
+    bool mid_packed = false;
+    double quant_ratio = 0.0;
+    // fixed-point error ratio (Gram head lengths + mid entries): over budget => rerun without the fixed-point kernels
+    auto check_quant_ratio = [&]() {
+        unsigned long long* rbits = work + 19;
+        k_quant_ratio<<<cdiv((long long)n_tiles * TILE, TB), TB, 0, st>>>(n_tiles * TILE, qerr, sums, rbits); CU_LAUNCH(); ++launches;
+        unsigned long long h_r = 0;
+        CU(cudaMemcpyAsync(&h_r, rbits, sizeof(h_r), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        memcpy(&quant_ratio, &h_r, sizeof(quant_ratio));
+        if (quant_ratio > envd("UNIFRAC_B200_QUANT_BUDGET", QUANT_RATIO_BUDGET) && !is_retry) throw RetryExact{};
+    };
     if (mid_rows) {
         if constexpr (std::is_same<T, float>::value) {
             if (mid_rows >= (1ull << 23)) throw StatusFail{UNIFRAC_ERR_UNSUPPORTED};     // packed entries keep the row in 23 bits
@@ -472,7 +503,10 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             k_mid_off<<<n_tiles, 1024, 0, st>>>(n_mid, mseg, moff, ttot); CU_LAUNCH(); ++launches;
             k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>(n_tiles, ttot, tbase); CU_LAUNCH(); ++launches;
             unsigned long long* smax = work + 15;
-            k_max_positive<<<cdiv((long long)n_tiles * TILE, TB), TB, 0, st>>>(n_tiles * TILE, sums, smax); CU_LAUNCH(); ++launches;
+            double* midsum = A.get_n<double>((size_t)n_tiles * TILE);
+            CU(cudaMemsetAsync(midsum, 0, sizeof(double) * (size_t)n_tiles * TILE, st));
+            k_mid_sums<<<cdiv((long long)n_mid * 32, TB), TB, 0, st>>>(n_mid, mbase, mlen, ts, reinterpret_cast<const float*>(tv), midsum); CU_LAUNCH(); ++launches;
+            k_max_positive<<<cdiv((long long)n_tiles * TILE, TB), TB, 0, st>>>(n_tiles * TILE, midsum, smax); CU_LAUNCH(); ++launches;
             unsigned long long h_smax = 0;
             CU(cudaMemcpyAsync(&h_smax, smax, sizeof(h_smax), cudaMemcpyDeviceToHost, st));
             uint32_t h_pk_total = 0;                            // packed entries incl. the even-length padding
@@ -483,11 +517,15 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             CU(cudaStreamSynchronize(st));
             double sm; memcpy(&sm, &h_smax, sizeof(sm));
             int ex = 0; frexp(sm > 0 ? sm : 1.0, &ex);          // sm < 2^ex
-            mid_F = 30 - ex;                                     // acc <= min(R_a, R_b) * 2^F < 2^30 (+ rounding slack)
+            // unsigned 32-bit cells: acc <= min(R^mid_a, R^mid_b) * 2^F + (rounding: at most half a unit per mid row)
+            mid_F = 32 - ex;
+            if (ldexp(sm, mid_F) + 0.5 * (double)n_mid + 1.0 > 4294967295.0) --mid_F;
             (void)mid_entries;
             uint2* pk = A.get_n<uint2>(h_pk_total ? h_pk_total : 1);
             k_mid_pack<<<cdiv((long long)n_mid * 32, TB), TB, 0, st>>>(n_mid, mbase, mlen, ts, reinterpret_cast<const float*>(tv), mseg, moff, tbase,
-                                                                      ldexpf(1.0f, mid_F), pk); CU_LAUNCH(); ++launches;
+                                                                      ldexpf(1.0f, mid_F), ldexp(1.0, -mid_F), sums, qerr, pk); CU_LAUNCH(); ++launches;
+            mid_packed = true;
+            check_quant_ratio();
             MidParams M{};
             M.pairs = mpairs; M.n_pairs = (uint32_t)h_mp.size(); M.counter = reinterpret_cast<unsigned int*>(work + 7);
             M.n_mid = n_mid; M.off = moff; M.tbase = tbase; M.pk = pk;
@@ -504,8 +542,17 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             }
         }
     }
+    if (use_gram && !mid_packed) check_quant_ratio();
     tm.mark();
 
+    // ------------------------------------------------------------------ near-duplicate guard list (filled by the finalize epilogues)
+    GuardList GL{nullptr, nullptr, 0u, (float)std::max(GUARD_THETA, quant_ratio / QUANT_REL)};
+    if (!(flags & (UNIFRAC_FLAG_LITERAL | UNIFRAC_FLAG_ABSDIFF))) {
+        const unsigned long long Pn = (unsigned long long)N * (N - 1) / 2;
+        GL.cap = (uint32_t)std::min<unsigned long long>(Pn, std::max<unsigned long long>(1ull << 22, 64ull * N));
+        GL.pairs = A.get_n<uint2>(GL.cap);
+        GL.count = reinterpret_cast<unsigned int*>(work + 18);         // zeroed with the other counters
+    }
     // ------------------------------------------------------------------ a-5 / a-6 stripe accumulation + finalize
     unsigned long long* kstats = work + 4;     // [0] rows executed, [1] rows staged (zeroed above)
     unsigned stripe_launches = 0;
@@ -526,7 +573,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             CUtensorMap tmB2 = make_u8_rowmajor_map(XG[3], Npad, K_pad, TILE, GRAM_BK);
             GramParams G{};
             G.pairs = pairs; G.n_pairs = n_pairs; G.K_pad = K_pad; G.sums = sums; G.n_samples = N;
-            G.out = reinterpret_cast<float*>(out); G.add_out = (tail_rows || mid_rows) ? 1 : 0; G.q = gram_q;
+            G.out = reinterpret_cast<float*>(out); G.add_out = (tail_rows || mid_rows) ? 1 : 0; G.q = gram_q; G.guard = GL;
             CU(cudaFuncSetAttribute(k_gram, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GRAM_SMEM));
             unsigned grid = (unsigned)std::min<long long>(n_sm, n_pairs);
             const int eshift = (int)envd("UNIFRAC_B200_GRAM_EPOCH_SHIFT", 5);
@@ -550,11 +597,12 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
                                             TILE, DenseCfg<T>::BK, CU_TENSOR_MAP_SWIZZLE_NONE);
         DenseParams D{};
         D.pairs = pairs; D.n_pairs = n_pairs; D.K_pad = Kd_pad; D.sums = sums; D.n_samples = N; D.weighted = weighted; D.out = out;
-        D.add_out = (tail_rows || mid_rows) ? 1 : 0;
+        D.add_out = (tail_rows || mid_rows) ? 1 : 0; D.guard = GL;
         const size_t smem = dense_smem_bytes<T>();
         unsigned grid = (unsigned)std::min<long long>(n_sm, n_pairs);
         D.scratch = A.get_n<double>((size_t)grid * 64 * 256);
-        if (f32 && envd("UNIFRAC_B200_DENSE16", 1) != 0) {       // fp32: 16 consumer warps
+        D.hsum = hsum;
+        if (dense16) {
             CU(cudaFuncSetAttribute(k_dense16, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             if (grid) { k_dense16<<<grid, DENSE16_THREADS, smem, st>>>(tmE, D); CU_LAUNCH(); ++launches; ++stripe_launches; }
         } else {
@@ -579,7 +627,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     P.tileE = reinterpret_cast<const void* const*>(tileE);
     P.tileQ = tileQ; P.flags = rflags; P.rank = rrank; P.nwords = nwords;
     P.pairs = pairs; P.n_pairs = n_pairs; P.counter = counter; P.sums = sums;
-    P.n_samples = N; P.weighted = weighted; P.out = out; P.stats = kstats; P.zero_row = zero_row;
+    P.n_samples = N; P.weighted = weighted; P.out = out; P.stats = kstats; P.zero_row = zero_row; P.guard = GL;
 
     if (flags & UNIFRAC_FLAG_LITERAL) {
         k_literal<T><<<n_pairs, 256, 0, st>>>(P); CU_LAUNCH(); ++launches; ++stripe_launches;
@@ -596,10 +644,21 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     }
     CU(cudaStreamSynchronize(st));           // h_pairs staging copy done before it goes out of scope
     }
+    // ------------------------------------------------------------------ near-duplicate guard: listed pairs from the definition
+    if (GL.pairs) {
+        const unsigned ggrid = (unsigned)std::max(1, std::min(n_sm, (int)std::min<unsigned long long>(GL.cap, 1u << 30)));
+        GuardParams GP{};
+        GP.n = n; GP.parent = parent; GP.len = len; GP.indptr = tab.indptr; GP.indices = tab.indices; GP.counts = tab.counts;
+        GP.Tsum = Tsum; GP.order = nullptr; GP.N = N; GP.weighted = weighted; GP.list = GL; GP.out = out;
+        GP.scratch = A.get_n<uint32_t>((size_t)ggrid * 3 * n);
+        CU(cudaMemsetAsync(GP.scratch, 0, sizeof(uint32_t) * (size_t)ggrid * 3 * n, st));
+        k_guard<T><<<ggrid, GUARD_THREADS, 0, st>>>(GP); CU_LAUNCH(); ++launches;
+    }
     // stripe counters -> pinned host block (read lazily by unifrac_last_stats)
-    if (!g_stats_pinned) { CU(cudaHostAlloc(&g_stats_pinned, 2 * sizeof(unsigned long long), cudaHostAllocDefault)); }
+    if (!g_stats_pinned) { CU(cudaHostAlloc(&g_stats_pinned, 4 * sizeof(unsigned long long), cudaHostAllocDefault)); }
     if (!g_stats_event) { CU(cudaEventCreateWithFlags(&g_stats_event, cudaEventDisableTiming)); }
     CU(cudaMemcpyAsync(g_stats_pinned, kstats, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(g_stats_pinned + 2, work + 18, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
     CU(cudaEventRecord(g_stats_event, st));
     g_stats_pending = true;
     tm.mark();
@@ -614,6 +673,8 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     g_stats.tail_launches = tail_launches;
     g_stats.mid_rows = mid_rows; g_stats.mid_updates = mid_updates; g_stats.mid_launches = mid_launches; g_stats.mid_F = (uint32_t)mid_F;
     g_stats.gram = use_gram ? 1u : 0u; g_stats.dense = dense_head ? 1u : 0u; g_stats.gram_k = K_pad; g_stats.gram_q = (uint32_t)gram_q;
+    g_stats.guard_capacity = GL.cap; g_stats.guard_theta = GL.theta;
+    g_stats.quant_err_ratio = (float)quant_ratio; g_stats.quant_fallback = is_retry ? 1u : 0u;
     g_stats.n_tile_pairs = n_pairs;
     g_stats.n_levels = (uint32_t)n_levels;
     g_stats.stripe_launches = stripe_launches;
@@ -644,9 +705,16 @@ int guarded(int32_t n_nodes, const int32_t* parent, const double* len, const int
     if ((long long)N > (1ll << 23)) return UNIFRAC_ERR_UNSUPPORTED;
     Arena A{alloc, user, st};
     int rc = UNIFRAC_OK;
+    const bool w = variant == UNIFRAC_WEIGHTED_NORMALIZED;
     try {
-        if (precision == UNIFRAC_FP32) run<float>(n_nodes, parent, len, postorder, tab, N, variant == UNIFRAC_WEIGHTED_NORMALIZED, out, A, flags, st, shard, n_shards);
-        else run<double>(n_nodes, parent, len, postorder, tab, N, variant == UNIFRAC_WEIGHTED_NORMALIZED, out, A, flags, st, shard, n_shards);
+        try {
+            if (precision == UNIFRAC_FP32) run<float>(n_nodes, parent, len, postorder, tab, N, w, out, A, flags, st, shard, n_shards, false);
+            else run<double>(n_nodes, parent, len, postorder, tab, N, w, out, A, flags, st, shard, n_shards, false);
+        } catch (const RetryExact&) {
+            // only the fp32 path has fixed-point kernels; head rows on the CUDA-core kernel, the rest on the fp32 scatter
+            A.release();
+            run<float>(n_nodes, parent, len, postorder, tab, N, w, out, A, flags | UNIFRAC_FLAG_NO_TENSOR | UNIFRAC_FLAG_NO_MID, st, shard, n_shards, true);
+        }
     } catch (const CudaFail& f) {
         char buf[512];
         snprintf(buf, sizeof(buf), "%s: %s (unifrac_b200.cu:%d)", f.what, cudaGetErrorString(f.e), f.line);
@@ -788,6 +856,7 @@ int unifrac_last_stats(unifrac_stats_t* out)
         if (g_stats.gram || g_stats.dense) g_stats.updates_executed_head = g_stats.head_rows * ((uint64_t)g_stats.updates_dense / (g_stats.branches_embedded ? g_stats.branches_embedded : 1));
         g_stats.updates_executed = g_stats.updates_executed_head + g_stats.tail_updates + g_stats.mid_updates;
         g_stats.rows_staged = g_stats_pinned[1];
+        g_stats.guard_pairs = (uint32_t)(g_stats_pinned[2] & 0xffffffffull);      // listed; min(guard_pairs, guard_capacity) were recomputed
         g_stats_pending = false;
     }
     *out = g_stats;
@@ -862,6 +931,12 @@ int unifrac_measure_rates(unifrac_rates_t* out, void* stream)
         out->fmnmx_per_s = (double)gf * 256 * it_f * 8 / t3;
         out->fadd_per_s = (double)gf * 256 * it_f * 8 / t4;
         out->fmnmx_fadd_per_s = (double)gf * 256 * it_f * 16 / t5;
+        double t6 = timed([&] { k_rate_alu<3><<<gf, 256, 0, st>>>(it_f, fsink); CU_LAUNCH(); });
+        double t7 = timed([&] { k_rate_alu<4><<<gf, 256, 0, st>>>(it_f, fsink); CU_LAUNCH(); });
+        double t8 = timed([&] { k_rate_alu<5><<<gf, 256, 0, st>>>(it_f, fsink); CU_LAUNCH(); });
+        out->fadd2_per_s = (double)gf * 256 * it_f * 8 / t6;               // 4 FADD2 = 8 lane-ops per iteration
+        out->fmnmx2_fadd2_updates_per_s = (double)gf * 256 * it_f * 8 / t7;
+        out->dense16_mix_updates_per_s = (double)gf * 256 * it_f * 8 / t8;
         out->sm_count = n_sm; out->sm_clock_khz = khz;
     } catch (const CudaFail& f) {
         char b[512];
@@ -892,6 +967,6 @@ const char* unifrac_status_string(int status)
 }
 
 const char* unifrac_last_cuda_error(void) { return g_cuda_err.c_str(); }
-int unifrac_abi_version(void) { return 4; }
+int unifrac_abi_version(void) { return 5; }
 
 }  // extern "C"

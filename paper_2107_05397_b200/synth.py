@@ -316,3 +316,46 @@ def condensed_index(n: int, i, j):
     i = np.asarray(i, dtype=np.int64)
     j = np.asarray(j, dtype=np.int64)
     return i * (2 * n - i - 1) // 2 + (j - i - 1)
+
+
+def rows_of(p: Problem) -> list:
+    """The table of `p` as a list of {tip node id: count} dicts (one per sample)."""
+    return [{int(t): int(c) for t, c in zip(p.indices[p.indptr[s]:p.indptr[s + 1]], p.counts[p.indptr[s]:p.indptr[s + 1]])}
+            for s in range(p.n_samples)]
+
+
+def with_rows(p: Problem, rows, branch_len=None) -> Problem:
+    """Same tree as `p` (optionally other branch lengths) with another table."""
+    q = problem_from_parent(p.parent, p.branch_len if branch_len is None else branch_len, rows, name=p.name)
+    q.postorder = p.postorder
+    return q
+
+
+def plant_near_duplicates(p: Problem, n_each: int, seed: int = 0):
+    """Overwrite 3 * n_each samples of `p` with (a) exact copies, (b) integer multiples and (c) copies with one count
+    changed by 1 and one feature dropped, of other samples, at positions spread so that sources and copies sit in different 128-sample tiles and
+    on tile boundaries.  Returns (problem, pairs [3 * n_each, 2] int32 with i < j, kinds) -- kinds 0 / 1 / 2."""
+    rng = np.random.default_rng(seed + 4242)
+    rows = rows_of(p)
+    n = p.n_samples
+    boundary = [s for t in range(128, n, 128) for s in (t - 1, t)]
+    pool = boundary + [int(x) for x in rng.permutation(n) if int(x) not in set(boundary)]
+    dst = pool[:3 * n_each]
+    taken = set(dst)
+    src = [int(x) for x in rng.permutation(n) if int(x) not in taken][:3 * n_each]
+    pairs, kinds = [], []
+    for k, (a, b) in enumerate(zip(src, dst)):
+        kind = k % 3
+        r = dict(rows[a])
+        if kind == 1:
+            m = int(rng.integers(2, 9))
+            r = {t: c * m for t, c in r.items()}
+        elif kind == 2:
+            keys = sorted(r)
+            r[keys[int(rng.integers(0, len(keys)))]] += 1
+            if len(keys) > 2:                           # and one feature dropped, so that presence changes as well
+                del r[keys[int(rng.integers(0, len(keys)))]]
+        rows[b] = r
+        pairs.append((min(a, b), max(a, b)))
+        kinds.append(kind)
+    return with_rows(p, rows), np.asarray(pairs, dtype=np.int32), np.asarray(kinds)

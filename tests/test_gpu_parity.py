@@ -106,24 +106,6 @@ def test_general_trees_multifurcation_unary_zero_length(B, O, seed):
             check(gpu_dm(B, p, variant, 0, flags), want, 0)
 
 
-def test_duplicate_and_proportional_samples_give_zero(B):
-    parent, bl = synth.random_tree(60, np.random.default_rng(9), p_zero_len=0.0)
-    tips = synth.tip_ids(parent)
-    rows = synth.random_table(tips, 6, np.random.default_rng(10))
-    rows.append(dict(rows[1]))
-    rows.append({t: 7 * c for t, c in rows[2].items()})
-    p = synth.problem_from_parent(parent, bl, rows)
-    n = p.n_samples
-    for variant in (U, W):
-        for precision, tol in ((1, 1e-14), (0, 1e-6)):
-            d = gpu_dm(B, p, variant, precision)
-            assert abs(d[int(synth.condensed_index(n, 1, 6))]) <= tol
-            assert abs(d[int(synth.condensed_index(n, 2, 7))]) <= tol
-            assert np.all(d >= 0) and np.all(d <= 1 + 1e-6) and not np.isnan(d).any()
-        d = gpu_dm(B, p, variant, 1, flags=8)          # direct form: exactly 0
-        assert d[int(synth.condensed_index(n, 1, 6))] == 0.0 and d[int(synth.condensed_index(n, 2, 7))] == 0.0
-
-
 def test_zero_denominator_gives_zero(B):
     parent, bl = synth.star_tree(3, [0.0, 0.0, 1.0])
     p = synth.problem_from_parent(parent, bl, [{0: 1}, {1: 2}, {2: 1}])
