@@ -27,7 +27,7 @@ def test_header_symbols_are_exported_and_bound():
 
 
 def test_version_and_status_strings_without_gpu():
-    assert binding.unifrac_abi_version() == 4
+    assert binding.unifrac_abi_version() == binding.ABI_VERSION
     assert binding.unifrac_status_string(0) == "ok"
     assert "tree" in binding.unifrac_status_string(binding.ERR_INVALID_TREE)
 
@@ -42,10 +42,13 @@ def test_host_checkable_errors_return_before_any_cuda_work():
     assert rc == binding.ERR_INVALID_ARG
 
 
-def test_library_is_built_for_sm_100a_with_bulk_copies():
+def test_library_is_built_for_sm_100a_with_tcgen05_tma_and_bulk_copies():
     sass = subprocess.run(["cuobjdump", "-sass", build.LIB], capture_output=True, text=True).stdout
     assert "sm_100a" in sass
-    assert "UBLKCP" in sass            # cp.async.bulk (TMA bulk copy) in the stripe kernel
+    assert "UBLKCP" in sass            # cp.async.bulk (TMA bulk copy): Mantel row staging, debug stripe kernel
+    assert "UTMALDG" in sass           # cp.async.bulk.tensor (TMA tile loads): k_dense16 / k_gram operand staging
+    assert "UTCIMMA" in sass           # tcgen05.mma kind::i8: the Gram kernel did not fall back to CUDA cores
+    assert "LDTM" in sass              # tcgen05.ld: TMEM accumulators read back by the Gram epilogue
 
 
 def test_shard_of_pair_is_a_partition_by_blocks_of_12_tiles():
