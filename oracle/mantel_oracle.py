@@ -1,4 +1,4 @@
-"""CPU oracle for the Mantel test with Pearson's correlation -- TEST INFRASTRUCTURE ONLY.
+"""CPU oracle for the Mantel test (Pearson and Spearman) -- TEST INFRASTRUCTURE ONLY.
 
 Only tests/ and bench.py's cpu_baseline leg may import this module; it imports nothing from the CUDA package.
 
@@ -56,6 +56,49 @@ def mantel_pearson(x_condensed, y_condensed, n: int, perms):
     for k, pi in enumerate(perms):
         Xp = X[pi][:, pi]                       # X^pi[i][j] = X[pi(i)][pi(j)]
         rk[k] = pearson(upper(Xp), y)
+    K = len(perms)
+    p_two = (np.sum(np.abs(rk) >= abs(r)) + 1.0) / (K + 1.0)
+    p_gr = (np.sum(rk >= r) + 1.0) / (K + 1.0)
+    p_le = (np.sum(rk <= r) + 1.0) / (K + 1.0)
+    return r, float(p_two), float(p_gr), float(p_le), rk
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Spearman variant.  PAPER.md:41 (section III): "... or Spearman's rank correlation coefficient"; "the
+# Spearman variety requires about 18 minutes".  Textbook definition (readings M5-M6): Spearman's rho of two
+# vectors is Pearson's correlation of their RANKS, ties receiving the average of the ranks they span (1-based,
+# "fractional ranking").  The Mantel test is otherwise unchanged: for every permutation the upper triangle of the
+# permuted X is ranked again and correlated with the ranks of y.
+def average_ranks(a: np.ndarray) -> np.ndarray:
+    """1-based ranks of a vector; a run of equal values gets the mean of the positions it occupies.  Plain loop over
+    the sorted order (no scipy): obviously correct, O(n log n)."""
+    a = np.asarray(a, dtype=np.float64)
+    order = np.argsort(a, kind="stable")
+    ranks = np.empty(a.shape[0], dtype=np.float64)
+    s = 0
+    n = a.shape[0]
+    while s < n:
+        e = s
+        while e + 1 < n and a[order[e + 1]] == a[order[s]]:
+            e += 1
+        ranks[order[s:e + 1]] = 0.5 * (s + e) + 1.0            # positions s..e (0-based) -> ranks s+1..e+1, averaged
+        s = e + 1
+    return ranks
+
+
+def spearman(a: np.ndarray, b: np.ndarray) -> float:
+    return pearson(average_ranks(a), average_ranks(b))
+
+
+def mantel_spearman(x_condensed, y_condensed, n: int, perms):
+    """Returns (rho, p_two_sided, p_greater, p_less, rho_perm[K]); same conventions as mantel_pearson."""
+    X = square_from_condensed(x_condensed, n)
+    y = np.asarray(y_condensed, dtype=np.float64)
+    r = spearman(upper(X), y)
+    perms = np.asarray(perms, dtype=np.int64).reshape(-1, n)
+    rk = np.empty(len(perms), dtype=np.float64)
+    for k, pi in enumerate(perms):
+        rk[k] = spearman(upper(X[pi][:, pi]), y)
     K = len(perms)
     p_two = (np.sum(np.abs(rk) >= abs(r)) + 1.0) / (K + 1.0)
     p_gr = (np.sum(rk >= r) + 1.0) / (K + 1.0)
