@@ -201,6 +201,20 @@ int unifrac_mantel_pearson(int32_t n_samples, const void *x_condensed, const voi
                            unifrac_precision_t precision, const int32_t *perms, int32_t n_perms, double *out,
                            unifrac_alloc_fn alloc, void *alloc_user, void *stream);
 
+/*
+ * unifrac_mantel_spearman -- the same test with Spearman's rank correlation ("either Pearson's product-moment
+ * correlation coefficient or Spearman's rank correlation coefficient").  rho = Pearson's r of the RANKS of the
+ * two condensed vectors, tied values sharing the mean of the ranks they span (1-based fractional ranking, DESIGN.md readings
+ * M5-M6); a permutation of the objects only moves entries around, so every rho_k is Pearson's r between the permuted rank
+ * matrix of X and the ranks of y.  Arguments, output layout, p-values and error behaviour are those of unifrac_mantel_pearson.
+ * The ranks come from a stable LSD radix sort of (value, position) pairs on the device (no library sort); they are held in
+ * fp64.  Workspace: ~2 x (key + position) x n(n-1)/2 for the sort, 2 x 8 x n(n-1)/2 for the ranks, 8 n^2 for the square copy.
+ * n(n-1)/2 >= 2^32 - 1: UNIFRAC_ERR_UNSUPPORTED.  NaNs are not supported.  Asynchronous on `stream`.
+ */
+int unifrac_mantel_spearman(int32_t n_samples, const void *x_condensed, const void *y_condensed,
+                            unifrac_precision_t precision, const int32_t *perms, int32_t n_perms, double *out,
+                            unifrac_alloc_fn alloc, void *alloc_user, void *stream);
+
 /* Device-rate probes (not on the data path): what this GPU retires per second of the two atomic units of work the
  * sparse kernels are made of; they are the constants of the head / mid / tail cost model and the `peak` of the
  * k_mid / k_tail_scatter rooflines in bench.py.  Runs ~20 ms of probe kernels on `stream` and synchronises it. */

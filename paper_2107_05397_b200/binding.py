@@ -24,7 +24,7 @@ OK = 0
 ERR_INVALID_ARG, ERR_INVALID_TREE, ERR_INVALID_TABLE, ERR_EMPTY_SAMPLE = -1, -2, -3, -4
 ERR_WORKSPACE, ERR_CUDA, ERR_UNSUPPORTED = -5, -6, -7
 
-EXPORTS = ("unifrac_dm", "unifrac_dm_shard", "unifrac_shard_of_pair", "unifrac_dm_host", "unifrac_mantel_pearson", "unifrac_measure_rates", "unifrac_last_stats", "unifrac_status_string",
+EXPORTS = ("unifrac_dm", "unifrac_dm_shard", "unifrac_shard_of_pair", "unifrac_dm_host", "unifrac_mantel_pearson", "unifrac_mantel_spearman", "unifrac_measure_rates", "unifrac_last_stats", "unifrac_status_string",
            "unifrac_last_cuda_error", "unifrac_abi_version")
 
 
@@ -92,6 +92,8 @@ def load(build_if_missing: bool = True) -> C.CDLL:
     lib.unifrac_mantel_pearson.restype = C.c_int
     lib.unifrac_mantel_pearson.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_int32, C.c_void_p,
                                            ALLOC_FN, C.c_void_p, C.c_void_p]
+    lib.unifrac_mantel_spearman.restype = C.c_int
+    lib.unifrac_mantel_spearman.argtypes = lib.unifrac_mantel_pearson.argtypes
     lib.unifrac_measure_rates.restype = C.c_int
     lib.unifrac_measure_rates.argtypes = [C.POINTER(Rates), C.c_void_p]
     lib.unifrac_last_stats.restype = C.c_int
@@ -184,7 +186,12 @@ def unifrac_last_stats() -> dict:
     return {k: getattr(s, k) for k, _ in Stats._fields_}
 
 
-def unifrac_mantel_pearson(x_condensed, y_condensed, n_samples: int, perms, stream=None):
+def unifrac_mantel_spearman(x_condensed, y_condensed, n_samples: int, perms, stream=None):
+    """Mantel test with Spearman's rank correlation; same arguments and result layout as unifrac_mantel_pearson."""
+    return unifrac_mantel_pearson(x_condensed, y_condensed, n_samples, perms, stream=stream, _entry="unifrac_mantel_spearman")
+
+
+def unifrac_mantel_pearson(x_condensed, y_condensed, n_samples: int, perms, stream=None, _entry="unifrac_mantel_pearson"):
     """Mantel test (Pearson) on two condensed CUDA tensors (both float32 or both float64); perms: CUDA int32 [K, n].
     Returns a CUDA float64 tensor [4 + K]: r, p two-sided, p greater, p less, r_1 .. r_K.  Asynchronous on the stream."""
     import torch
@@ -211,7 +218,7 @@ def unifrac_mantel_pearson(x_condensed, y_condensed, n_samples: int, perms, stre
     with torch.cuda.device(dev):
         s = stream if stream is not None else torch.cuda.current_stream(dev)
         with torch.cuda.stream(s):
-            rc = lib.unifrac_mantel_pearson(n, x_condensed.data_ptr(), y_condensed.data_ptr(),
+            rc = getattr(lib, _entry)(n, x_condensed.data_ptr(), y_condensed.data_ptr(),
                                             FP32 if x_condensed.dtype == torch.float32 else FP64,
                                             perms.data_ptr() if K else None, K, out.data_ptr(), cb, None,
                                             C.c_void_p(s.cuda_stream))

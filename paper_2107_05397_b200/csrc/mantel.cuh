@@ -22,14 +22,17 @@ __device__ __forceinline__ double warp_sum(double v) {
     return v;
 }
 
-// moments over the condensed vectors: out[0..4] += {sum x, sum y, sum x^2, sum y^2, sum x y}
+// moments over the condensed vectors, SHIFTED by the first elements x0 = x[0], y0 = y[0] (a constant vector then sums to
+// exactly 0, and the variances below lose no digits to the mean):
+//   out[0..4] += {sum (x - x0), sum (y - y0), sum (x - x0)^2, sum (y - y0)^2, sum (x - x0)(y - y0)}
 template <typename T>
 __global__ void __launch_bounds__(256)
 k_mantel_moments(const T* __restrict__ x, const T* __restrict__ y, unsigned long long P, double* __restrict__ out)
 {
     double s[5] = {0, 0, 0, 0, 0};
+    const double x0 = (double)x[0], y0 = (double)y[0];
     for (unsigned long long k = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; k < P; k += (unsigned long long)gridDim.x * blockDim.x) {
-        const double a = (double)x[k], b = (double)y[k];
+        const double a = (double)x[k] - x0, b = (double)y[k] - y0;
         s[0] += a; s[1] += b; s[2] += a * a; s[3] += b * b; s[4] += a * b;
     }
     __shared__ double part[5][8];
@@ -138,12 +141,17 @@ k_mantel_perm(const T* __restrict__ Xs, long long pitch, const T* __restrict__ y
 }
 
 // out[0] = r, out[1..3] = p two-sided / greater / less, out[4 + k] = r_k (k = 0 .. K-1)
-__global__ void k_mantel_final(const double* __restrict__ mom, const double* __restrict__ S, int K, double P, double* __restrict__ out)
+// S[k] = sum of the raw products x^pi y;  mom = the shifted moments of k_mantel_moments, (x0, y0) the shifts.
+template <typename T>
+__global__ void k_mantel_final(const double* __restrict__ mom, const double* __restrict__ S, int K, double P, const T* __restrict__ x,
+                               const T* __restrict__ y, double* __restrict__ out)
 {
-    const double sx = mom[0], sy = mom[1], sxx = mom[2], syy = mom[3];
-    const double vx = sxx - sx * sx / P, vy = syy - sy * sy / P;
+    const double x0 = (double)x[0], y0 = (double)y[0];
+    const double dx = mom[0], dy = mom[1];                         // sum (x - x0), sum (y - y0)
+    const double vx = mom[2] - dx * dx / P, vy = mom[3] - dy * dy / P;
+    const double sx = dx + P * x0, sy = dy + P * y0;               // plain sums
     const double den = sqrt(vx * vy);
-    auto corr = [&](double sxy) { return den > 0.0 ? (sxy - sx * sy / P) / den : 0.0; };
+    auto corr = [&](double sxy) { return (vx > 0.0 && vy > 0.0 && den > 0.0) ? (sxy - sx * sy / P) / den : 0.0; };
     const double r = corr(S[0]);
     int two = 0, gr = 0, le = 0;
     for (int k = threadIdx.x; k < K; k += blockDim.x) {

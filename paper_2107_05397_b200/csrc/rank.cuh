@@ -1,0 +1,208 @@
+// rank.cuh -- average-rank transform of a condensed distance vector, for the Spearman variant of the Mantel test
+// ("... or Spearman's rank correlation coefficient"; "the Spearman variety requires about 18
+// minutes", readings M5-M6).  Spearman's rho is Pearson's r of the RANKS, ties sharing the mean of the
+// ranks they span, so the device path is: a stable LSD radix sort of (key, position) pairs -- hand-written, 8-bit digits,
+// no cub / thrust --, a prefix-max scan that gives every sorted position the start of its run of equal keys, and a scatter
+// of  rank = start + (run length - 1) / 2 + 1  (1-based, fp64: half-integers up to 2^32 are exact) back to the original
+// positions.  k_mantel_perm (mantel.cuh) then runs unchanged on the two rank vectors.
+// Bound: HBM.  One pass moves 4 + 8 + 8 bytes per element (histogram read, scatter read + write of key and position).
+#pragma once
+#include "common.cuh"
+
+namespace ufb {
+
+constexpr int RADIX_THREADS = 256;
+constexpr int RADIX_ITEMS = 16;                         // per thread and tile: warp w owns 512 consecutive elements
+constexpr int RADIX_TILE = RADIX_THREADS * RADIX_ITEMS; // 4096
+constexpr int RADIX_WARPS = RADIX_THREADS / 32;
+
+template <typename T> struct RankKey;
+template <> struct RankKey<float> {
+    using K = uint32_t;
+    static constexpr int PASSES = 4;
+    // order-preserving map of IEEE floats to unsigned integers; -0 is folded onto +0 so that equal VALUES are equal KEYS
+    __device__ static __forceinline__ K make(float v) {
+        const uint32_t u = __float_as_uint(v + 0.0f);
+        return u ^ ((u >> 31) ? 0xffffffffu : 0x80000000u);
+    }
+};
+template <> struct RankKey<double> {
+    using K = unsigned long long;
+    static constexpr int PASSES = 8;
+    __device__ static __forceinline__ K make(double v) {
+        const unsigned long long u = (unsigned long long)__double_as_longlong(v + 0.0);
+        return u ^ ((u >> 63) ? 0xffffffffffffffffull : 0x8000000000000000ull);
+    }
+};
+
+// block b owns the contiguous element range [b * per_block, min(P, (b + 1) * per_block)), per_block a multiple of RADIX_TILE
+__device__ __forceinline__ void radix_range(unsigned long long P, unsigned long long per_block, unsigned long long& lo, unsigned long long& hi) {
+    lo = (unsigned long long)blockIdx.x * per_block;
+    hi = lo + per_block;
+    if (lo > P) lo = P;
+    if (hi > P) hi = P;
+}
+
+// hist[d * gridDim.x + b] = number of elements of block b's range whose digit (key >> shift) & 255 is d
+template <typename T, bool FIRST>
+__global__ void __launch_bounds__(RADIX_THREADS)
+k_radix_hist(const T* __restrict__ raw, const typename RankKey<T>::K* __restrict__ keys, unsigned long long P,
+             unsigned long long per_block, int shift, uint32_t* __restrict__ hist)
+{
+    using K = typename RankKey<T>::K;
+    __shared__ uint32_t h[256];
+    h[threadIdx.x] = 0;
+    __syncthreads();
+    unsigned long long lo, hi;
+    radix_range(P, per_block, lo, hi);
+    const int lane = threadIdx.x & 31;
+    for (unsigned long long base = lo; base < hi; base += RADIX_THREADS) {
+        const unsigned long long e = base + threadIdx.x;
+        const bool ok = e < hi;
+        K k = 0;
+        if (ok) k = FIRST ? RankKey<T>::make(raw[e]) : keys[e];
+        const uint32_t d = ok ? (uint32_t)((k >> shift) & 255u) : 256u;            // 256 = the inactive lanes' own group
+        const uint32_t peers = __match_any_sync(0xffffffffu, d);
+        if (ok && lane == __ffs(peers) - 1) atomicAdd(&h[d], (uint32_t)__popc(peers));
+    }
+    __syncthreads();
+    hist[(size_t)threadIdx.x * gridDim.x + blockIdx.x] = h[threadIdx.x];
+}
+
+// stable scatter of one digit: offs = exclusive scan of hist (digit-major), i.e. the global position of the first element
+// of block b with digit d.  Tiles of the block's range are processed in order; within a tile warp w owns 512 consecutive
+// elements and handles them in 16 rounds of 32 (lane order = element order), so equal digits keep their input order.
+template <typename T, bool FIRST>
+__global__ void __launch_bounds__(RADIX_THREADS)
+k_radix_scatter(const T* __restrict__ raw, const typename RankKey<T>::K* __restrict__ keys_in, const uint32_t* __restrict__ idx_in,
+                unsigned long long P, unsigned long long per_block, int shift, const uint32_t* __restrict__ offs,
+                typename RankKey<T>::K* __restrict__ keys_out, uint32_t* __restrict__ idx_out)
+{
+    using K = typename RankKey<T>::K;
+    __shared__ uint32_t gbase[256];
+    __shared__ uint32_t wh[RADIX_WARPS][256];
+    gbase[threadIdx.x] = offs[(size_t)threadIdx.x * gridDim.x + blockIdx.x];
+    unsigned long long lo, hi;
+    radix_range(P, per_block, lo, hi);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t lt = (1u << lane) - 1u;
+    for (unsigned long long tile = lo; tile < hi; tile += RADIX_TILE) {
+        for (int w = 0; w < RADIX_WARPS; ++w) wh[w][threadIdx.x] = 0;
+        __syncthreads();
+        K k[RADIX_ITEMS];
+        uint32_t id[RADIX_ITEMS];
+        const unsigned long long wbase = tile + (unsigned long long)warp * (32 * RADIX_ITEMS) + lane;
+#pragma unroll
+        for (int r = 0; r < RADIX_ITEMS; ++r) {
+            const unsigned long long e = wbase + (unsigned long long)r * 32;
+            if (e < hi) {
+                if (FIRST) { k[r] = RankKey<T>::make(raw[e]); id[r] = (uint32_t)e; }
+                else { k[r] = keys_in[e]; id[r] = idx_in[e]; }
+            } else { k[r] = 0; id[r] = 0; }
+        }
+        // per-warp digit counts
+#pragma unroll
+        for (int r = 0; r < RADIX_ITEMS; ++r) {
+            const bool ok = wbase + (unsigned long long)r * 32 < hi;
+            const uint32_t d = ok ? (uint32_t)((k[r] >> shift) & 255u) : 256u;
+            const uint32_t peers = __match_any_sync(0xffffffffu, d);
+            if (ok && lane == __ffs(peers) - 1) wh[warp][d] += (uint32_t)__popc(peers);
+            __syncwarp();
+        }
+        __syncthreads();
+        {   // thread d: positions of digit d for warp 0, 1, ... of this tile, then the block's running offset moves on
+            uint32_t run = gbase[threadIdx.x];
+            for (int w = 0; w < RADIX_WARPS; ++w) { const uint32_t t = wh[w][threadIdx.x]; wh[w][threadIdx.x] = run; run += t; }
+            gbase[threadIdx.x] = run;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int r = 0; r < RADIX_ITEMS; ++r) {
+            const bool ok = wbase + (unsigned long long)r * 32 < hi;
+            const uint32_t d = ok ? (uint32_t)((k[r] >> shift) & 255u) : 256u;
+            const uint32_t peers = __match_any_sync(0xffffffffu, d);
+            if (ok) {
+                const uint32_t pos = wh[warp][d] + (uint32_t)__popc(peers & lt);
+                keys_out[pos] = k[r];
+                idx_out[pos] = id[r];
+            }
+            __syncwarp();
+            if (ok && lane == __ffs(peers) - 1) wh[warp][d] += (uint32_t)__popc(peers);
+            __syncwarp();
+        }
+        __syncthreads();
+    }
+}
+
+// ---- runs of equal keys in the sorted order ---------------------------------------------------------------------------
+// blast[b] = 1 + (last position in block b's range that starts a run), 0 if none
+template <typename K>
+__global__ void __launch_bounds__(RADIX_THREADS)
+k_rank_block_heads(const K* __restrict__ keys, unsigned long long P, unsigned long long per_block, uint32_t* __restrict__ blast)
+{
+    __shared__ uint32_t best;
+    if (threadIdx.x == 0) best = 0;
+    __syncthreads();
+    unsigned long long lo, hi;
+    radix_range(P, per_block, lo, hi);
+    uint32_t mine = 0;
+    for (unsigned long long e = lo + threadIdx.x; e < hi; e += RADIX_THREADS)
+        if (e == 0 || keys[e] != keys[e - 1]) mine = (uint32_t)e + 1u;
+    atomicMax(&best, mine);
+    __syncthreads();
+    if (threadIdx.x == 0) blast[blockIdx.x] = best;
+}
+
+// start[p] = first position of the run of equal keys that p belongs to (prefix maximum of the run-start positions);
+// the last element of every run also records the run's length at rlen[start].
+template <typename K>
+__global__ void __launch_bounds__(RADIX_THREADS)
+k_rank_starts(const K* __restrict__ keys, unsigned long long P, unsigned long long per_block, const uint32_t* __restrict__ blast,
+              uint32_t* __restrict__ start, uint32_t* __restrict__ rlen)
+{
+    __shared__ uint32_t wmax[RADIX_WARPS];
+    __shared__ uint32_t carry_s;
+    unsigned long long lo, hi;
+    radix_range(P, per_block, lo, hi);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) {
+        uint32_t c = 0;
+        for (unsigned b = 0; b < blockIdx.x; ++b) c = max(c, blast[b]);
+        carry_s = c;
+    }
+    __syncthreads();
+    for (unsigned long long base = lo; base < hi; base += RADIX_THREADS) {
+        const unsigned long long e = base + threadIdx.x;
+        const bool ok = e < hi;
+        uint32_t v = 0;                                                   // 1 + start position, 0 = not a run start
+        if (ok && (e == 0 || keys[e] != keys[e - 1])) v = (uint32_t)e + 1u;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, v, o); if (lane >= o) v = max(v, t); }
+        if (lane == 31) wmax[warp] = v;
+        __syncthreads();
+        uint32_t pre = carry_s;
+        for (int w = 0; w < warp; ++w) pre = max(pre, wmax[w]);
+        v = max(v, pre);
+        if (ok) {
+            const uint32_t s = v - 1u;                                    // v >= 1: position 0 always starts a run
+            start[e] = s;
+            if (e + 1 == P || keys[e + 1] != keys[e]) rlen[s] = (uint32_t)e - s + 1u;
+        }
+        __syncthreads();
+        if (threadIdx.x == RADIX_THREADS - 1) carry_s = v;                // inclusive maximum of everything so far
+        __syncthreads();
+    }
+}
+
+// rank[idx[p]] = start[p] + (rlen[start[p]] - 1) / 2 + 1     (1-based average rank, exact in fp64)
+__global__ void __launch_bounds__(256)
+k_rank_write(const uint32_t* __restrict__ idx, const uint32_t* __restrict__ start, const uint32_t* __restrict__ rlen,
+             unsigned long long P, double* __restrict__ rank)
+{
+    for (unsigned long long p = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; p < P; p += (unsigned long long)gridDim.x * blockDim.x) {
+        const uint32_t s = start[p];
+        rank[idx[p]] = (double)s + 0.5 * (double)(rlen[s] - 1u) + 1.0;
+    }
+}
+
+}  // namespace ufb

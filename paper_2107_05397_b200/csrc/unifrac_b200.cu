@@ -12,6 +12,7 @@
 #include "dense.cuh"
 #include "rates.cuh"
 #include "mantel.cuh"
+#include "rank.cuh"
 #include "guard.cuh"
 
 #include <cstdio>
@@ -765,8 +766,57 @@ void run_mantel(int32_t N, const T* x, const T* y, const int32_t* perms, int32_t
             Xs, pitch, y, perms, N, seg, n_split, k0, S);
         CU_LAUNCH();
     }
-    k_mantel_final<<<1, 256, 0, st>>>(mom, S, K, (double)P, out); CU_LAUNCH();
+    k_mantel_final<T><<<1, 256, 0, st>>>(mom, S, K, (double)P, x, y, out); CU_LAUNCH();
     A.release();
+}
+
+// average ranks (fp64, 1-based) of the P values v[] -> rank[]; sort buffers are shared between the two vectors of a call
+struct RankBufs { void* keys[2]; uint32_t* idx[2]; uint32_t* hist; uint32_t* offs; uint32_t* blast; unsigned nb; unsigned long long per_block; };
+template <typename T>
+void rank_transform(const T* v, unsigned long long P, double* rank, const RankBufs& B, cudaStream_t st)
+{
+    using K = typename RankKey<T>::K;
+    K* keys[2] = {reinterpret_cast<K*>(B.keys[0]), reinterpret_cast<K*>(B.keys[1])};
+    int src = 0;                                                     // pass 0 reads v[] itself and writes buffer 0
+    for (int pass = 0; pass < RankKey<T>::PASSES; ++pass) {
+        const int shift = 8 * pass, dst = pass == 0 ? 0 : src ^ 1;
+        if (pass == 0) k_radix_hist<T, true><<<B.nb, RADIX_THREADS, 0, st>>>(v, nullptr, P, B.per_block, shift, B.hist);
+        else k_radix_hist<T, false><<<B.nb, RADIX_THREADS, 0, st>>>(nullptr, keys[src], P, B.per_block, shift, B.hist);
+        CU_LAUNCH();
+        k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>((int)(256 * B.nb), B.hist, B.offs); CU_LAUNCH();
+        if (pass == 0) k_radix_scatter<T, true><<<B.nb, RADIX_THREADS, 0, st>>>(v, nullptr, nullptr, P, B.per_block, shift, B.offs, keys[dst], B.idx[dst]);
+        else k_radix_scatter<T, false><<<B.nb, RADIX_THREADS, 0, st>>>(nullptr, keys[src], B.idx[src], P, B.per_block, shift, B.offs, keys[dst], B.idx[dst]);
+        CU_LAUNCH();
+        src = dst;
+    }
+    uint32_t* start = reinterpret_cast<uint32_t*>(keys[src ^ 1]);     // the other key buffer and position buffer are free now
+    uint32_t* rlen = B.idx[src ^ 1];
+    k_rank_block_heads<K><<<B.nb, RADIX_THREADS, 0, st>>>(keys[src], P, B.per_block, B.blast); CU_LAUNCH();
+    k_rank_starts<K><<<B.nb, RADIX_THREADS, 0, st>>>(keys[src], P, B.per_block, B.blast, start, rlen); CU_LAUNCH();
+    k_rank_write<<<B.nb * 4, 256, 0, st>>>(B.idx[src], start, rlen, P, rank); CU_LAUNCH();
+}
+
+template <typename T>
+void run_spearman(int32_t N, const T* x, const T* y, const int32_t* perms, int32_t K, double* out, Arena& A, cudaStream_t st)
+{
+    const unsigned long long P = (unsigned long long)N * (N - 1) / 2;
+    if (P >= (1ull << 32) - 1) throw StatusFail{UNIFRAC_ERR_UNSUPPORTED};      // positions and ranks are kept in 32 bits
+    int dev = 0, n_sm = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    RankBufs B{};
+    B.nb = (unsigned)n_sm * 8;
+    B.per_block = ((P + B.nb - 1) / B.nb + RADIX_TILE - 1) / RADIX_TILE * RADIX_TILE;
+    const size_t ksz = sizeof(typename RankKey<T>::K);
+    for (int i = 0; i < 2; ++i) { B.keys[i] = A.get(P * ksz); B.idx[i] = A.get_n<uint32_t>(P); }
+    B.hist = A.get_n<uint32_t>((size_t)256 * B.nb + 1);
+    B.offs = A.get_n<uint32_t>((size_t)256 * B.nb + 1);
+    B.blast = A.get_n<uint32_t>(B.nb);
+    double* rx = A.get_n<double>(P);
+    double* ry = A.get_n<double>(P);
+    rank_transform<T>(x, P, rx, B, st);
+    rank_transform<T>(y, P, ry, B, st);
+    run_mantel<double>(N, rx, ry, perms, K, out, A, st);
 }
 }  // namespace
 
@@ -880,6 +930,28 @@ int unifrac_mantel_pearson(int32_t N, const void* x, const void* y, unifrac_prec
         snprintf(b, sizeof(b), "%s: %s (unifrac_b200.cu:%d)", f.what, cudaGetErrorString(f.e), f.line);
         g_cuda_err = b; cudaGetLastError(); rc = UNIFRAC_ERR_CUDA;
     } catch (const WorkspaceFail&) { rc = UNIFRAC_ERR_WORKSPACE; }
+    catch (...) { rc = UNIFRAC_ERR_CUDA; g_cuda_err = "unexpected C++ exception"; }
+    if (rc != UNIFRAC_OK) A.release();
+    return rc;
+}
+
+int unifrac_mantel_spearman(int32_t N, const void* x, const void* y, unifrac_precision_t precision, const int32_t* perms,
+                            int32_t K, double* out, unifrac_alloc_fn alloc, void* user, void* stream)
+{
+    if (!x || !y || !out || K < 0 || (K > 0 && !perms) || N < 3) return UNIFRAC_ERR_INVALID_ARG;
+    if (precision != UNIFRAC_FP32 && precision != UNIFRAC_FP64) return UNIFRAC_ERR_INVALID_ARG;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    Arena A{alloc, user, st};
+    int rc = UNIFRAC_OK;
+    try {
+        if (precision == UNIFRAC_FP32) run_spearman<float>(N, reinterpret_cast<const float*>(x), reinterpret_cast<const float*>(y), perms, K, out, A, st);
+        else run_spearman<double>(N, reinterpret_cast<const double*>(x), reinterpret_cast<const double*>(y), perms, K, out, A, st);
+    } catch (const CudaFail& f) {
+        char b[512];
+        snprintf(b, sizeof(b), "%s: %s (unifrac_b200.cu:%d)", f.what, cudaGetErrorString(f.e), f.line);
+        g_cuda_err = b; cudaGetLastError(); rc = UNIFRAC_ERR_CUDA;
+    } catch (const WorkspaceFail&) { rc = UNIFRAC_ERR_WORKSPACE; }
+    catch (const StatusFail& s) { rc = s.status; }
     catch (...) { rc = UNIFRAC_ERR_CUDA; g_cuda_err = "unexpected C++ exception"; }
     if (rc != UNIFRAC_OK) A.release();
     return rc;
