@@ -215,6 +215,27 @@ int unifrac_mantel_spearman(int32_t n_samples, const void *x_condensed, const vo
                             unifrac_precision_t precision, const int32_t *perms, int32_t n_perms, double *out,
                             unifrac_alloc_fn alloc, void *alloc_user, void *stream);
 
+/*
+ * unifrac_pcoa -- principal coordinates analysis of a distance matrix that is already resident in HBM ("researchers
+ * often apply principal coordinates analysis (PCoA)"; "PCoA can also be computed as part of the Hybrid UniFrac
+ * compute itself").  Classical scaling (readings P1-P5): A = -1/2 D o D, B = Gower-centred A,
+ * leading eigenpairs (lambda_i, v_i) of B in descending order, coordinates of axis i = v_i sqrt(lambda_i), proportion
+ * explained = lambda_i / trace(B).
+ *   d_condensed  DEVICE; n(n-1)/2 float or double (the layout unifrac_dm writes), read-only
+ *   k            number of axes, 1 <= k <= 16, k < n
+ *   max_iter     cap on the products B Q of the block subspace iteration (block of 32 vectors); tol: stop when every one of
+ *                the k leading Ritz values moved by <= tol * |value| over the last 4 products (e.g. 200, 1e-9)
+ *   out          DEVICE; 2 k + n k doubles: [k eigenvalues | k proportions explained | n x k coordinates, row-major].
+ *                An eigenvector's sign is arbitrary; axes with a non-positive eigenvalue get zero coordinates.
+ *   iterations   HOST, optional: products used.
+ * The only O(n^2) work is Y = B Q: a hand-written tcgen05 kind::tf32 GEMM with a 3-term hi/lo split (fp32 accumulation in
+ * TMEM); orthonormalisation and the 32 x 32 Rayleigh-Ritz step are fp64.  Workspace: 8 n^2 bytes (B as two fp32 matrices).
+ * Eigenvalues of well-separated axes agree with a full fp64 eigendecomposition to ~1e-6 relative.  The call synchronises the
+ * stream (it reads the Ritz values back to test convergence).  n < 3, k out of range: UNIFRAC_ERR_INVALID_ARG.
+ */
+int unifrac_pcoa(int32_t n_samples, const void *d_condensed, unifrac_precision_t precision, int32_t k, int32_t max_iter,
+                 double tol, double *out, int32_t *iterations, unifrac_alloc_fn alloc, void *alloc_user, void *stream);
+
 /* Device-rate probes (not on the data path): what this GPU retires per second of the two atomic units of work the
  * sparse kernels are made of; they are the constants of the head / mid / tail cost model and the `peak` of the
  * k_mid / k_tail_scatter rooflines in bench.py.  Runs ~20 ms of probe kernels on `stream` and synchronises it. */

@@ -24,7 +24,7 @@ OK = 0
 ERR_INVALID_ARG, ERR_INVALID_TREE, ERR_INVALID_TABLE, ERR_EMPTY_SAMPLE = -1, -2, -3, -4
 ERR_WORKSPACE, ERR_CUDA, ERR_UNSUPPORTED = -5, -6, -7
 
-EXPORTS = ("unifrac_dm", "unifrac_dm_shard", "unifrac_shard_of_pair", "unifrac_dm_host", "unifrac_mantel_pearson", "unifrac_mantel_spearman", "unifrac_measure_rates", "unifrac_last_stats", "unifrac_status_string",
+EXPORTS = ("unifrac_dm", "unifrac_dm_shard", "unifrac_shard_of_pair", "unifrac_dm_host", "unifrac_mantel_pearson", "unifrac_mantel_spearman", "unifrac_pcoa", "unifrac_measure_rates", "unifrac_last_stats", "unifrac_status_string",
            "unifrac_last_cuda_error", "unifrac_abi_version")
 
 
@@ -94,6 +94,9 @@ def load(build_if_missing: bool = True) -> C.CDLL:
                                            ALLOC_FN, C.c_void_p, C.c_void_p]
     lib.unifrac_mantel_spearman.restype = C.c_int
     lib.unifrac_mantel_spearman.argtypes = lib.unifrac_mantel_pearson.argtypes
+    lib.unifrac_pcoa.restype = C.c_int
+    lib.unifrac_pcoa.argtypes = [C.c_int32, C.c_void_p, C.c_int, C.c_int32, C.c_int32, C.c_double, C.c_void_p,
+                                 C.POINTER(C.c_int32), ALLOC_FN, C.c_void_p, C.c_void_p]
     lib.unifrac_measure_rates.restype = C.c_int
     lib.unifrac_measure_rates.argtypes = [C.POINTER(Rates), C.c_void_p]
     lib.unifrac_last_stats.restype = C.c_int
@@ -225,6 +228,38 @@ def unifrac_mantel_pearson(x_condensed, y_condensed, n_samples: int, perms, stre
     del held
     _check(lib, rc)
     return out
+
+
+def unifrac_pcoa(d_condensed, n_samples: int, k: int, max_iter: int = 200, tol: float = 1e-7, stream=None):
+    """PCoA of a condensed CUDA distance vector (float32 / float64).  Returns (eigenvalues[k], proportion[k], coords[n, k])
+    as CUDA float64 tensors and the number of B Q products used."""
+    import torch
+    lib = load()
+    dev = d_condensed.device
+    n, k = int(n_samples), int(k)
+    assert dev.type == "cuda" and d_condensed.is_contiguous() and d_condensed.dtype in (torch.float32, torch.float64)
+    assert d_condensed.numel() == n * (n - 1) // 2
+    out = torch.empty(2 * k + n * k, dtype=torch.float64, device=dev)
+    held = []
+
+    def _alloc(nbytes, _user):
+        try:
+            t = torch.empty(int(nbytes), dtype=torch.uint8, device=dev)
+        except Exception:
+            return None
+        held.append(t)
+        return t.data_ptr()
+
+    cb = ALLOC_FN(_alloc)
+    its = C.c_int32(0)
+    with torch.cuda.device(dev):
+        s = stream if stream is not None else torch.cuda.current_stream(dev)
+        with torch.cuda.stream(s):
+            rc = lib.unifrac_pcoa(n, d_condensed.data_ptr(), FP32 if d_condensed.dtype == torch.float32 else FP64, k,
+                                  int(max_iter), float(tol), out.data_ptr(), C.byref(its), cb, None, C.c_void_p(s.cuda_stream))
+    del held
+    _check(lib, rc)
+    return out[:k], out[k:2 * k], out[2 * k:].view(n, k), int(its.value)
 
 
 def unifrac_measure_rates(stream=None) -> dict:

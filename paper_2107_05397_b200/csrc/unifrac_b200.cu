@@ -13,6 +13,7 @@
 #include "rates.cuh"
 #include "mantel.cuh"
 #include "rank.cuh"
+#include "pcoa.cuh"
 #include "guard.cuh"
 
 #include <cstdio>
@@ -818,6 +819,78 @@ void run_spearman(int32_t N, const T* x, const T* y, const int32_t* perms, int32
     rank_transform<T>(y, P, ry, B, st);
     run_mantel<double>(N, rx, ry, perms, K, out, A, st);
 }
+
+// PCoA: block subspace iteration with Rayleigh-Ritz (pcoa.cuh).  Synchronous: the Ritz values are read back every
+// PCOA_CHECK products to test convergence.
+constexpr int PCOA_CHECK = 4;
+template <typename T>
+void run_pcoa(int32_t N, const T* d, int32_t k, int32_t max_iter, double tol, double* out, int32_t* iters_out, Arena& A, cudaStream_t st)
+{
+    const long long n_pad = ((long long)N + 127) / 128 * 128;
+    int dev = 0, n_sm = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    float* Bhi = A.get_n<float>((size_t)n_pad * n_pad);
+    float* Blo = A.get_n<float>((size_t)n_pad * n_pad);
+    double* rs = A.get_n<double>((size_t)N + 1);
+    double* tot = rs + N;
+    float* Y = A.get_n<float>((size_t)n_pad * PCOA_NB);
+    float* Q = A.get_n<float>((size_t)n_pad * PCOA_NB);
+    float* Qt_hi = A.get_n<float>((size_t)n_pad * PCOA_NB);
+    float* Qt_lo = A.get_n<float>((size_t)n_pad * PCOA_NB);
+    double* G = A.get_n<double>(1024);
+    double* Rinv = A.get_n<double>(1024);
+    double* W = A.get_n<double>(1024);
+    double* lam = A.get_n<double>(32);
+    CU(cudaMemsetAsync(tot, 0, sizeof(double), st));
+    const unsigned nb32 = (unsigned)(n_pad / 32);
+    k_pcoa_square<T><<<dim3(nb32, nb32), dim3(32, 8), 0, st>>>(d, N, n_pad, Bhi); CU_LAUNCH();
+    k_pcoa_rowsum<<<cdiv((long long)N * 32, 256), 256, 0, st>>>(Bhi, N, n_pad, rs, tot); CU_LAUNCH();
+    k_pcoa_center<<<(unsigned)((n_pad * n_pad / 4 + 255) / 256), 256, 0, st>>>(Bhi, Blo, N, n_pad, rs, tot); CU_LAUNCH();
+    double h_tot = 0.0;
+    CU(cudaMemcpyAsync(&h_tot, tot, sizeof(double), cudaMemcpyDeviceToHost, st));
+    CUtensorMap tmBhi = make_rowmajor_map(Bhi, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (uint64_t)n_pad, (uint64_t)n_pad, PCOA_BK, 128, CU_TENSOR_MAP_SWIZZLE_128B);
+    CUtensorMap tmBlo = make_rowmajor_map(Blo, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (uint64_t)n_pad, (uint64_t)n_pad, PCOA_BK, 128, CU_TENSOR_MAP_SWIZZLE_128B);
+    CUtensorMap tmQhi = make_rowmajor_map(Qt_hi, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (uint64_t)n_pad, PCOA_NB, PCOA_BK, PCOA_NB, CU_TENSOR_MAP_SWIZZLE_128B);
+    CUtensorMap tmQlo = make_rowmajor_map(Qt_lo, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (uint64_t)n_pad, PCOA_NB, PCOA_BK, PCOA_NB, CU_TENSOR_MAP_SWIZZLE_128B);
+    CU(cudaFuncSetAttribute(k_pcoa_gemm, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)PCOA_SMEM));
+    const unsigned gblocks = (unsigned)std::min<long long>(n_sm, n_pad / 32);
+    auto orth = [&]() {                                   // Q = orth(Y): Cholesky QR (fp64)
+        CU(cudaMemsetAsync(G, 0, sizeof(double) * 1024, st));
+        k_pcoa_gram32<<<gblocks, dim3(32, 32), 0, st>>>(Y, Y, n_pad, G); CU_LAUNCH();
+        k_pcoa_chol<<<1, 32, 0, st>>>(G, Rinv); CU_LAUNCH();
+        k_pcoa_apply<<<(unsigned)std::min<long long>(n_sm * 2, (n_pad + 255) / 256), 256, 0, st>>>(Y, Rinv, n_pad, Q, Qt_hi, Qt_lo); CU_LAUNCH();
+    };
+    k_pcoa_init<<<(unsigned)((n_pad * PCOA_NB + 255) / 256), 256, 0, st>>>(Y, N, n_pad); CU_LAUNCH();
+    orth();
+    std::swap(Y, Q);                                      // a second pass (Cholesky QR 2) makes the start block orthonormal to fp32 rounding
+    orth();
+    double h_lam[32], prev[32];
+    for (auto& x : prev) x = 0.0;
+    int it = 0;
+    if (max_iter < 1) max_iter = 1;
+    for (;;) {
+        k_pcoa_gemm<<<(unsigned)(n_pad / 128), PCOA_THREADS, PCOA_SMEM, st>>>(tmBhi, tmBlo, tmQhi, tmQlo, (uint32_t)n_pad, Y); CU_LAUNCH();
+        ++it;
+        if (it % PCOA_CHECK == 0 || it >= max_iter) {
+            CU(cudaMemsetAsync(G, 0, sizeof(double) * 1024, st));
+            k_pcoa_gram32<<<gblocks, dim3(32, 32), 0, st>>>(Q, Y, n_pad, G); CU_LAUNCH();
+            k_pcoa_jacobi<<<1, 32, 0, st>>>(G, lam, W); CU_LAUNCH();
+            CU(cudaMemcpyAsync(h_lam, lam, sizeof(h_lam), cudaMemcpyDeviceToHost, st));
+            CU(cudaStreamSynchronize(st));
+            bool conv = true;
+            for (int a = 0; a < k; ++a) conv = conv && fabs(h_lam[a] - prev[a]) <= tol * fabs(h_lam[a]);
+            for (int a = 0; a < 32; ++a) prev[a] = h_lam[a];
+            if (conv || it >= max_iter) break;
+        }
+        orth();
+    }
+    CU(cudaStreamSynchronize(st));
+    const double trace = -h_tot / (double)N;              // trace(B) = -(sum of A) / n = (1/n) sum_{i<j} d_ij^2
+    k_pcoa_coords<<<(unsigned)(((long long)N * k + 255) / 256), 256, 0, st>>>(Q, lam, W, N, k, trace, out); CU_LAUNCH();
+    if (iters_out) *iters_out = it;
+    A.release();
+}
 }  // namespace
 
 extern "C" {
@@ -946,6 +1019,29 @@ int unifrac_mantel_spearman(int32_t N, const void* x, const void* y, unifrac_pre
     try {
         if (precision == UNIFRAC_FP32) run_spearman<float>(N, reinterpret_cast<const float*>(x), reinterpret_cast<const float*>(y), perms, K, out, A, st);
         else run_spearman<double>(N, reinterpret_cast<const double*>(x), reinterpret_cast<const double*>(y), perms, K, out, A, st);
+    } catch (const CudaFail& f) {
+        char b[512];
+        snprintf(b, sizeof(b), "%s: %s (unifrac_b200.cu:%d)", f.what, cudaGetErrorString(f.e), f.line);
+        g_cuda_err = b; cudaGetLastError(); rc = UNIFRAC_ERR_CUDA;
+    } catch (const WorkspaceFail&) { rc = UNIFRAC_ERR_WORKSPACE; }
+    catch (const StatusFail& s) { rc = s.status; }
+    catch (...) { rc = UNIFRAC_ERR_CUDA; g_cuda_err = "unexpected C++ exception"; }
+    if (rc != UNIFRAC_OK) A.release();
+    return rc;
+}
+
+int unifrac_pcoa(int32_t N, const void* d, unifrac_precision_t precision, int32_t k, int32_t max_iter, double tol, double* out,
+                 int32_t* iterations, unifrac_alloc_fn alloc, void* user, void* stream)
+{
+    if (!d || !out || N < 3 || k < 1 || k > 16 || k >= N || !(tol >= 0.0)) return UNIFRAC_ERR_INVALID_ARG;
+    if (precision != UNIFRAC_FP32 && precision != UNIFRAC_FP64) return UNIFRAC_ERR_INVALID_ARG;
+    if ((long long)N > (1ll << 20)) return UNIFRAC_ERR_UNSUPPORTED;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    Arena A{alloc, user, st};
+    int rc = UNIFRAC_OK;
+    try {
+        if (precision == UNIFRAC_FP32) run_pcoa<float>(N, reinterpret_cast<const float*>(d), k, max_iter, tol, out, iterations, A, st);
+        else run_pcoa<double>(N, reinterpret_cast<const double*>(d), k, max_iter, tol, out, iterations, A, st);
     } catch (const CudaFail& f) {
         char b[512];
         snprintf(b, sizeof(b), "%s: %s (unifrac_b200.cu:%d)", f.what, cudaGetErrorString(f.e), f.line);
