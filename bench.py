@@ -2,14 +2,17 @@
 """bench.py -- UniFrac all-pairs hot path on B200.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload emp|large|medium|small|tiny]
-                    [--impl ours|reference] [--no-cpu-baseline] [--no-e2e]
+                    [--impl ours|reference] [--no-cpu-baseline] [--no-e2e] [--no-emp] [--replicas]
 
 A "step" is one pass of the whole hot path (plan, embedding, stripe accumulation, finalize) for
 every variant the workload lists (unweighted and weighted-normalized), inputs resident in HBM.
 metric = dense-equivalent sample-pair x branch updates per second  (BASELINE.json "metric"):
          sum over the step's calls of P * B_emb, divided by the step time.
-Prints ONE JSON line (rank 0).  N > 1: one process per GPU, independent replicas (the path runs on
-one GPU), barrier + max-over-ranks timing, value = all ranks' updates / time.
+Prints ONE JSON line (rank 0).  The default workload is Large (N = 50,000); before it the EMP-shaped workload
+(N = 25,000) runs for max(1, steps/4) steps and is reported under "wall_emp" (BASELINE.json's metric names both sizes).
+N > 1: one process per GPU computing disjoint SHARDS of one matrix (unifrac_dm_shard) followed, inside the timed
+region, by the NCCL merge of the shard buffers (strong scaling); --replicas gives independent replicas instead (weak).
+Barrier + max-over-ranks timing either way.
 """
 from __future__ import annotations
 
@@ -36,9 +39,11 @@ ALU_PEAK_TFLOPS = SM_COUNT * FP32_LANES * SM_MAX_GHZ / 1e3    # FADD/FMNMX-class
 # lane-ops/clk/SM, independent of bank conflicts; 1.94e11 L2-resident scattered fp32 REDs/s)
 SMEM_ATOMIC_PER_S, L2_RED_PER_S = 8.84 * SM_COUNT * SM_MAX_GHZ * 1e9, 1.94e11
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full captures of profiles/r01_summary.md
-# (default flags, seed 0; k_mid: mean of the unweighted and the weighted launch); other workloads: null
-NCU_TRAFFIC_BYTES = {"large": {"k_dense16": 308.4e9, "k_gram": 300.1e9, "k_mid": 240.2e9, "k_tail_scatter": 0.227e9}}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch, copied from the ncu --set full captures summarised in the file
+# TRAFFIC_SOURCE names (default flags, seed 0; k_mid: mean of the unweighted and the weighted launch); not measured by this
+# run -- other workloads and kernels that changed since the capture report null
+TRAFFIC_SOURCE = "profiles/r01_summary.md (ncu --set full, round-1 kernels)"
+NCU_TRAFFIC_BYTES = {"large": {"k_gram": 300.1e9, "k_mid": 240.2e9}}
 
 WORKLOADS = {   # name -> (variants, precision)    BASELINE.json:7-11
     "tiny": ((0, 1), 1), "small": ((0, 1), 1), "medium": ((0,), 0), "emp": ((0, 1), 0), "large": ((0, 1), 0),
@@ -124,6 +129,109 @@ def oracle_leg(p, variants, budget_s, seed=0):
                        f"(includes building the per-sample branch lists)")
 
 
+def cpu_model_name():
+    try:
+        for ln in open("/proc/cpuinfo"):
+            if ln.startswith("model name"):
+                return ln.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def variant_name(v):
+    return "unweighted" if v == 0 else "weighted_normalized"
+
+
+def wall_of(all_stats, variants, n_nodes, nnz):
+    """Per-variant wall time split and derived figures."""
+    per_variant = {}
+    for k, v in enumerate(variants):
+        ss = [st[k] for st in all_stats]
+        mean = lambda key: float(np.mean([s[key] for s in ss]))
+        s0 = ss[0]
+        t_a5 = (mean("ms_tail") + mean("ms_mid") + mean("ms_stripe")) * 1e-3
+        n_words = (s0["n_samples"] + 31) // 32 if "n_samples" in s0 else 0
+        # algorithmic bytes of a-1 .. a-4 (estimate from the list sizes): CSR read, presence bits written + read once,
+        # sparse (sample, value) entries written (+ integer counts written and read for the weighted variant)
+        embed_bytes = nnz * 8.0 + 2.0 * n_nodes * n_words * 4 + s0["tail_entries"] * (8.0 if v == 0 else 16.0)
+        per_variant[variant_name(v)] = dict(
+            ms_total=mean("ms_total"), ms_plan=mean("ms_plan"), ms_embed=mean("ms_embed"), ms_tail=mean("ms_tail"),
+            ms_mid=mean("ms_mid"), ms_stripe=mean("ms_stripe"),
+            algorithmic_frac=(2.0 * s0["updates_inter"] / (ALU_PEAK_TFLOPS * 1e12) / t_a5) if t_a5 > 0 else None,
+            updates_executed_per_s=(s0["updates_executed"] / t_a5) if t_a5 > 0 else None,
+            embed_gbs=(embed_bytes / (mean("ms_embed") * 1e-3) / 1e9) if mean("ms_embed") > 0 else None,
+            mid_rows=s0["mid_rows"], mid_updates=s0["mid_updates"], mid_F=s0["mid_F"],
+            head_rows=s0["head_rows"], tail_rows=s0["tail_rows"], tail_updates=s0["tail_updates"],
+            gram=s0["gram"], gram_k=s0["gram_k"], gram_q=s0["gram_q"], guard_pairs=s0["guard_pairs"],
+            tail_entries=s0["tail_entries"], tail_launches=s0["tail_launches"],
+            updates_executed_head=s0["updates_executed_head"], updates_dense=s0["updates_dense"],
+            updates_executed=s0["updates_executed"], updates_union=s0["updates_union"], updates_inter=s0["updates_inter"],
+            branches_embedded=s0["branches_embedded"], workspace_gb=s0["workspace_bytes"] / 2**30)
+    return per_variant
+
+
+def parity_check(p, variants, outs, n_pairs=2000, seed=3):
+    """max / p99.99 relative error of resident outputs against the oracle on a seeded pair sample."""
+    import torch
+    from oracle import oracle
+    pairs = synth.sample_pairs(p.n_samples, n_pairs, seed=seed)
+    idx = torch.from_numpy(synth.condensed_index(p.n_samples, pairs[:, 0], pairs[:, 1])).to(next(iter(outs.values())).device)
+    rels = []
+    for v in variants:
+        want = oracle.pair_list(p.parent, p.branch_len, p.indptr, p.indices, p.counts, v, pairs)
+        got = outs[v][idx].double().cpu().numpy()
+        rels.append(np.abs(got - want) / np.maximum(np.abs(want), 1e-30))
+    rel = np.concatenate(rels)
+    return dict(max_rel=float(rel.max()), p9999_rel=float(np.quantile(rel, 0.9999)), pairs=int(rel.shape[0]),
+                sample=f"{n_pairs} seeded pairs per variant vs the oracle's pair-list driver, after the timed region")
+
+
+def run_workload(binding, torch, dist, p, variants, precision, dev, steps, warmup, flags, shard, world, sampler_gpu=None):
+    """warm-up, then `steps` timed steps (one unifrac_dm[_shard] call per variant [+ the NCCL merge of the shard buffers]),
+    CUDA events on the launch stream, barrier + synchronize on both sides.  Returns (ms, all_stats, outs, clock lines)."""
+    from paper_2107_05397_b200 import multigpu
+    args = binding.to_device(p, dev)
+    outs = {v: torch.empty(p.n_pairs, dtype=torch.float32 if precision == 0 else torch.float64, device=dev) for v in variants}
+
+    def step():
+        stats = []
+        for v in variants:
+            binding.unifrac_dm(*args, p.n_samples, v, precision, out=outs[v], flags=flags, shard=shard)
+            st = binding.unifrac_last_stats()               # waits for the call's stripe kernel (stats event)
+            st["n_samples"] = p.n_samples
+            stats.append(st)
+            if shard:
+                multigpu.merge_shards(outs[v])              # all-reduce(SUM) over NCCL: every pair has one owner
+        return stats
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize(dev)
+
+    for _ in range(warmup):
+        step()
+    barrier()
+    stop, lines = threading.Event(), []
+    th = None
+    if sampler_gpu is not None:
+        th = threading.Thread(target=clocks_sampler, args=(stop, lines, sampler_gpu), daemon=True)
+        th.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    all_stats = []
+    e0.record()
+    for _ in range(steps):
+        all_stats.append(step())
+    e1.record()
+    barrier()
+    stop.set()
+    if th is not None:
+        th.join(timeout=3)
+    return e0.elapsed_time(e1), all_stats, outs, lines, args, barrier
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -136,12 +244,14 @@ def main():
     ap.add_argument("--cpu-budget-s", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-emp", action="store_true", help="skip the EMP-shaped (N = 25,000) leg that precedes the Large workload")
+    ap.add_argument("--no-next", action="store_true", help="skip the Mantel / PCoA legs that follow the timed region")
     ap.add_argument("--mantel-perms", type=int, default=9,
-                    help="after the timed region: Mantel / Pearson test between the unweighted and the weighted matrix with this "
-                         "many permutations (0 = skip); reported under \"mantel\", not part of the step")
-    ap.add_argument("--shard", action="store_true",
-                    help="N > 1: the ranks compute disjoint shards of ONE matrix (unifrac_dm_shard, strong scaling) "
-                         "instead of independent replicas (default, weak scaling)")
+                    help="after the timed region: Mantel test (Pearson, then Spearman) between the unweighted and the weighted "
+                         "matrix with this many permutations (0 = skip); reported under \"mantel\", not part of the step")
+    ap.add_argument("--shard", action="store_true", help="accepted for compatibility: shards are the default for N > 1")
+    ap.add_argument("--replicas", action="store_true",
+                    help="N > 1: independent replicas (weak scaling, no merge) instead of shards of one matrix + NCCL merge")
     a = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -166,78 +276,108 @@ def main():
                     dtype="f64", data="synthetic", impl="reference",
                     config=dict(workload=a.workload, n_samples=p.n_samples, n_nodes=p.n_nodes, nnz=p.nnz, seed=a.seed,
                                 variants=list(variants), step="bounded pair sample of the workload"),
-                    cpu_baseline=dict(value=val, unit=UNIT, cores=timed[0]["cores"], kind="oracle", sample=timed[0]["sample"]),
+                    cpu_baseline=dict(value=val, unit=UNIT, cores=timed[0]["cores"], kind="oracle", sample=timed[0]["sample"],
+                                      cpu_model=cpu_model_name()),
                     e2e=dict(value=val, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
         print(json.dumps(line))
         return 0
 
     # ---------------------------------------------------------------- our arm
-    shard = (rank, world) if (a.shard and world > 1) else None
-    p = synth.make_config(a.workload, seed=a.seed if shard else rank_seed(a.seed, rank))   # generated before CUDA is touched (fork pool)
+    shard = (rank, world) if (world > 1 and not a.replicas) else None
+    seed = a.seed if (shard or world == 1) else rank_seed(a.seed, rank)
+    run_emp = a.workload == "large" and not a.no_emp
+    p_emp = synth.make_config("emp", seed=seed) if run_emp else None     # generated before CUDA is touched (fork pool)
+    p = synth.make_config(a.workload, seed=seed)
     os.environ["UNIFRAC_B200_TIMING"] = "1"
     import torch
     from paper_2107_05397_b200 import binding
     binding.load()
     dev = torch.device("cuda", local_rank)
     torch.cuda.set_device(dev)
+    dist = None
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
-    args = binding.to_device(p, dev)
-    outs = {v: torch.empty(p.n_pairs, dtype=torch.float32 if precision == 0 else torch.float64, device=dev) for v in variants}
 
-    def step():
-        stats = []
-        for v in variants:
-            binding.unifrac_dm(*args, p.n_samples, v, precision, out=outs[v], flags=a.flags, shard=shard)
-            stats.append(binding.unifrac_last_stats())     # waits for the call's stripe kernel (stats event)
-        return stats
+    wall_emp = None
+    launches_emp = 0
+    if run_emp:
+        steps_emp = max(1, a.steps // 4)
+        ms_e, st_e, outs_e, _, args_e, _ = run_workload(binding, torch, dist, p_emp, (0, 1), 0, dev, steps_emp, a.warmup, a.flags,
+                                                         shard, world)
+        ms_e, _ = reduce_over_ranks(ms_e, 0.0, world, dev)
+        wall_emp = dict(n_samples=p_emp.n_samples, n_nodes=p_emp.n_nodes, steps=steps_emp, ms_per_step=ms_e / steps_emp,
+                        **wall_of(st_e, (0, 1), p_emp.n_nodes, p_emp.nnz))
+        if rank == 0:
+            wall_emp["parity"] = parity_check(p_emp, (0, 1), outs_e)
+        launches_emp = int(sum(s["kernel_launches"] for st in st_e for s in st))
+        del outs_e, args_e
+        torch.cuda.empty_cache()
 
-    def barrier():
-        torch.cuda.synchronize(dev)
-        if world > 1:
-            dist.barrier()
-            torch.cuda.synchronize(dev)
-
-    for _ in range(a.warmup):
-        step()
-    barrier()
-    stop, lines = threading.Event(), []
-    th = threading.Thread(target=clocks_sampler, args=(stop, lines, local_rank), daemon=True)
-    th.start()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    all_stats = []
-    e0.record()
-    for _ in range(a.steps):
-        all_stats.append(step())
-    e1.record()
-    barrier()
-    stop.set()
-    th.join(timeout=3)
+    ms, all_stats, outs, lines, args, barrier = run_workload(binding, torch, dist, p, variants, precision, dev, a.steps, a.warmup,
+                                                             a.flags, shard, world, sampler_gpu=local_rank)
     flat = [s for st in all_stats for s in st]
     upd_local = float(sum(s["updates_dense"] for s in flat))
     if shard:
         upd_local /= world               # the ranks share one matrix: its updates are counted once
-    ms, upd_all = reduce_over_ranks(e0.elapsed_time(e1), upd_local, world, dev)
+    ms, upd_all = reduce_over_ranks(ms, upd_local, world, dev)
     value = upd_all / (ms * 1e-3)
+    parity = parity_check(p, variants, outs) if rank == 0 else None      # on the merged matrix when sharded
 
-    # ---------------- next row: Mantel / Pearson between the two variants' matrices, still resident in HBM
-    mantel = None
-    if len(variants) == 2 and a.mantel_perms > 0 and not shard:
+    # ---------------- next rows on the two matrices still resident in HBM; not part of the step
+    mantel = pcoa = None
+    single = world == 1
+    if single and not a.no_next and len(variants) == 2 and a.mantel_perms > 0:
         g = torch.Generator(device=dev).manual_seed(a.seed)
         perms = torch.stack([torch.randperm(p.n_samples, device=dev, generator=g) for _ in range(a.mantel_perms)]).to(torch.int32).contiguous()
-        binding.unifrac_mantel_pearson(outs[variants[0]], outs[variants[1]], p.n_samples, perms)      # warm-up
-        barrier()
-        m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        m0.record()
-        mo = binding.unifrac_mantel_pearson(outs[variants[0]], outs[variants[1]], p.n_samples, perms)
-        m1.record()
-        barrier()
-        m_ms = m0.elapsed_time(m1)
-        alg = (a.mantel_perms + 1) * 2.0 * p.n_pairs * 4            # both condensed matrices once per (permuted) statistic
-        mantel = dict(n_samples=p.n_samples, permutations=a.mantel_perms, ms=m_ms, ms_per_permutation=m_ms / (a.mantel_perms + 1),
-                      r=float(mo[0]), p_two_sided=float(mo[1]), algorithmic_gbs=alg / m_ms / 1e6)
+        def timed(fn):
+            fn()                                                       # warm-up
+            barrier()
+            m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            m0.record()
+            r = fn()
+            m1.record()
+            barrier()
+            return m0.elapsed_time(m1), r
+        x, y = outs[variants[0]], outs[variants[1]]
+        esz = x.element_size()
+        m_ms, mo = timed(lambda: binding.unifrac_mantel_pearson(x, y, p.n_samples, perms))
+        alg = (a.mantel_perms + 1) * 2.0 * p.n_pairs * esz          # both condensed matrices once per (permuted) statistic
+        mantel = dict(n_samples=p.n_samples, permutations=a.mantel_perms,
+                      pearson=dict(ms=m_ms, ms_per_permutation=m_ms / (a.mantel_perms + 1), r=float(mo[0]), p_two_sided=float(mo[1]),
+                                   algorithmic_gbs=alg / m_ms / 1e6))
+        try:
+            s_ms, so = timed(lambda: binding.unifrac_mantel_spearman(x, y, p.n_samples, perms))
+            # the rank transform: 2 vectors x 4 radix passes x (4 + 8 + 8) bytes per element, then the fp64 rank vectors
+            mantel["spearman"] = dict(ms=s_ms, rho=float(so[0]), p_two_sided=float(so[1]),
+                                      ms_rank_transform_and_fp64_statistics=s_ms,
+                                      note="device radix-sort rank transform of both matrices + the same permutation kernel on fp64 ranks")
+        except binding.UnifracError as e:                              # e.g. workspace
+            mantel["spearman"] = dict(error=str(e))
         del perms, mo
+        torch.cuda.empty_cache()
+    if single and not a.no_next:
+        try:
+            x = outs[variants[-1]]
+            def run_pcoa(iters):
+                torch.cuda.synchronize(dev)
+                t0 = time.perf_counter()
+                lam, prop, _, its = binding.unifrac_pcoa(x, p.n_samples, 5, max_iter=iters, tol=0.0)
+                torch.cuda.synchronize(dev)
+                return time.perf_counter() - t0, lam, prop, its
+            run_pcoa(4)
+            t8, _, _, _ = run_pcoa(8)
+            t24, lam, prop, its = run_pcoa(24)
+            per_product = (t24 - t8) / 16.0
+            n_pad = (p.n_samples + 127) // 128 * 128
+            gbs = 8.0 * n_pad * n_pad / per_product / 1e9
+            pcoa = dict(matrix=variant_name(variants[-1]), axes=5, products=its, seconds=t24, ms_per_product=1e3 * per_product,
+                        setup_seconds=t8 - 8 * per_product, eigenvalues=[float(v) for v in lam], proportion_explained=[float(v) for v in prop],
+                        bound="hbm", product_gbs=gbs, note="Y = B Q streams B_hi and B_lo (8 N^2 bytes) per product; tcgen05 kind::tf32, 3-term split; "
+                        "fixed 24 products here (convergence is checked in tests/test_gpu_pcoa.py)")
+        except binding.UnifracError as e:
+            pcoa = dict(error=str(e))
+        torch.cuda.empty_cache()
 
     # ---------------- end to end through the host-buffer C-ABI call (H2D + D2H inside the timed region)
     e2e = None
@@ -267,7 +407,6 @@ def main():
         if world > 1:
             dist.destroy_process_group()
         return 0
-
     # ---------------- device rates of the atomic units (peaks of the k_mid / k_tail_scatter rooflines), measured live
     rates = dict(smem_atomic_random_per_s=SMEM_ATOMIC_PER_S, l2_red_random_per_s=L2_RED_PER_S)
     rates_src = "fallback constants (bench.py)"
@@ -348,42 +487,46 @@ def main():
     roofline["step_updates"] = dict(dense=upd_all / max(1, world), executed=w_exec_all, inter=w_inter,
                                     embed_seconds=sum(s["ms_embed"] for s in flat) * 1e-3)
 
+    roofline["traffic_source"] = TRAFFIC_SOURCE + "; null = no capture of the current kernel"
+
     cpu = None
     if not a.no_cpu_baseline:
         leg = oracle_leg(p, variants, a.cpu_budget_s)
         b_emb = flat[0]["branches_embedded"]
+        per_pair = leg["seconds"] / leg["pairs"]
         cpu = dict(value=leg["pairs"] * b_emb / leg["seconds"], unit=UNIT, cores=leg["cores"], kind="oracle",
-                   sample=leg["sample"], seconds=leg["seconds"])
+                   sample=leg["sample"], seconds=leg["seconds"], cpu_model=cpu_model_name(),
+                   extrapolated_all_pairs_s=per_pair * p.n_pairs * len(variants),
+                   extrapolated_note="EXTRAPOLATED: sampled seconds per pair x N(N-1)/2 x variants; the oracle is a plain "
+                                     "definition (long double, Neumaier sums), not an optimised CPU implementation")
 
-    per_variant = {}
-    for k, v in enumerate(variants):
-        ss = [st[k] for st in all_stats]
-        per_variant["unweighted" if v == 0 else "weighted_normalized"] = dict(
-            ms_total=float(np.mean([s["ms_total"] for s in ss])), ms_plan=float(np.mean([s["ms_plan"] for s in ss])),
-            ms_embed=float(np.mean([s["ms_embed"] for s in ss])), ms_tail=float(np.mean([s["ms_tail"] for s in ss])), ms_mid=float(np.mean([s["ms_mid"] for s in ss])),
-            mid_rows=ss[0]["mid_rows"], mid_updates=ss[0]["mid_updates"], mid_F=ss[0]["mid_F"],
-            ms_stripe=float(np.mean([s["ms_stripe"] for s in ss])),
-            head_rows=ss[0]["head_rows"], tail_rows=ss[0]["tail_rows"], tail_updates=ss[0]["tail_updates"],
-            gram=ss[0]["gram"], gram_k=ss[0]["gram_k"], gram_q=ss[0]["gram_q"],
-            tail_entries=ss[0]["tail_entries"], tail_launches=ss[0]["tail_launches"],
-            updates_executed_head=ss[0]["updates_executed_head"],
-            updates_dense=ss[0]["updates_dense"], updates_executed=ss[0]["updates_executed"],
-            updates_union=ss[0]["updates_union"], updates_inter=ss[0]["updates_inter"],
-            branches_embedded=ss[0]["branches_embedded"], workspace_gb=ss[0]["workspace_bytes"] / 2**30)
-
+    per_variant = wall_of(all_stats, variants, p.n_nodes, p.nnz)
+    if shard:
+        par = f"shards x{world}: disjoint tile-pair blocks per rank, then NCCL all-reduce(SUM) merge inside the timed region"
+    else:
+        par = f"replicas x{world}"
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=a.steps, warmup=a.warmup, ms_per_step=ms / a.steps,
                 higher_is_better=True, scaling="strong" if shard else "weak", vs_baseline=None, dtype=dtype, data="synthetic",
                 config=dict(workload=a.workload, n_samples=p.n_samples, n_nodes=p.n_nodes, nnz=p.nnz, seed=a.seed,
-                            variants=list(variants), precision=dtype, flags=a.flags,
-                            parallelism=f"shards x{world} (disjoint tile-pair blocks, no collective)" if shard else f"replicas x{world}",
+                            variants=list(variants), precision=dtype, flags=a.flags, parallelism=par,
                             l2="inputs larger than L2 (compact embedding >> 126 MB)"),
-                clocks=summarize_clocks(lines), e2e=e2e, gpu_launches=int(sum(s["kernel_launches"] for s in flat)),
-                roofline=roofline, cpu_baseline=cpu, wall=per_variant)
+                clocks=summarize_clocks(lines), e2e=e2e,
+                gpu_launches=int(sum(s["kernel_launches"] for s in flat)),
+                roofline=roofline, cpu_baseline=cpu, wall=per_variant, parity=parity)
+    if wall_emp is not None:
+        line["wall_emp"] = wall_emp
+        line["gpu_launches_emp_leg"] = launches_emp
     if mantel:
         hbm = peaks.get("hbm_gbs", 6550.0)
-        mantel.update(bound="hbm", peak_gbs=hbm, frac=mantel["algorithmic_gbs"] / hbm,
-                      note="algorithmic bytes = 2 x N(N-1)/2 x 4 B per statistic; the kernel moves ~1.5x that (full rows of the square copy)")
+        mantel["pearson"].update(bound="hbm", peak_gbs=hbm, frac=mantel["pearson"]["algorithmic_gbs"] / hbm,
+                                 note="algorithmic bytes = both condensed matrices once per statistic; the kernel moves ~1.5x that "
+                                      "(full rows of the square copy)")
         line["mantel"] = mantel
+    if pcoa:
+        if "product_gbs" in pcoa:
+            hbm = peaks.get("hbm_gbs", 6550.0)
+            pcoa.update(peak_gbs=hbm, frac=pcoa["product_gbs"] / hbm)
+        line["pcoa"] = pcoa
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -290,3 +290,24 @@ def test_randomized_shapes_all_pairs(B, O, case):
         for precision in (0, 1):
             for flags in (0, 128):
                 check(gpu_dm(B, p, variant, precision, flags), want, precision)
+
+
+@pytest.mark.parametrize("variant", [U, W])
+def test_two_shards_on_two_streams_merge_to_the_oracle_matrix(B, O, variant):
+    """The N > 1 path of bench.py on one GPU: shards 0 and 1 of 2 run on two streams into two buffers; their element-wise sum
+    (what multigpu.merge_shards' all-reduce(SUM) produces) is compared with the oracle on EVERY pair.  1,700 samples = 14
+    tiles = blocks (0,0), (0,1), (1,1) of 12 x 12 tiles dealt to shards 0, 1, 0."""
+    import torch
+    cfg = synth.CONFIGS["small"]
+    p = synth.make_problem(3000, 1700, 0.1, 1.1, cfg[4], cfg[5], seed=5)
+    n = p.n_samples
+    want = O.all_pairs(p.parent, p.branch_len, p.indptr, p.indices, p.counts, variant)
+    args = B.to_device(p)
+    torch.cuda.synchronize()
+    s0, s1 = torch.cuda.Stream(), torch.cuda.Stream()
+    a = B.unifrac_dm(*args, n, variant, B.FP32, shard=(0, 2), stream=s0)
+    b = B.unifrac_dm(*args, n, variant, B.FP32, shard=(1, 2), stream=s1)
+    torch.cuda.synchronize()
+    assert int(torch.count_nonzero((a != 0) & (b != 0))) == 0          # disjoint owners
+    assert int(torch.count_nonzero(a)) > 0 and int(torch.count_nonzero(b)) > 0
+    check((a + b).cpu().numpy().astype(np.float64), want, 0)
