@@ -35,6 +35,18 @@ template <> struct RankKey<double> {
     }
 };
 
+// plain unsigned keys (sample / row orderings inside unifrac_dm: perm.cuh, skip.cuh)
+template <> struct RankKey<uint32_t> {
+    using K = uint32_t;
+    static constexpr int PASSES = 4;
+    __device__ static __forceinline__ K make(uint32_t v) { return v; }
+};
+template <> struct RankKey<unsigned long long> {
+    using K = unsigned long long;
+    static constexpr int PASSES = 8;
+    __device__ static __forceinline__ K make(unsigned long long v) { return v; }
+};
+
 // block b owns the contiguous element range [b * per_block, min(P, (b + 1) * per_block)), per_block a multiple of RADIX_TILE
 __device__ __forceinline__ void radix_range(unsigned long long P, unsigned long long per_block, unsigned long long& lo, unsigned long long& hi) {
     lo = (unsigned long long)blockIdx.x * per_block;

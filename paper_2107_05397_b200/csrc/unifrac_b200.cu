@@ -13,6 +13,7 @@
 #include "rates.cuh"
 #include "mantel.cuh"
 #include "rank.cuh"
+#include "perm.cuh"
 #include "pcoa.cuh"
 #include "guard.cuh"
 
@@ -74,6 +75,7 @@ struct Arena {
 };
 
 inline int cdiv(long long a, long long b) { return (int)((a + b - 1) / b); }
+inline double env_double(const char* k, double d) { const char* e = getenv(k); return e ? atof(e) : d; }
 
 // cuTensorMapEncodeTiled through the runtime's driver entry point (the library does not link libcuda)
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
@@ -132,6 +134,55 @@ struct Timer {
     float ms(int a, int b) { float m = 0; if (on && b < n) cudaEventElapsedTime(&m, ev[a], ev[b]); return m; }
 };
 
+// stable LSD radix sort of (key, position) pairs (rank.cuh); the sort buffers are shared between the sorts of a call
+struct RankBufs { void* keys[2]; uint32_t* idx[2]; uint32_t* hist; uint32_t* offs; uint32_t* blast; unsigned nb; unsigned long long per_block; };
+template <typename T>
+RankBufs make_rank_bufs(Arena& A, unsigned long long P, int n_sm)
+{
+    RankBufs B{};
+    B.nb = (unsigned)n_sm * 8;
+    B.per_block = ((P + B.nb - 1) / B.nb + RADIX_TILE - 1) / RADIX_TILE * RADIX_TILE;
+    const size_t ksz = sizeof(typename RankKey<T>::K);
+    for (int i = 0; i < 2; ++i) { B.keys[i] = A.get(P * ksz); B.idx[i] = A.get_n<uint32_t>(P); }
+    B.hist = A.get_n<uint32_t>((size_t)256 * B.nb + 1);
+    B.offs = A.get_n<uint32_t>((size_t)256 * B.nb + 1);
+    B.blast = A.get_n<uint32_t>(B.nb);
+    return B;
+}
+// returns the buffer index that holds the sorted keys / positions
+template <typename T>
+int radix_sort(const T* v, unsigned long long P, const RankBufs& B, cudaStream_t st)
+{
+    using K = typename RankKey<T>::K;
+    K* keys[2] = {reinterpret_cast<K*>(B.keys[0]), reinterpret_cast<K*>(B.keys[1])};
+    int src = 0;                                                     // pass 0 reads v[] itself and writes buffer 0
+    for (int pass = 0; pass < RankKey<T>::PASSES; ++pass) {
+        const int shift = 8 * pass, dst = pass == 0 ? 0 : src ^ 1;
+        if (pass == 0) k_radix_hist<T, true><<<B.nb, RADIX_THREADS, 0, st>>>(v, nullptr, P, B.per_block, shift, B.hist);
+        else k_radix_hist<T, false><<<B.nb, RADIX_THREADS, 0, st>>>(nullptr, keys[src], P, B.per_block, shift, B.hist);
+        CU_LAUNCH();
+        k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>((int)(256 * B.nb), B.hist, B.offs); CU_LAUNCH();
+        if (pass == 0) k_radix_scatter<T, true><<<B.nb, RADIX_THREADS, 0, st>>>(v, nullptr, nullptr, P, B.per_block, shift, B.offs, keys[dst], B.idx[dst]);
+        else k_radix_scatter<T, false><<<B.nb, RADIX_THREADS, 0, st>>>(nullptr, keys[src], B.idx[src], P, B.per_block, shift, B.offs, keys[dst], B.idx[dst]);
+        CU_LAUNCH();
+        src = dst;
+    }
+    return src;
+}
+// average ranks (fp64, 1-based) of the P values v[] -> rank[]
+template <typename T>
+void rank_transform(const T* v, unsigned long long P, double* rank, const RankBufs& B, cudaStream_t st)
+{
+    using K = typename RankKey<T>::K;
+    const int src = radix_sort<T>(v, P, B, st);
+    K* keys[2] = {reinterpret_cast<K*>(B.keys[0]), reinterpret_cast<K*>(B.keys[1])};
+    uint32_t* start = reinterpret_cast<uint32_t*>(keys[src ^ 1]);     // the other key buffer and position buffer are free now
+    uint32_t* rlen = B.idx[src ^ 1];
+    k_rank_block_heads<K><<<B.nb, RADIX_THREADS, 0, st>>>(keys[src], P, B.per_block, B.blast); CU_LAUNCH();
+    k_rank_starts<K><<<B.nb, RADIX_THREADS, 0, st>>>(keys[src], P, B.per_block, B.blast, start, rlen); CU_LAUNCH();
+    k_rank_write<<<B.nb * 4, 256, 0, st>>>(B.idx[src], start, rlen, P, rank); CU_LAUNCH();
+}
+
 template <typename T>
 void run(int32_t n, const int32_t* parent, const double* len, const int32_t* postorder, unifrac_csr_t tab,
          int32_t N, int weighted, void* out, Arena& A, uint32_t flags, cudaStream_t st, int shard, int n_shards, bool is_retry)
@@ -141,9 +192,48 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     Timer tm(timing, st);
     unsigned launches = 0;
     tm.mark();
+    const int TB = 256;
+    int dev_id = 0, n_sm_dev = 0;
+    CU(cudaGetDevice(&dev_id));
+    CU(cudaDeviceGetAttribute(&n_sm_dev, cudaDevAttrMultiProcessorCount, dev_id));
+
+    // ------------------------------------------------------------------ richness order of the samples (perm.cuh): the weighted
+    // fp32 path decides per (branch, tile) between the skip kernel and the join, which pays off when rich samples share tiles
+    const bool skip_path = std::is_same<T, float>::value && weighted &&
+                           !(flags & (UNIFRAC_FLAG_ABSDIFF | UNIFRAC_FLAG_LITERAL | UNIFRAC_FLAG_NO_TAIL | UNIFRAC_FLAG_SPARSE_STRIPE |
+                                      UNIFRAC_FLAG_NO_MID | UNIFRAC_FLAG_ALL_TAIL)) && env_double("UNIFRAC_B200_SKIP", 1) != 0;
+    uint32_t* inv_perm = nullptr;                 // sample -> position; NULL = identity
+    void* const out_user = out;
+    if (skip_path && n_shards == 1 && N > TILE && env_double("UNIFRAC_B200_PERMUTE", 1) != 0) {
+        uint32_t* key = A.get_n<uint32_t>(N);
+        unsigned int* bad = A.get_n<unsigned int>(1);
+        CU(cudaMemsetAsync(bad, 0, sizeof(unsigned int), st));
+        k_perm_keys<<<cdiv(N, TB), TB, 0, st>>>(N, tab.indptr, key, bad); CU_LAUNCH(); ++launches;
+        unsigned int h_bad = 0; long long h_nnz = 0;
+        CU(cudaMemcpyAsync(&h_bad, bad, sizeof(h_bad), cudaMemcpyDeviceToHost, st));
+        CU(cudaMemcpyAsync(&h_nnz, tab.indptr + N, sizeof(h_nnz), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        if (!h_bad && h_nnz >= 0 && h_nnz < (1ll << 32)) {       // otherwise: validation below reports what is wrong
+            RankBufs RB = make_rank_bufs<uint32_t>(A, (unsigned long long)N, n_sm_dev);
+            const int src = radix_sort<uint32_t>(key, (unsigned long long)N, RB, st);
+            launches += 12;
+            const uint32_t* perm = RB.idx[src];                  // position -> sample
+            uint32_t* rowlen = A.get_n<uint32_t>((size_t)N + 1);
+            uint32_t* rowoff = A.get_n<uint32_t>((size_t)N + 1);
+            inv_perm = A.get_n<uint32_t>(N);
+            k_perm_rowlen<<<cdiv(N, TB), TB, 0, st>>>(N, tab.indptr, perm, rowlen, inv_perm); CU_LAUNCH(); ++launches;
+            k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>(N, rowlen, rowoff); CU_LAUNCH(); ++launches;
+            int64_t* p_indptr = A.get_n<int64_t>((size_t)N + 1);
+            int32_t* p_indices = A.get_n<int32_t>(h_nnz ? (size_t)h_nnz : 1);
+            int32_t* p_counts = A.get_n<int32_t>(h_nnz ? (size_t)h_nnz : 1);
+            k_perm_gather<<<cdiv((long long)N * 32, TB), TB, 0, st>>>(N, tab.indptr, tab.indices, tab.counts, perm, rowoff, p_indptr, p_indices, p_counts);
+            CU_LAUNCH(); ++launches;
+            tab.indptr = p_indptr; tab.indices = p_indices; tab.counts = p_counts;      // from here on: position space
+            out = A.get_n<T>((size_t)N * (N - 1) / 2);
+        }
+    }
 
     // ------------------------------------------------------------------ a-0 plan / validate
-    const int TB = 256;
     PlanWords* pw = A.get_n<PlanWords>(1);
     int32_t* child_count = A.get_n<int32_t>(n);
     int32_t* seen = A.get_n<int32_t>(n);
@@ -656,6 +746,11 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         CU(cudaMemsetAsync(GP.scratch, 0, sizeof(uint32_t) * (size_t)ggrid * 3 * n, st));
         k_guard<T><<<ggrid, GUARD_THREADS, 0, st>>>(GP); CU_LAUNCH(); ++launches;
     }
+    if (inv_perm) {
+        k_unpermute<T><<<dim3((unsigned)cdiv(N, 256), (unsigned)std::min(N, 65535)), 256, 0, st>>>((long long)N, inv_perm, reinterpret_cast<const T*>(out),
+                                                                                                  reinterpret_cast<T*>(out_user));
+        CU_LAUNCH(); ++launches;
+    }
     // stripe counters -> pinned host block (read lazily by unifrac_last_stats)
     if (!g_stats_pinned) { CU(cudaHostAlloc(&g_stats_pinned, 4 * sizeof(unsigned long long), cudaHostAllocDefault)); }
     if (!g_stats_event) { CU(cudaEventCreateWithFlags(&g_stats_event, cudaEventDisableTiming)); }
@@ -771,32 +866,6 @@ void run_mantel(int32_t N, const T* x, const T* y, const int32_t* perms, int32_t
     A.release();
 }
 
-// average ranks (fp64, 1-based) of the P values v[] -> rank[]; sort buffers are shared between the two vectors of a call
-struct RankBufs { void* keys[2]; uint32_t* idx[2]; uint32_t* hist; uint32_t* offs; uint32_t* blast; unsigned nb; unsigned long long per_block; };
-template <typename T>
-void rank_transform(const T* v, unsigned long long P, double* rank, const RankBufs& B, cudaStream_t st)
-{
-    using K = typename RankKey<T>::K;
-    K* keys[2] = {reinterpret_cast<K*>(B.keys[0]), reinterpret_cast<K*>(B.keys[1])};
-    int src = 0;                                                     // pass 0 reads v[] itself and writes buffer 0
-    for (int pass = 0; pass < RankKey<T>::PASSES; ++pass) {
-        const int shift = 8 * pass, dst = pass == 0 ? 0 : src ^ 1;
-        if (pass == 0) k_radix_hist<T, true><<<B.nb, RADIX_THREADS, 0, st>>>(v, nullptr, P, B.per_block, shift, B.hist);
-        else k_radix_hist<T, false><<<B.nb, RADIX_THREADS, 0, st>>>(nullptr, keys[src], P, B.per_block, shift, B.hist);
-        CU_LAUNCH();
-        k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>((int)(256 * B.nb), B.hist, B.offs); CU_LAUNCH();
-        if (pass == 0) k_radix_scatter<T, true><<<B.nb, RADIX_THREADS, 0, st>>>(v, nullptr, nullptr, P, B.per_block, shift, B.offs, keys[dst], B.idx[dst]);
-        else k_radix_scatter<T, false><<<B.nb, RADIX_THREADS, 0, st>>>(nullptr, keys[src], B.idx[src], P, B.per_block, shift, B.offs, keys[dst], B.idx[dst]);
-        CU_LAUNCH();
-        src = dst;
-    }
-    uint32_t* start = reinterpret_cast<uint32_t*>(keys[src ^ 1]);     // the other key buffer and position buffer are free now
-    uint32_t* rlen = B.idx[src ^ 1];
-    k_rank_block_heads<K><<<B.nb, RADIX_THREADS, 0, st>>>(keys[src], P, B.per_block, B.blast); CU_LAUNCH();
-    k_rank_starts<K><<<B.nb, RADIX_THREADS, 0, st>>>(keys[src], P, B.per_block, B.blast, start, rlen); CU_LAUNCH();
-    k_rank_write<<<B.nb * 4, 256, 0, st>>>(B.idx[src], start, rlen, P, rank); CU_LAUNCH();
-}
-
 template <typename T>
 void run_spearman(int32_t N, const T* x, const T* y, const int32_t* perms, int32_t K, double* out, Arena& A, cudaStream_t st)
 {
@@ -805,14 +874,7 @@ void run_spearman(int32_t N, const T* x, const T* y, const int32_t* perms, int32
     int dev = 0, n_sm = 0;
     CU(cudaGetDevice(&dev));
     CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-    RankBufs B{};
-    B.nb = (unsigned)n_sm * 8;
-    B.per_block = ((P + B.nb - 1) / B.nb + RADIX_TILE - 1) / RADIX_TILE * RADIX_TILE;
-    const size_t ksz = sizeof(typename RankKey<T>::K);
-    for (int i = 0; i < 2; ++i) { B.keys[i] = A.get(P * ksz); B.idx[i] = A.get_n<uint32_t>(P); }
-    B.hist = A.get_n<uint32_t>((size_t)256 * B.nb + 1);
-    B.offs = A.get_n<uint32_t>((size_t)256 * B.nb + 1);
-    B.blast = A.get_n<uint32_t>(B.nb);
+    RankBufs B = make_rank_bufs<T>(A, P, n_sm);
     double* rx = A.get_n<double>(P);
     double* ry = A.get_n<double>(P);
     rank_transform<T>(x, P, rx, B, st);
