@@ -164,6 +164,8 @@ def wall_of(all_stats, variants, n_nodes, nnz):
             mid_rows=s0["mid_rows"], mid_updates=s0["mid_updates"], mid_F=s0["mid_F"],
             head_rows=s0["head_rows"], tail_rows=s0["tail_rows"], tail_updates=s0["tail_updates"],
             gram=s0["gram"], gram_k=s0["gram_k"], gram_q=s0["gram_q"], guard_pairs=s0["guard_pairs"],
+            skip=s0["skip"], skip_rows=s0["skip_rows"], list_rows=s0["list_rows"], skip_row_pair_visits=s0["skip_row_pair_visits"],
+            skip_updates_executed=s0["skip_updates_executed"],
             tail_entries=s0["tail_entries"], tail_launches=s0["tail_launches"],
             updates_executed_head=s0["updates_executed_head"], updates_dense=s0["updates_dense"],
             updates_executed=s0["updates_executed"], updates_union=s0["updates_union"], updates_inter=s0["updates_inter"],

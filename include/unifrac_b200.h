@@ -63,6 +63,11 @@ typedef enum {
                                              head and tail only                                            */
 #define UNIFRAC_FLAG_SPARSE_STRIPE   256u  /* head branches on the sparse-aware compact-row stripe kernel (row flags, quarter masks)
                                              instead of the dense min-GEMM kernel                          */
+#define UNIFRAC_FLAG_RICHNESS_ZONES  512u  /* weighted + fp32: sort the samples by richness inside the call and split step a-5 per
+                                             (branch, tile): tile pairs inside a branch's dense zone on the register-tile kernel
+                                             k_zone, the rest on the join.  Same results; pays off when
+                                             presence is strongly clustered over the samples (on the iid synthetic configs it is
+                                             as fast as the default per-branch split, so it is opt-in).  Ignored otherwise.     */
 #define UNIFRAC_FLAG_NO_TENSOR       64u  /* unweighted + fp32: head branches on the CUDA-core stripe kernel
                                              instead of the tensor-core Gram kernel                        */
 
@@ -163,6 +168,8 @@ typedef struct {
     uint64_t rows_staged;        /* rows the producer staged into shared memory, over all tile pairs  */
     uint64_t embed_rows;         /* sum over sample tiles of non-empty rows (compact embedding rows)  */
     uint64_t workspace_bytes;    /* device bytes requested from the allocator                         */
+    uint64_t skip_updates_executed; /* RICHNESS_ZONES (k_zone): 128 x 128 pair updates per (row, tile pair) visit           */
+    uint64_t skip_row_pair_visits;  /* (row, tile pair) visits of k_zone                                                     */
     uint32_t n_tile_pairs;       /* 128x128 tile pairs in the upper triangle                          */
     uint32_t n_levels;           /* tree depth levels                                                 */
     uint32_t stripe_launches;    /* stripe-kernel launches in this call                               */
@@ -174,6 +181,10 @@ typedef struct {
     uint32_t gram_k;             /* K (head branches, padded to 64) of that GEMM                       */
     uint32_t gram_q;             /* fixed-point scale: L_v = round(len_v * 2^q)                        */
     uint32_t dense;              /* 1 if the head branches went through the dense CUDA-core kernel (k_dense) */
+    uint32_t skip;               /* 1 if the call used the per-(branch, tile) split k_zone + join (UNIFRAC_FLAG_RICHNESS_ZONES);
+                                    then head_rows = rows with a dense copy, mid_rows = list_rows, mid_updates = joined updates */
+    uint32_t skip_rows;          /* rows of the dense operand matrix of k_zone                                       */
+    uint32_t list_rows;          /* non-tail rows (ordered by their tile cut D_v)                                    */
     uint32_t guard_pairs;        /* pairs with d < 1/16 that the near-duplicate guard recomputed from the definition */
     uint32_t guard_capacity;     /* size of the guard's pair list: min(P, max(2^22, 64 N)); pairs listed beyond it keep
                                     their separable-form value (absolute error ~1e-7 in fp32)                           */
@@ -257,7 +268,7 @@ int unifrac_measure_rates(unifrac_rates_t *out, void *stream);
 
 const char *unifrac_status_string(int status);
 const char *unifrac_last_cuda_error(void);   /* text of the last CUDA error seen by this thread  */
-int unifrac_abi_version(void);               /* 5                                                */
+int unifrac_abi_version(void);               /* 6                                                */
 
 #ifdef __cplusplus
 }

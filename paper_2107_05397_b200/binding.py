@@ -17,9 +17,9 @@ from . import build as _build
 UNWEIGHTED, WEIGHTED_NORMALIZED = 0, 1
 FP32, FP64 = 0, 1
 FLAG_LITERAL, FLAG_TENSOR_GRAM, FLAG_SKIP_VALIDATION, FLAG_ABSDIFF = 1, 2, 4, 8
-FLAG_NO_TAIL, FLAG_ALL_TAIL, FLAG_NO_TENSOR, FLAG_NO_MID, FLAG_SPARSE_STRIPE = 16, 32, 64, 128, 256
+FLAG_NO_TAIL, FLAG_ALL_TAIL, FLAG_NO_TENSOR, FLAG_NO_MID, FLAG_SPARSE_STRIPE, FLAG_RICHNESS_ZONES = 16, 32, 64, 128, 256, 512
 
-ABI_VERSION = 5          # unifrac_abi_version() of the header this binding was written against
+ABI_VERSION = 6          # unifrac_abi_version() of the header this binding was written against
 OK = 0
 ERR_INVALID_ARG, ERR_INVALID_TREE, ERR_INVALID_TABLE, ERR_EMPTY_SAMPLE = -1, -2, -3, -4
 ERR_WORKSPACE, ERR_CUDA, ERR_UNSUPPORTED = -5, -6, -7
@@ -38,9 +38,10 @@ class Stats(C.Structure):
                 ("head_rows", C.c_uint64), ("tail_rows", C.c_uint64), ("tail_updates", C.c_uint64),
                 ("tail_entries", C.c_uint64), ("mid_rows", C.c_uint64), ("mid_updates", C.c_uint64),
                 ("rows_staged", C.c_uint64),
-                ("embed_rows", C.c_uint64), ("workspace_bytes", C.c_uint64), ("n_tile_pairs", C.c_uint32),
+                ("embed_rows", C.c_uint64), ("workspace_bytes", C.c_uint64), ("skip_updates_executed", C.c_uint64),
+                ("skip_row_pair_visits", C.c_uint64), ("n_tile_pairs", C.c_uint32),
                 ("n_levels", C.c_uint32), ("stripe_launches", C.c_uint32), ("tail_launches", C.c_uint32),
-                ("kernel_launches", C.c_uint32), ("mid_launches", C.c_uint32), ("mid_F", C.c_uint32), ("gram", C.c_uint32), ("gram_k", C.c_uint32), ("gram_q", C.c_uint32), ("dense", C.c_uint32), ("guard_pairs", C.c_uint32), ("guard_capacity", C.c_uint32), ("quant_fallback", C.c_uint32), ("guard_theta", C.c_float), ("quant_err_ratio", C.c_float),
+                ("kernel_launches", C.c_uint32), ("mid_launches", C.c_uint32), ("mid_F", C.c_uint32), ("gram", C.c_uint32), ("gram_k", C.c_uint32), ("gram_q", C.c_uint32), ("dense", C.c_uint32), ("skip", C.c_uint32), ("skip_rows", C.c_uint32), ("list_rows", C.c_uint32), ("guard_pairs", C.c_uint32), ("guard_capacity", C.c_uint32), ("quant_fallback", C.c_uint32), ("guard_theta", C.c_float), ("quant_err_ratio", C.c_float),
                 ("ms_plan", C.c_float), ("ms_embed", C.c_float), ("ms_tail", C.c_float), ("ms_mid", C.c_float), ("ms_stripe", C.c_float),
                 ("ms_total", C.c_float)]
 

@@ -72,7 +72,8 @@ k_mid_seg(uint32_t n_mid, const int32_t* __restrict__ mrows, const uint32_t* __r
 // off[t][r], r = 0..n_mid: offset (within tile t's packed entries) of row r's first entry in tile t;
 // off[t][n_mid] = ttot[t] = number of packed entries of tile t.  One CTA per tile (exclusive scan over rows).
 __global__ void __launch_bounds__(1024)
-k_mid_off(uint32_t n_mid, const uint32_t* __restrict__ seg, uint32_t* __restrict__ off, uint32_t* __restrict__ ttot)
+k_mid_off(uint32_t n_mid, const uint32_t* __restrict__ seg, uint32_t* __restrict__ off, uint32_t* __restrict__ ttot,
+          const uint32_t* __restrict__ cut /* rows r < cut[0] are never joined (zone.cuh), or NULL */)
 {
     __shared__ uint32_t part[1024];
     const uint32_t t = blockIdx.x;
@@ -80,12 +81,14 @@ k_mid_off(uint32_t n_mid, const uint32_t* __restrict__ seg, uint32_t* __restrict
     const uint32_t* s1 = s0 + n_mid;
     uint32_t* o = off + (size_t)t * (n_mid + 1);
     const int th = threadIdx.x;
+    const uint32_t r0 = cut ? cut[0] : 0u;       // rows below cut[0] are in the dense zone of every tile
+    auto cnt = [&](uint32_t r) { return r >= r0 ? ((s1[r] - s0[r] + 1u) & ~1u) : 0u; };   // every (row, tile) list padded to an even length
     const uint32_t chunk = (n_mid + 1023u) / 1024u;
     uint32_t lo = th * chunk, hi = lo + chunk;
     if (lo > n_mid) lo = n_mid;
     if (hi > n_mid) hi = n_mid;
     uint32_t s = 0;
-    for (uint32_t r = lo; r < hi; ++r) s += (s1[r] - s0[r] + 1u) & ~1u;      // every (row, tile) list padded to an even length
+    for (uint32_t r = lo; r < hi; ++r) s += cnt(r);
     part[th] = s;
     __syncthreads();
     for (int k = 1; k < 1024; k <<= 1) {
@@ -95,7 +98,7 @@ k_mid_off(uint32_t n_mid, const uint32_t* __restrict__ seg, uint32_t* __restrict
         __syncthreads();
     }
     uint32_t run = th ? part[th - 1] : 0;
-    for (uint32_t r = lo; r < hi; ++r) { o[r] = run; run += (s1[r] - s0[r] + 1u) & ~1u; }
+    for (uint32_t r = lo; r < hi; ++r) { o[r] = run; run += cnt(r); }
     if (th == 1023) { o[n_mid] = part[1023]; ttot[t] = part[1023]; }
 }
 
@@ -103,13 +106,18 @@ k_mid_off(uint32_t n_mid, const uint32_t* __restrict__ seg, uint32_t* __restrict
 // One warp per mid row.
 __global__ void __launch_bounds__(256)
 k_mid_sums(uint32_t n_mid, const uint32_t* __restrict__ mbase, const uint32_t* __restrict__ mlen,
-           const uint32_t* __restrict__ ts, const float* __restrict__ tv, double* __restrict__ midsum)
+           const uint32_t* __restrict__ ts, const float* __restrict__ tv, double* __restrict__ midsum,
+           const uint32_t* __restrict__ cut /* or NULL */)
 {
     const uint32_t r = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
     if (r >= n_mid) return;
     const uint32_t base = mbase[r], m = mlen[r];
-    for (uint32_t k = lane; k < m; k += 32) atomicAdd(&midsum[ts[base + k]], (double)tv[base + k]);
+    for (uint32_t k = lane; k < m; k += 32) {
+        const uint32_t s = ts[base + k];
+        if (cut && r < cut[0]) continue;                       // this row is never joined
+        atomicAdd(&midsum[s], (double)tv[base + k]);
+    }
 }
 
 // packed tile-major entries: pk[tbase[t] + off[t][r] + k] = { r << 9 | (sample - 128 t) << 2,  q = round(u~ * 2^F) }
@@ -120,7 +128,7 @@ __global__ void __launch_bounds__(256)
 k_mid_pack(uint32_t n_mid, const uint32_t* __restrict__ mbase, const uint32_t* __restrict__ mlen,
            const uint32_t* __restrict__ ts, const float* __restrict__ tv, const uint32_t* __restrict__ seg,
            const uint32_t* __restrict__ off, const uint32_t* __restrict__ tbase, float qscale, double inv_qscale,
-           double* __restrict__ sums, double* __restrict__ qerr, uint2* __restrict__ pk)
+           double* __restrict__ sums, double* __restrict__ qerr, uint2* __restrict__ pk, const uint32_t* __restrict__ cut /* or NULL */)
 {
     const uint32_t r = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
@@ -129,6 +137,7 @@ k_mid_pack(uint32_t n_mid, const uint32_t* __restrict__ mbase, const uint32_t* _
     for (uint32_t k = lane; k < m; k += 32) {
         const uint32_t s = ts[base + k];
         const uint32_t t = s >> 7;
+        if (cut && r < cut[0]) continue;
         const uint32_t g0 = seg[(size_t)t * n_mid + r], g1 = seg[(size_t)(t + 1) * n_mid + r];
         const uint32_t pos = tbase[t] + off[(size_t)t * (n_mid + 1) + r] + (k - g0);
         const uint32_t x = (r << 9) | ((s & 127u) << 2);
@@ -148,6 +157,7 @@ struct MidParams {
     const uint32_t* off;          // [n_tiles][n_mid+1]
     const uint32_t* tbase;        // [n_tiles+1]
     const uint2* pk;              // packed entries, tile-major, rows ascending within a tile
+    const uint32_t* cut;          // pair (I, J) joins the rows r >= cut[I] only (zone.cuh); NULL = every row
     int n_samples;
     float* out;
     double inv_qscale;            // 2^-F
@@ -181,7 +191,8 @@ k_mid(const MidParams P)
         const int pi = s_pair;
         if ((uint32_t)pi >= P.n_pairs) break;
         const int2 ij = P.pairs[pi];
-        const uint32_t eI0 = P.tbase[ij.x], eI1 = P.tbase[ij.x + 1], eJ0 = P.tbase[ij.y];
+        const uint32_t eI1 = P.tbase[ij.x + 1], eJ0 = P.tbase[ij.y];
+        const uint32_t eI0 = P.tbase[ij.x] + (P.cut ? P.off[(size_t)ij.x * pitch + P.cut[ij.x]] : 0u);
         const uint32_t* offJ = P.off + (size_t)ij.y * pitch;
         const uint32_t nchunk = (eI1 - eI0 + 31u) >> 5;
 

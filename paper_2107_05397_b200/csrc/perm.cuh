@@ -1,23 +1,23 @@
 // perm.cuh -- richness ordering of the samples inside one unifrac_dm call (SURVEY 8a-5d(5) "sample re-ordering"
 // "sparse-aware optimizations", mechanism ours -- DESIGN.md "richness order").  Presence of a branch is far from uniform over
 // the samples: a sample with many features is present on many more branches than a poor one.  With the samples sorted by their
-// number of table entries (descending), every branch is dense in the leading 128-sample tiles and sparse in the trailing ones,
-// and step a-5 can decide per (branch, tile) which kernel handles it (skip.cuh).  The call then runs on the permuted table in
+// number of table entries (ascending), every branch is sparse in the leading 128-sample tiles and dense in the trailing ones,
+// and step a-5 can decide per (branch, tile) which kernel handles it (zone.cuh).  The call then runs on the permuted table in
 // "position space" and the finished condensed matrix is un-permuted once at the end.
 #pragma once
 #include "common.cuh"
 
 namespace ufb {
 
-// key[s] = 2^32 - 1 - (entries of sample s): an ascending stable sort gives descending richness, ties in sample order.
+// key[s] = entries of sample s: an ascending stable sort gives ascending richness, ties in sample order.
 // bad != 0: indptr is not a plausible CSR pointer array (the caller then skips the permutation and lets validation report it)
 __global__ void k_perm_keys(int N, const int64_t* __restrict__ indptr, uint32_t* __restrict__ key, unsigned int* __restrict__ bad)
 {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= N) return;
     const long long lo = indptr[s], hi = indptr[s + 1];
-    if ((s == 0 && lo != 0) || hi < lo || hi - lo >= (1ll << 31)) { atomicOr(bad, 1u); key[s] = 0xffffffffu; return; }
-    key[s] = 0xffffffffu - (uint32_t)(hi - lo);
+    if ((s == 0 && lo != 0) || hi < lo || hi - lo >= (1ll << 31)) { atomicOr(bad, 1u); key[s] = 0u; return; }
+    key[s] = (uint32_t)(hi - lo);
 }
 
 // rowlen[pos] = entries of the sample at position pos; inv[sample] = position

@@ -14,6 +14,7 @@
 #include "mantel.cuh"
 #include "rank.cuh"
 #include "perm.cuh"
+#include "zone.cuh"
 #include "pcoa.cuh"
 #include "guard.cuh"
 
@@ -24,6 +25,7 @@
 #include <type_traits>
 #include <vector>
 #include <algorithm>
+#include <queue>
 
 using namespace ufb;
 
@@ -197,11 +199,11 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     CU(cudaGetDevice(&dev_id));
     CU(cudaDeviceGetAttribute(&n_sm_dev, cudaDevAttrMultiProcessorCount, dev_id));
 
-    // ------------------------------------------------------------------ richness order of the samples (perm.cuh): the weighted
-    // fp32 path decides per (branch, tile) between the skip kernel and the join, which pays off when rich samples share tiles
-    const bool skip_path = std::is_same<T, float>::value && weighted &&
+    // ------------------------------------------------------------------ UNIFRAC_FLAG_RICHNESS_ZONES (weighted fp32): samples in
+    // richness order (perm.cuh) and a per-(branch, tile) split between the dense kernel and the join (zone.cuh)
+    const bool skip_path = std::is_same<T, float>::value && weighted && (flags & UNIFRAC_FLAG_RICHNESS_ZONES) &&
                            !(flags & (UNIFRAC_FLAG_ABSDIFF | UNIFRAC_FLAG_LITERAL | UNIFRAC_FLAG_NO_TAIL | UNIFRAC_FLAG_SPARSE_STRIPE |
-                                      UNIFRAC_FLAG_NO_MID | UNIFRAC_FLAG_ALL_TAIL)) && env_double("UNIFRAC_B200_SKIP", 1) != 0;
+                                      UNIFRAC_FLAG_NO_MID | UNIFRAC_FLAG_ALL_TAIL));
     uint32_t* inv_perm = nullptr;                 // sample -> position; NULL = identity
     void* const out_user = out;
     if (skip_path && n_shards == 1 && N > TILE && env_double("UNIFRAC_B200_PERMUTE", 1) != 0) {
@@ -367,7 +369,9 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     // ------------------------------------------------------------------ tensor-core Gram path: u8 operand matrices from the bits
     bool use_gram = gram && head_rows > 0 && head_rows < (1ull << 23);
     // CUDA-core head path: dense min-GEMM kernel (dense.cuh) unless a debug form needs the sparse-aware compact-row kernel
-    const bool dense_head = !use_gram && !(flags & (UNIFRAC_FLAG_ABSDIFF | UNIFRAC_FLAG_LITERAL | UNIFRAC_FLAG_NO_TAIL | UNIFRAC_FLAG_SPARSE_STRIPE));
+    // weighted fp32, default flags: per-(branch, tile) split between k_zone and the join (zone.cuh) instead of the per-branch one
+    const bool skip_on = skip_path && mid_ok && n_tiles <= ROWCUT_MAX_TILES && head_rows + mid_rows > 0 && head_rows + mid_rows < (1ull << 23);
+    const bool dense_head = !skip_on && !use_gram && !(flags & (UNIFRAC_FLAG_ABSDIFF | UNIFRAC_FLAG_LITERAL | UNIFRAC_FLAG_NO_TAIL | UNIFRAC_FLAG_SPARSE_STRIPE));
     double* uval = nullptr;
     double* uerr = nullptr;                                    // Gram path: |u~_v - len_v| of the fixed-point head lengths
     uint8_t* XG[4] = {nullptr, nullptr, nullptr, nullptr};
@@ -446,6 +450,11 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     const size_t Npad = (size_t)n_tiles * TILE;
     uint32_t Kd_pad = 0;
     const bool dense16 = dense_head && std::is_same<T, float>::value && envd("UNIFRAC_B200_DENSE16", 1) != 0;   // fp32: 16 consumer warps, mixed forms
+    // skip path (zone.cuh)
+    uint32_t sk_n = 0, sk_KE = 0;
+    int32_t* sk_rows = nullptr; uint32_t* sk_base = nullptr; uint32_t* sk_len = nullptr; uint32_t* sk_cut = nullptr; float* sk_E = nullptr;
+    std::vector<uint32_t> h_cut;
+    unsigned long long h_skstat[2] = {0, 0};
     double* hsum = nullptr;
     if (dense16) {
         hsum = A.get_n<double>((size_t)n_tiles * TILE);
@@ -484,6 +493,43 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             CU_LAUNCH(); ++launches;
             embed_rows = head_rows * (uint64_t)n_tiles;
         }
+    } else if (skip_on) {
+        // rows in (D_v ascending, n_v descending) order, the cut table, the dense rows k_zone needs (zone.cuh)
+        sk_n = (uint32_t)(head_rows + mid_rows);
+        int32_t* lnode = A.get_n<int32_t>(sk_n);
+        unsigned int* lcount = reinterpret_cast<unsigned int*>(work + 20);
+        k_list_compact<<<cdiv(n, TB), TB, 0, st>>>(n, cls, lnode, lcount); CU_LAUNCH(); ++launches;
+        unsigned long long* keys = A.get_n<unsigned long long>(sk_n);
+        // cost model of k_row_cut in SM-clocks (measured on B200, sweeps in profiles/r02_summary.md; overridable for tuning):
+        // one (row, tile pair) of k_zone, pair updates per clock of the join, one (entry, tile pair) visit of the join
+        CutModel CM{(float)env_double("UNIFRAC_B200_ZONE_C0", 330.0), (float)(0.5 / env_double("UNIFRAC_B200_JOIN_RATE", 4.64)),
+                    (float)env_double("UNIFRAC_B200_JOIN_ENT", 0.87)};
+        k_row_cut<<<cdiv(sk_n, ROWCUT_WARPS), ROWCUT_WARPS * 32, 0, st>>>(sk_n, lnode, bits, NW, n_tiles, (uint32_t)N, CM, keys); CU_LAUNCH(); ++launches;
+        RankBufs RB = make_rank_bufs<unsigned long long>(A, sk_n, n_sm_dev);
+        const int src = radix_sort<unsigned long long>(keys, sk_n, RB, st);
+        launches += 24;
+        sk_rows = A.get_n<int32_t>(sk_n);
+        uint32_t* Dr = A.get_n<uint32_t>(sk_n);
+        sk_base = A.get_n<uint32_t>(sk_n);
+        sk_len = A.get_n<uint32_t>(sk_n);
+        k_rows_from_sort<<<cdiv(sk_n, TB), TB, 0, st>>>(sk_n, RB.idx[src], reinterpret_cast<const unsigned long long*>(RB.keys[src]), lnode, tptr, nv,
+                                                         sk_rows, Dr, sk_base, sk_len); CU_LAUNCH(); ++launches;
+        sk_cut = A.get_n<uint32_t>((size_t)n_tiles + 1);
+        k_cut_table<<<cdiv(n_tiles + 1, TB), TB, 0, st>>>(n_tiles, sk_n, Dr, ZONE_BK, sk_cut); CU_LAUNCH(); ++launches;
+        k_cut_stats<<<cdiv((long long)sk_n * 32, TB), TB, 0, st>>>(sk_n, sk_rows, bits, NW, n_tiles, sk_cut, work + 21); CU_LAUNCH(); ++launches;
+        h_cut.resize((size_t)n_tiles + 1);
+        CU(cudaMemcpyAsync(h_cut.data(), sk_cut, sizeof(uint32_t) * ((size_t)n_tiles + 1), cudaMemcpyDeviceToHost, st));
+        CU(cudaMemcpyAsync(h_skstat, work + 21, sizeof(h_skstat), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        sk_KE = h_cut[n_tiles - 1];                              // cut is non-decreasing in the tile index
+        const size_t e_rows = sk_KE ? sk_KE : ZONE_BK;
+        sk_E = A.get_n<float>(e_rows * Npad);
+        CU(cudaMemsetAsync(sk_E, 0, sizeof(float) * e_rows * Npad, st));
+        if (sk_KE) {
+            k_E_scatter<<<cdiv((long long)sk_KE * 32, TB), TB, 0, st>>>(sk_KE, sk_base, sk_len, ts, reinterpret_cast<const float*>(tv), sk_E, Npad);
+            CU_LAUNCH(); ++launches;
+        }
+        embed_rows = (uint64_t)sk_KE * n_tiles;
     } else if (!use_gram) {
         rflags = A.get_n<uint32_t>((size_t)n_tiles * nwords);
         rrank = A.get_n<uint32_t>((size_t)n_tiles * nwords);
@@ -522,7 +568,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
 
     // ------------------------------------------------------------------ a-5 (tail branches): scatter into the condensed matrix
     unsigned tail_launches = 0;
-    if (tail_rows || mid_rows || n_shards > 1) CU(cudaMemsetAsync(out, 0, sizeof(T) * ((size_t)N * (N - 1) / 2), st));
+    if (tail_rows || mid_rows || skip_on || n_shards > 1) CU(cudaMemsetAsync(out, 0, sizeof(T) * ((size_t)N * (N - 1) / 2), st));
     if (tail_rows) {
         // super tiles: SUP x SUP samples whose condensed row segments (SUP * SUP * sizeof(T)) stay L2-resident
         size_t l2_budget = (size_t)48 << 20;
@@ -574,36 +620,41 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         memcpy(&quant_ratio, &h_r, sizeof(quant_ratio));
         if (quant_ratio > envd("UNIFRAC_B200_QUANT_BUDGET", QUANT_RATIO_BUDGET) && !is_retry) throw RetryExact{};
     };
-    if (mid_rows) {
+    if (mid_rows || skip_on) {
         if constexpr (std::is_same<T, float>::value) {
             if (mid_rows >= (1ull << 23)) throw StatusFail{UNIFRAC_ERR_UNSUPPORTED};     // packed entries keep the row in 23 bits
-            const uint32_t n_mid = (uint32_t)mid_rows;
-            uint32_t* mhist = A.get_n<uint32_t>((size_t)N + 2);
-            uint32_t* mcur = A.get_n<uint32_t>((size_t)N + 2);
-            int32_t* mrows = A.get_n<int32_t>(n_mid);
-            uint32_t* mbase = A.get_n<uint32_t>(n_mid);
-            uint32_t* mlen = A.get_n<uint32_t>(n_mid);
-            CU(cudaMemsetAsync(mhist, 0, sizeof(uint32_t) * ((size_t)N + 2), st));
-            k_mid_hist<<<cdiv(n, TB), TB, 0, st>>>(n, cls, nv, mhist); CU_LAUNCH(); ++launches;
-            k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>(N + 1, mhist, mcur); CU_LAUNCH(); ++launches;
-            k_mid_rows<<<cdiv(n, TB), TB, 0, st>>>(n, cls, nv, mcur, tptr, mrows, mbase, mlen); CU_LAUNCH(); ++launches;
+            const uint32_t n_mid = skip_on ? sk_n : (uint32_t)mid_rows;
+            int32_t* mrows = sk_rows; uint32_t* mbase = sk_base; uint32_t* mlen = sk_len;
+            if (!skip_on) {
+                uint32_t* mhist = A.get_n<uint32_t>((size_t)N + 2);
+                uint32_t* mcur = A.get_n<uint32_t>((size_t)N + 2);
+                mrows = A.get_n<int32_t>(n_mid);
+                mbase = A.get_n<uint32_t>(n_mid);
+                mlen = A.get_n<uint32_t>(n_mid);
+                CU(cudaMemsetAsync(mhist, 0, sizeof(uint32_t) * ((size_t)N + 2), st));
+                k_mid_hist<<<cdiv(n, TB), TB, 0, st>>>(n, cls, nv, mhist); CU_LAUNCH(); ++launches;
+                k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>(N + 1, mhist, mcur); CU_LAUNCH(); ++launches;
+                k_mid_rows<<<cdiv(n, TB), TB, 0, st>>>(n, cls, nv, mcur, tptr, mrows, mbase, mlen); CU_LAUNCH(); ++launches;
+            }
             uint32_t* mseg = A.get_n<uint32_t>((size_t)(n_tiles + 1) * n_mid);
             k_mid_seg<<<cdiv((long long)n_mid * 32, TB), TB, 0, st>>>(n_mid, mrows, tptr, ts, n_tiles, mseg); CU_LAUNCH(); ++launches;
             uint32_t* moff = A.get_n<uint32_t>((size_t)n_tiles * ((size_t)n_mid + 1));
             uint32_t* ttot = A.get_n<uint32_t>(n_tiles);
             uint32_t* tbase = A.get_n<uint32_t>((size_t)n_tiles + 1);
-            k_mid_off<<<n_tiles, 1024, 0, st>>>(n_mid, mseg, moff, ttot); CU_LAUNCH(); ++launches;
+            k_mid_off<<<n_tiles, 1024, 0, st>>>(n_mid, mseg, moff, ttot, sk_cut); CU_LAUNCH(); ++launches;
             k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>(n_tiles, ttot, tbase); CU_LAUNCH(); ++launches;
             unsigned long long* smax = work + 15;
             double* midsum = A.get_n<double>((size_t)n_tiles * TILE);
             CU(cudaMemsetAsync(midsum, 0, sizeof(double) * (size_t)n_tiles * TILE, st));
-            k_mid_sums<<<cdiv((long long)n_mid * 32, TB), TB, 0, st>>>(n_mid, mbase, mlen, ts, reinterpret_cast<const float*>(tv), midsum); CU_LAUNCH(); ++launches;
+            k_mid_sums<<<cdiv((long long)n_mid * 32, TB), TB, 0, st>>>(n_mid, mbase, mlen, ts, reinterpret_cast<const float*>(tv), midsum, sk_cut); CU_LAUNCH(); ++launches;
             k_max_positive<<<cdiv((long long)n_tiles * TILE, TB), TB, 0, st>>>(n_tiles * TILE, midsum, smax); CU_LAUNCH(); ++launches;
             unsigned long long h_smax = 0;
             CU(cudaMemcpyAsync(&h_smax, smax, sizeof(h_smax), cudaMemcpyDeviceToHost, st));
             uint32_t h_pk_total = 0;                            // packed entries incl. the even-length padding
             CU(cudaMemcpyAsync(&h_pk_total, tbase + n_tiles, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
             std::vector<int2> h_mp = blocked_pairs(n_tiles, 8, shard, n_shards);
+            if (skip_on)                                          // pairs whose rows all go to k_zone have nothing to join
+                h_mp.erase(std::remove_if(h_mp.begin(), h_mp.end(), [&](const int2& q) { return h_cut[q.x] >= sk_n; }), h_mp.end());
             int2* mpairs = A.get_n<int2>(h_mp.size());
             CU(cudaMemcpyAsync(mpairs, h_mp.data(), sizeof(int2) * h_mp.size(), cudaMemcpyHostToDevice, st));
             CU(cudaStreamSynchronize(st));
@@ -615,12 +666,12 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             (void)mid_entries;
             uint2* pk = A.get_n<uint2>(h_pk_total ? h_pk_total : 1);
             k_mid_pack<<<cdiv((long long)n_mid * 32, TB), TB, 0, st>>>(n_mid, mbase, mlen, ts, reinterpret_cast<const float*>(tv), mseg, moff, tbase,
-                                                                      ldexpf(1.0f, mid_F), ldexp(1.0, -mid_F), sums, qerr, pk); CU_LAUNCH(); ++launches;
+                                                                      ldexpf(1.0f, mid_F), ldexp(1.0, -mid_F), sums, qerr, pk, sk_cut); CU_LAUNCH(); ++launches;
             mid_packed = true;
             check_quant_ratio();
             MidParams M{};
             M.pairs = mpairs; M.n_pairs = (uint32_t)h_mp.size(); M.counter = reinterpret_cast<unsigned int*>(work + 7);
-            M.n_mid = n_mid; M.off = moff; M.tbase = tbase; M.pk = pk;
+            M.n_mid = n_mid; M.off = moff; M.tbase = tbase; M.pk = pk; M.cut = sk_cut;
             M.n_samples = N; M.out = reinterpret_cast<float*>(out); M.inv_qscale = ldexp(1.0, -mid_F);
             CU(cudaFuncSetAttribute(k_mid, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MID_SMEM));
             int occ = 0, dev2 = 0, n_sm2 = 0;
@@ -678,6 +729,39 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             }
             if (grid) { k_gram<<<grid, GRAM_THREADS, GRAM_SMEM, st>>>(tmA, tmB0, tmB1, tmB2, G); CU_LAUNCH(); ++launches; ++stripe_launches; }
             CU(cudaStreamSynchronize(st));       // h_pairs staging copy done before it goes out of scope
+        }
+    } else if (skip_on) {
+        if constexpr (std::is_same<T, float>::value) {
+            // tile pairs dealt to the CTAs in cache-blocked order, each to the least loaded CTA (work ~ stages + epilogue)
+            std::vector<int2> order = blocked_pairs(n_tiles, 8, shard, n_shards);
+            n_pairs = (uint32_t)order.size();
+            const unsigned grid = (unsigned)std::max<long long>(1, std::min<long long>(n_sm, n_pairs));
+            std::vector<std::vector<int2>> per(grid);
+            typedef std::pair<unsigned long long, unsigned> QE;
+            std::priority_queue<QE, std::vector<QE>, std::greater<QE>> pq;
+            for (unsigned b = 0; b < grid; ++b) pq.push(QE(0ull, b));
+            for (const int2& q : order) {
+                QE top = pq.top(); pq.pop();
+                per[top.second].push_back(q);
+                top.first += h_cut[q.x] / ZONE_BK + 3;
+                pq.push(top);
+            }
+            std::vector<int2> h_pairs; h_pairs.reserve(n_pairs);
+            std::vector<uint32_t> h_off(grid + 1, 0);
+            for (unsigned b = 0; b < grid; ++b) { h_pairs.insert(h_pairs.end(), per[b].begin(), per[b].end()); h_off[b + 1] = (uint32_t)h_pairs.size(); }
+            int2* pairs = A.get_n<int2>(n_pairs ? n_pairs : 1);
+            uint32_t* cta_off = A.get_n<uint32_t>(grid + 1);
+            CU(cudaMemcpyAsync(pairs, h_pairs.data(), sizeof(int2) * n_pairs, cudaMemcpyHostToDevice, st));
+            CU(cudaMemcpyAsync(cta_off, h_off.data(), sizeof(uint32_t) * (grid + 1), cudaMemcpyHostToDevice, st));
+            CU(cudaStreamSynchronize(st));           // staging copies of the host vectors are done
+            CUtensorMap tmE = make_rowmajor_map(sk_E, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, sizeof(float), Npad, sk_KE ? sk_KE : ZONE_BK, TILE, ZONE_BK,
+                                                CU_TENSOR_MAP_SWIZZLE_NONE);
+            ZoneParams SP{};
+            SP.pairs = pairs; SP.cta_off = cta_off; SP.cut = sk_cut; SP.sums = sums; SP.n_samples = N;
+            SP.out = reinterpret_cast<float*>(out); SP.add_out = 1; SP.guard = GL;
+            SP.scratch = A.get_n<double>((size_t)grid * 32 * 512);
+            CU(cudaFuncSetAttribute(k_zone, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZONE_SMEM));
+            if (n_pairs) { k_zone<<<grid, ZONE_THREADS, ZONE_SMEM, st>>>(tmE, SP); CU_LAUNCH(); ++launches; ++stripe_launches; }
         }
     } else if (dense_head) {
         std::vector<int2> h_pairs = blocked_pairs(n_tiles, 12, shard, n_shards);
@@ -769,6 +853,8 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     g_stats.head_rows = head_rows; g_stats.tail_rows = tail_rows; g_stats.tail_updates = tail_updates; g_stats.tail_entries = tail_entries;
     g_stats.tail_launches = tail_launches;
     g_stats.mid_rows = mid_rows; g_stats.mid_updates = mid_updates; g_stats.mid_launches = mid_launches; g_stats.mid_F = (uint32_t)mid_F;
+    g_stats.skip = skip_on ? 1u : 0u; g_stats.skip_rows = sk_KE; g_stats.list_rows = sk_n;
+    if (skip_on) { g_stats.mid_updates = h_skstat[0]; g_stats.skip_row_pair_visits = h_skstat[1]; g_stats.skip_updates_executed = h_skstat[1] * 16384ull; g_stats.mid_rows = sk_n; g_stats.head_rows = sk_KE; }
     g_stats.gram = use_gram ? 1u : 0u; g_stats.dense = dense_head ? 1u : 0u; g_stats.gram_k = K_pad; g_stats.gram_q = (uint32_t)gram_q;
     g_stats.guard_capacity = GL.cap; g_stats.guard_theta = GL.theta;
     g_stats.quant_err_ratio = (float)quant_ratio; g_stats.quant_fallback = is_retry ? 1u : 0u;
@@ -797,7 +883,8 @@ int guarded(int32_t n_nodes, const int32_t* parent, const double* len, const int
     if (variant != UNIFRAC_UNWEIGHTED && variant != UNIFRAC_WEIGHTED_NORMALIZED) return UNIFRAC_ERR_INVALID_ARG;
     if (precision != UNIFRAC_FP32 && precision != UNIFRAC_FP64) return UNIFRAC_ERR_INVALID_ARG;
     if (flags & ~(UNIFRAC_FLAG_LITERAL | UNIFRAC_FLAG_TENSOR_GRAM | UNIFRAC_FLAG_SKIP_VALIDATION | UNIFRAC_FLAG_ABSDIFF |
-                  UNIFRAC_FLAG_NO_TAIL | UNIFRAC_FLAG_ALL_TAIL | UNIFRAC_FLAG_NO_TENSOR | UNIFRAC_FLAG_NO_MID | UNIFRAC_FLAG_SPARSE_STRIPE))
+                  UNIFRAC_FLAG_NO_TAIL | UNIFRAC_FLAG_ALL_TAIL | UNIFRAC_FLAG_NO_TENSOR | UNIFRAC_FLAG_NO_MID | UNIFRAC_FLAG_SPARSE_STRIPE |
+                  UNIFRAC_FLAG_RICHNESS_ZONES))
         return UNIFRAC_ERR_INVALID_ARG;
     if ((long long)N > (1ll << 23)) return UNIFRAC_ERR_UNSUPPORTED;
     Arena A{alloc, user, st};
@@ -1038,7 +1125,8 @@ int unifrac_last_stats(unifrac_stats_t* out)
     if (g_stats_pending) {
         if (cudaEventSynchronize(g_stats_event) != cudaSuccess) { cudaGetLastError(); return UNIFRAC_ERR_CUDA; }
         g_stats.updates_executed_head = g_stats_pinned[0] * 2048ull;    // one (warp,row) = 32 x 64 pair updates
-        if (g_stats.gram || g_stats.dense) g_stats.updates_executed_head = g_stats.head_rows * ((uint64_t)g_stats.updates_dense / (g_stats.branches_embedded ? g_stats.branches_embedded : 1));
+        if (g_stats.skip) g_stats.updates_executed_head = g_stats.skip_updates_executed;
+        else if (g_stats.gram || g_stats.dense) g_stats.updates_executed_head = g_stats.head_rows * ((uint64_t)g_stats.updates_dense / (g_stats.branches_embedded ? g_stats.branches_embedded : 1));
         g_stats.updates_executed = g_stats.updates_executed_head + g_stats.tail_updates + g_stats.mid_updates;
         g_stats.rows_staged = g_stats_pinned[1];
         g_stats.guard_pairs = (uint32_t)(g_stats_pinned[2] & 0xffffffffull);      // listed; min(guard_pairs, guard_capacity) were recomputed
@@ -1197,6 +1285,6 @@ const char* unifrac_status_string(int status)
 }
 
 const char* unifrac_last_cuda_error(void) { return g_cuda_err.c_str(); }
-int unifrac_abi_version(void) { return 5; }
+int unifrac_abi_version(void) { return 6; }
 
 }  // extern "C"

@@ -77,9 +77,11 @@ def test_planted_near_duplicates_across_tiles_all_pairs(B, O, variant):
     near = want[idx[kinds == 2]]
     assert np.all(near > 0.0) and near.max() < 0.0625                           # d ~ 1e-4 .. 1e-2: all below the guard threshold
     for precision in (0, 1):
-        for flags in ((0, B.FLAG_NO_TENSOR) if (variant == U and precision == 0) else (0,)):
+        for flags in ((0, B.FLAG_NO_TENSOR) if (variant == U and precision == 0) else
+                      (0, B.FLAG_RICHNESS_ZONES) if (variant == W and precision == 0) else (0,)):
             got = gpu_dm(B, p, variant, precision, flags)
             st = B.unifrac_last_stats()
+            assert st["skip"] == (1 if flags == B.FLAG_RICHNESS_ZONES else 0)
             if precision == 0:
                 assert st["head_rows"] > 0 and st["mid_rows"] > 0 and st["tail_rows"] > 0, st
                 assert st["gram"] == (1 if (variant == U and flags == 0) else 0)

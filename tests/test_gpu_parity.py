@@ -53,7 +53,7 @@ def test_tiny_all_pairs(B, O, variant, precision, flags):
 
 @pytest.mark.parametrize("variant", [U, W])
 @pytest.mark.parametrize("precision", [1, 0])
-@pytest.mark.parametrize("flags", [0, 128, 64, 16, 32, 8])
+@pytest.mark.parametrize("flags", [0, 128, 64, 16, 32, 8, 512, 256, 4])
 def test_three_tiles_ragged_tail_all_pairs(B, O, variant, precision, flags):
     """300 samples = 2 full 128-tiles + a 44-sample tail; 3000 tips -> 5998 branches (several stages)."""
     p = synth.make_problem(3000, 300, 0.1, 1.1, synth.CONFIGS["small"][4], synth.CONFIGS["small"][5], seed=3)
@@ -262,6 +262,26 @@ def test_other_seeds_six_tiles_all_pairs_fp32_and_fp64(B, O, variant, seed):
     check(gpu_dm(B, p, variant, 0), want, 0)
     st = B.unifrac_last_stats()
     assert st["head_rows"] > 0 and st["tail_rows"] > 0
+
+
+@pytest.mark.parametrize("seed", [1, 2])
+def test_richness_zones_flag_weighted_fp32(B, O, seed):
+    """UNIFRAC_FLAG_RICHNESS_ZONES: samples sorted by richness inside the call, k_zone for the tile pairs inside a branch's dense
+    zone, the join for the rest, result un-permuted -- all 244,650 pairs of a 6-tile problem against the oracle, and the stats
+    say that both kernels had work.  A table whose poorest and richest samples differ by 30x makes the zones non-trivial."""
+    cfg = synth.CONFIGS["small"]
+    p = synth.make_problem(8000, 700, 0.05, 1.05, cfg[4], cfg[5], seed=seed)
+    rows = synth.rows_of(p)
+    for s in range(0, 700, 3):                                  # thin every third sample down to ~1/10 of its features
+        keys = sorted(rows[s])
+        rows[s] = {t: rows[s][t] for t in keys[::10]} or {keys[0]: 1}
+    p = synth.with_rows(p, rows)
+    want = O.all_pairs(p.parent, p.branch_len, p.indptr, p.indices, p.counts, W)
+    check(gpu_dm(B, p, W, 0, flags=B.FLAG_RICHNESS_ZONES), want, 0)
+    st = B.unifrac_last_stats()
+    assert st["skip"] == 1 and st["skip_row_pair_visits"] > 0 and st["mid_updates"] > 0 and st["tail_rows"] > 0
+    assert 0 < st["skip_rows"] <= st["list_rows"]
+    check(gpu_dm(B, p, U, 0, flags=B.FLAG_RICHNESS_ZONES), O.all_pairs(p.parent, p.branch_len, p.indptr, p.indices, p.counts, U), 0)   # ignored for unweighted
 
 
 def test_measure_rates_probe(B):
