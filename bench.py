@@ -386,12 +386,11 @@ def main():
     if not a.no_e2e and not shard:      # the host-buffer entry point computes whole matrices
         pin = lambda arr: torch.from_numpy(np.ascontiguousarray(arr)).pin_memory().numpy()
         hp = [pin(x) for x in (p.parent, p.branch_len, p.postorder, p.indptr, p.indices, p.counts)]
-        hout = torch.empty(p.n_pairs, dtype=torch.float32 if precision == 0 else torch.float64).pin_memory().numpy()
+        houts = [torch.empty(p.n_pairs, dtype=torch.float32 if precision == 0 else torch.float64).pin_memory().numpy() for _ in variants]
         del outs
         torch.cuda.empty_cache()
-        def e2e_step():
-            for v in variants:
-                binding.unifrac_dm_host(*hp, p.n_samples, v, precision, out=hout)
+        def e2e_step():                              # one call for the step's variants: inputs uploaded once, D2H overlaps compute
+            binding.unifrac_dm_host_multi(*hp, p.n_samples, list(variants), precision, outs=houts)
         e2e_step()                                   # one untimed warm-up step (device memory pool, page mappings)
         barrier()
         t0 = time.perf_counter()
@@ -400,8 +399,9 @@ def main():
         barrier()
         t_e2e = (time.perf_counter() - t0) / a.steps
         t_e2e, _ = reduce_over_ranks(t_e2e, 0.0, world, dev)
-        h2d = sum(x.nbytes for x in hp) * len(variants)
-        d2h = hout.nbytes * len(variants)
+        h2d = sum(x.nbytes for x in hp)
+        d2h = sum(h.nbytes for h in houts)
+        binding.unifrac_release_host_pool()
         e2e = dict(value=(upd_all / a.steps) / t_e2e, unit=UNIT, h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h),
                    seconds_per_step=t_e2e)
 

@@ -137,17 +137,30 @@ int unifrac_dm_shard(int32_t n_nodes, const int32_t *tree_parent, const double *
 int32_t unifrac_shard_of_pair(int32_t i, int32_t j, int32_t shard_count);
 
 /*
- * unifrac_dm_host -- same computation with HOST buffers (pageable or pinned).  The library
- * allocates device memory itself from the device's default stream-ordered pool (cudaMallocAsync), copies the
- * inputs in, runs unifrac_dm on an internal stream, copies the condensed result out to `out_condensed_host`,
- * returns every buffer to the pool and returns after completion (synchronous).  The pool's release threshold is
- * raised so that the memory stays mapped for the next call (cudaMemPoolTrimTo(pool, 0) gives it back).
- * `nnz` is read from indptr[n_samples].
+ * unifrac_dm_host -- same computation with HOST buffers (pageable or pinned).  The library allocates device memory itself
+ * from its OWN stream-ordered pool (one per device; other users of the device's default pool are not affected), copies the
+ * inputs in, runs unifrac_dm on an internal stream, copies the condensed result out to `out_condensed_host`, returns every
+ * buffer to the pool and returns after completion (synchronous).  The pool keeps its memory mapped for the next call;
+ * unifrac_release_host_pool() gives it back to the device.  `nnz` is read from indptr[n_samples].
  */
 int unifrac_dm_host(int32_t n_nodes, const int32_t *tree_parent, const double *branch_len,
                     const int32_t *postorder, unifrac_csr_t table_host, int32_t n_samples,
                     unifrac_variant_t variant, unifrac_precision_t precision,
                     void *out_condensed_host, uint32_t flags);
+
+/*
+ * unifrac_dm_host_multi -- both variants of one table in one call (the paper's use: "both unweighted and the weighted
+ * normalized versions").  The inputs are uploaded once; variant k + 1 is computed while the result of variant k
+ * travels back to the host on a second stream (unifrac_dm is asynchronous after its planning step).  variants[k] is a
+ * unifrac_variant_t, outs_host[k] the host buffer of variant k (n(n-1)/2 elements); 1 <= n_variants <= 2.  Synchronous.
+ */
+int unifrac_dm_host_multi(int32_t n_nodes, const int32_t *tree_parent, const double *branch_len,
+                          const int32_t *postorder, unifrac_csr_t table_host, int32_t n_samples,
+                          int32_t n_variants, const int32_t *variants, unifrac_precision_t precision,
+                          void *const *outs_host, uint32_t flags);
+
+/* trims the host entry points' device memory pool(s) to zero (after the calls that used them have returned) */
+int unifrac_release_host_pool(void);
 
 /* Statistics of the calling thread's last unifrac_dm call (work counters are exact, computed on
  * the device from the per-branch sample counts; times are CUDA-event milliseconds, valid only
@@ -268,7 +281,7 @@ int unifrac_measure_rates(unifrac_rates_t *out, void *stream);
 
 const char *unifrac_status_string(int status);
 const char *unifrac_last_cuda_error(void);   /* text of the last CUDA error seen by this thread  */
-int unifrac_abi_version(void);               /* 6                                                */
+int unifrac_abi_version(void);               /* 7                                                */
 
 #ifdef __cplusplus
 }

@@ -19,12 +19,12 @@ FP32, FP64 = 0, 1
 FLAG_LITERAL, FLAG_TENSOR_GRAM, FLAG_SKIP_VALIDATION, FLAG_ABSDIFF = 1, 2, 4, 8
 FLAG_NO_TAIL, FLAG_ALL_TAIL, FLAG_NO_TENSOR, FLAG_NO_MID, FLAG_SPARSE_STRIPE, FLAG_RICHNESS_ZONES = 16, 32, 64, 128, 256, 512
 
-ABI_VERSION = 6          # unifrac_abi_version() of the header this binding was written against
+ABI_VERSION = 7          # unifrac_abi_version() of the header this binding was written against
 OK = 0
 ERR_INVALID_ARG, ERR_INVALID_TREE, ERR_INVALID_TABLE, ERR_EMPTY_SAMPLE = -1, -2, -3, -4
 ERR_WORKSPACE, ERR_CUDA, ERR_UNSUPPORTED = -5, -6, -7
 
-EXPORTS = ("unifrac_dm", "unifrac_dm_shard", "unifrac_shard_of_pair", "unifrac_dm_host", "unifrac_mantel_pearson", "unifrac_mantel_spearman", "unifrac_pcoa", "unifrac_measure_rates", "unifrac_last_stats", "unifrac_status_string",
+EXPORTS = ("unifrac_dm", "unifrac_dm_shard", "unifrac_shard_of_pair", "unifrac_dm_host", "unifrac_dm_host_multi", "unifrac_release_host_pool", "unifrac_mantel_pearson", "unifrac_mantel_spearman", "unifrac_pcoa", "unifrac_measure_rates", "unifrac_last_stats", "unifrac_status_string",
            "unifrac_last_cuda_error", "unifrac_abi_version")
 
 
@@ -90,6 +90,10 @@ def load(build_if_missing: bool = True) -> C.CDLL:
     lib.unifrac_dm_host.restype = C.c_int
     lib.unifrac_dm_host.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, CSR, C.c_int32, C.c_int, C.c_int,
                                     C.c_void_p, C.c_uint32]
+    lib.unifrac_dm_host_multi.restype = C.c_int
+    lib.unifrac_dm_host_multi.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, CSR, C.c_int32, C.c_int32,
+                                          C.POINTER(C.c_int32), C.c_int, C.POINTER(C.c_void_p), C.c_uint32]
+    lib.unifrac_release_host_pool.restype = C.c_int
     lib.unifrac_mantel_pearson.restype = C.c_int
     lib.unifrac_mantel_pearson.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_int32, C.c_void_p,
                                            ALLOC_FN, C.c_void_p, C.c_void_p]
@@ -181,6 +185,30 @@ def unifrac_dm_host(tree_parent, branch_len, postorder, indptr, indices, counts,
                              int(precision), out.ctypes.data, int(flags))
     _check(lib, rc)
     return out
+
+
+def unifrac_dm_host_multi(tree_parent, branch_len, postorder, indptr, indices, counts, n_samples: int, variants,
+                          precision: int, outs=None, flags: int = 0):
+    """Host entry point for several variants of one table (inputs uploaded once, result copies overlap the next
+    variant's compute).  Returns the list of condensed numpy arrays."""
+    lib = load()
+    a = [np.ascontiguousarray(tree_parent, np.int32), np.ascontiguousarray(branch_len, np.float64),
+         np.ascontiguousarray(postorder, np.int32), np.ascontiguousarray(indptr, np.int64),
+         np.ascontiguousarray(indices, np.int32), np.ascontiguousarray(counts, np.int32)]
+    n, k = int(n_samples), len(variants)
+    if outs is None:
+        outs = [np.empty(n * (n - 1) // 2, dtype=np.float32 if precision == FP32 else np.float64) for _ in range(k)]
+    vs = (C.c_int32 * k)(*[int(v) for v in variants])
+    ptrs = (C.c_void_p * k)(*[o.ctypes.data for o in outs])
+    rc = lib.unifrac_dm_host_multi(int(a[0].shape[0]), a[0].ctypes.data, a[1].ctypes.data, a[2].ctypes.data,
+                                   CSR(a[3].ctypes.data, a[4].ctypes.data, a[5].ctypes.data), n, k, vs, int(precision), ptrs, int(flags))
+    _check(lib, rc)
+    return outs
+
+
+def unifrac_release_host_pool() -> None:
+    lib = load()
+    _check(lib, lib.unifrac_release_host_pool())
 
 
 def unifrac_last_stats() -> dict:

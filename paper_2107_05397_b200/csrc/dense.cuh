@@ -46,6 +46,18 @@ struct DenseParams {
     const double* hsum;           // k_dense16: [n_tiles*128] Rh_s = sum over the head rows of E_ks
 };
 
+// head rows in ascending n_v order: keys for the stable radix sort, then the reordered row list
+__global__ void k_head_keys(uint32_t n_head, const int32_t* __restrict__ hrows, const uint32_t* __restrict__ nv, uint32_t* __restrict__ key)
+{
+    const uint32_t h = blockIdx.x * blockDim.x + threadIdx.x;
+    if (h < n_head) key[h] = nv[hrows[h]];
+}
+__global__ void k_head_reorder(uint32_t n_head, const int32_t* __restrict__ hrows, const uint32_t* __restrict__ idx, int32_t* __restrict__ out)
+{
+    const uint32_t h = blockIdx.x * blockDim.x + threadIdx.x;
+    if (h < n_head) out[h] = hrows[idx[h]];
+}
+
 // dense head embedding: E[h][s] for head row h (node hrows[h]); one warp per (row, tile), lane l owns samples 4l..4l+3
 template <typename T>
 __global__ void __launch_bounds__(256)

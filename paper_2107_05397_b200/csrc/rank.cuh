@@ -35,7 +35,7 @@ template <> struct RankKey<double> {
     }
 };
 
-// plain unsigned keys (sample / row orderings inside unifrac_dm: perm.cuh, skip.cuh)
+// plain unsigned keys (sample / row orderings inside unifrac_dm: perm.cuh, zone.cuh)
 template <> struct RankKey<uint32_t> {
     using K = uint32_t;
     static constexpr int PASSES = 4;

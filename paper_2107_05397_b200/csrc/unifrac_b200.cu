@@ -26,6 +26,7 @@
 #include <vector>
 #include <algorithm>
 #include <queue>
+#include <mutex>
 
 using namespace ufb;
 
@@ -35,6 +36,7 @@ thread_local std::string g_cuda_err;
 thread_local unifrac_stats_t g_stats;
 thread_local unsigned long long* g_stats_pinned = nullptr;   // [2] stripe counters, pinned host
 thread_local cudaEvent_t g_stats_event = nullptr;
+thread_local int g_stats_event_dev = -1;                     // the device g_stats_event belongs to
 thread_local bool g_stats_pending = false;
 
 struct CudaFail { cudaError_t e; const char* what; int line; };
@@ -57,6 +59,7 @@ constexpr double QUANT_RATIO_BUDGET = 0.5 * QUANT_REL;
 // bump of caller-provided (or stream-ordered) device allocations
 struct Arena {
     unifrac_alloc_fn fn; void* user; cudaStream_t stream;
+    cudaMemPool_t pool = nullptr;          // alloc == NULL: this pool instead of the device's default one (unifrac_dm_host)
     std::vector<void*> owned;
     size_t total = 0;
     void* get(size_t bytes) {
@@ -65,7 +68,7 @@ struct Arena {
         void* p = nullptr;
         if (fn) { p = fn(bytes, user); if (!p) throw WorkspaceFail{}; }
         else {
-            cudaError_t e = cudaMallocAsync(&p, bytes, stream);
+            cudaError_t e = pool ? cudaMallocFromPoolAsync(&p, bytes, pool, stream) : cudaMallocAsync(&p, bytes, stream);
             if (e != cudaSuccess) { cudaGetLastError(); throw WorkspaceFail{}; }
             owned.push_back(p);
         }
@@ -472,15 +475,16 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             {
                 // fp32 accuracy: K order = ascending n_v (stable), so the few root-adjacent branches whose u~ is O(0.1) for every
                 // sample come last and are folded into fp64 stage by stage (k_dense) instead of swamping the fp32 partial
-                // sums that the thousands of small terms are added to
-                std::vector<int32_t> h_rows(head_rows);
-                std::vector<uint32_t> h_nv(n);
-                CU(cudaMemcpyAsync(h_rows.data(), hrows, sizeof(int32_t) * head_rows, cudaMemcpyDeviceToHost, st));
-                CU(cudaMemcpyAsync(h_nv.data(), nv, sizeof(uint32_t) * n, cudaMemcpyDeviceToHost, st));
-                CU(cudaStreamSynchronize(st));
-                std::stable_sort(h_rows.begin(), h_rows.end(), [&](int32_t a, int32_t b) { return h_nv[a] < h_nv[b]; });
-                CU(cudaMemcpyAsync(hrows, h_rows.data(), sizeof(int32_t) * head_rows, cudaMemcpyHostToDevice, st));
-                CU(cudaStreamSynchronize(st));
+                // sums that the thousands of small terms are added to.  Sorted on the device
+                // (stable radix sort, rank.cuh): no host work on the data path.
+                uint32_t* hkey = A.get_n<uint32_t>(head_rows);
+                int32_t* hsorted = A.get_n<int32_t>(head_rows);
+                k_head_keys<<<cdiv((long long)head_rows, TB), TB, 0, st>>>((uint32_t)head_rows, hrows, nv, hkey); CU_LAUNCH(); ++launches;
+                RankBufs RBh = make_rank_bufs<uint32_t>(A, head_rows, n_sm_dev);
+                const int hsrc = radix_sort<uint32_t>(hkey, head_rows, RBh, st);
+                launches += 12;
+                k_head_reorder<<<cdiv((long long)head_rows, TB), TB, 0, st>>>((uint32_t)head_rows, hrows, RBh.idx[hsrc], hsorted); CU_LAUNCH(); ++launches;
+                hrows = hsorted;
             }
             uint32_t* hpref = nullptr;
             if (weighted) {
@@ -705,6 +709,8 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
     if (use_gram) {
         if constexpr (std::is_same<T, float>::value) {
+            // (an H2D cudaMemcpyAsync from pageable memory returns once the source has been staged, so the host vectors of the
+            //  pair lists may go out of scope right after it: no synchronisation follows the launch of an a-5 kernel)
             std::vector<int2> h_pairs = blocked_pairs(n_tiles, 12, shard, n_shards);
             n_pairs = (uint32_t)h_pairs.size();
             int2* pairs = A.get_n<int2>(n_pairs);
@@ -728,7 +734,6 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
                 CU(cudaMemsetAsync(G.epoch_cnt, 0, sizeof(unsigned int) * n_ep, st));
             }
             if (grid) { k_gram<<<grid, GRAM_THREADS, GRAM_SMEM, st>>>(tmA, tmB0, tmB1, tmB2, G); CU_LAUNCH(); ++launches; ++stripe_launches; }
-            CU(cudaStreamSynchronize(st));       // h_pairs staging copy done before it goes out of scope
         }
     } else if (skip_on) {
         if constexpr (std::is_same<T, float>::value) {
@@ -753,7 +758,6 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             uint32_t* cta_off = A.get_n<uint32_t>(grid + 1);
             CU(cudaMemcpyAsync(pairs, h_pairs.data(), sizeof(int2) * n_pairs, cudaMemcpyHostToDevice, st));
             CU(cudaMemcpyAsync(cta_off, h_off.data(), sizeof(uint32_t) * (grid + 1), cudaMemcpyHostToDevice, st));
-            CU(cudaStreamSynchronize(st));           // staging copies of the host vectors are done
             CUtensorMap tmE = make_rowmajor_map(sk_E, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, sizeof(float), Npad, sk_KE ? sk_KE : ZONE_BK, TILE, ZONE_BK,
                                                 CU_TENSOR_MAP_SWIZZLE_NONE);
             ZoneParams SP{};
@@ -785,7 +789,6 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             CU(cudaFuncSetAttribute(k_dense<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             if (grid) { k_dense<T><<<grid, DENSE_THREADS, smem, st>>>(tmE, D); CU_LAUNCH(); ++launches; ++stripe_launches; }
         }
-        CU(cudaStreamSynchronize(st));           // h_pairs staging copy done before it goes out of scope
     } else {
     std::vector<int2> h_pairs;
     h_pairs.reserve((size_t)n_tiles * (n_tiles + 1) / 2);
@@ -818,7 +821,6 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         P.scratch = A.get_n<double>((size_t)grid * 64 * 256);
         kern<<<grid, STRIPE_THREADS, smem, st>>>(P); CU_LAUNCH(); ++launches; ++stripe_launches;
     }
-    CU(cudaStreamSynchronize(st));           // h_pairs staging copy done before it goes out of scope
     }
     // ------------------------------------------------------------------ near-duplicate guard: listed pairs from the definition
     if (GL.pairs) {
@@ -837,7 +839,8 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     }
     // stripe counters -> pinned host block (read lazily by unifrac_last_stats)
     if (!g_stats_pinned) { CU(cudaHostAlloc(&g_stats_pinned, 4 * sizeof(unsigned long long), cudaHostAllocDefault)); }
-    if (!g_stats_event) { CU(cudaEventCreateWithFlags(&g_stats_event, cudaEventDisableTiming)); }
+    if (g_stats_event && g_stats_event_dev != dev_id) { cudaEventDestroy(g_stats_event); g_stats_event = nullptr; }    // thread moved to another GPU
+    if (!g_stats_event) { CU(cudaEventCreateWithFlags(&g_stats_event, cudaEventDisableTiming)); g_stats_event_dev = dev_id; }
     CU(cudaMemcpyAsync(g_stats_pinned, kstats, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
     CU(cudaMemcpyAsync(g_stats_pinned + 2, work + 18, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
     CU(cudaEventRecord(g_stats_event, st));
@@ -873,7 +876,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
 
 int guarded(int32_t n_nodes, const int32_t* parent, const double* len, const int32_t* postorder, unifrac_csr_t tab,
             int32_t N, unifrac_variant_t variant, unifrac_precision_t precision, void* out, unifrac_alloc_fn alloc,
-            void* user, uint32_t flags, cudaStream_t st, int shard = 0, int n_shards = 1)
+            void* user, uint32_t flags, cudaStream_t st, int shard = 0, int n_shards = 1, cudaMemPool_t pool = nullptr)
 {
     if (n_shards < 1 || n_shards > 255 || shard < 0 || shard >= n_shards) return UNIFRAC_ERR_INVALID_ARG;
     if (n_shards > 1 && (flags & (UNIFRAC_FLAG_LITERAL | UNIFRAC_FLAG_ABSDIFF | UNIFRAC_FLAG_SPARSE_STRIPE | UNIFRAC_FLAG_NO_TAIL)))
@@ -888,6 +891,7 @@ int guarded(int32_t n_nodes, const int32_t* parent, const double* len, const int
         return UNIFRAC_ERR_INVALID_ARG;
     if ((long long)N > (1ll << 23)) return UNIFRAC_ERR_UNSUPPORTED;
     Arena A{alloc, user, st};
+    A.pool = pool;
     int rc = UNIFRAC_OK;
     const bool w = variant == UNIFRAC_WEIGHTED_NORMALIZED;
     try {
@@ -1068,36 +1072,61 @@ int32_t unifrac_shard_of_pair(int32_t i, int32_t j, int32_t shard_count)
     return shard_of_tiles(a / TILE, b / TILE, shard_count);
 }
 
-int unifrac_dm_host(int32_t n_nodes, const int32_t* tree_parent, const double* branch_len, const int32_t* postorder,
-                    unifrac_csr_t th, int32_t N, unifrac_variant_t variant, unifrac_precision_t precision,
-                    void* out_host, uint32_t flags)
+// the library's own stream-ordered pool for the host entry points (one per device, created on first use; it keeps what it
+// has mapped between calls -- release threshold = max -- and unifrac_release_host_pool gives it back)
+static cudaMemPool_t g_host_pool[64] = {};
+static cudaMemPool_t host_pool(int dev)
 {
-    if (!tree_parent || !branch_len || !postorder || !th.indptr || !th.indices || !th.counts || !out_host) return UNIFRAC_ERR_INVALID_ARG;
-    if (n_nodes < 2 || N < 2) return UNIFRAC_ERR_INVALID_ARG;
+    if (dev < 0 || dev >= 64) return nullptr;
+    static std::mutex mu;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!g_host_pool[dev]) {
+        cudaMemPoolProps props{};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        cudaMemPool_t pool = nullptr;
+        if (cudaMemPoolCreate(&pool, &props) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+        uint64_t keep = UINT64_MAX;
+        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        g_host_pool[dev] = pool;
+    }
+    return g_host_pool[dev];
+}
+
+int unifrac_dm_host_multi(int32_t n_nodes, const int32_t* tree_parent, const double* branch_len, const int32_t* postorder,
+                          unifrac_csr_t th, int32_t N, int32_t n_variants, const int32_t* variants, unifrac_precision_t precision,
+                          void* const* outs_host, uint32_t flags)
+{
+    if (!tree_parent || !branch_len || !postorder || !th.indptr || !th.indices || !th.counts || !outs_host || !variants) return UNIFRAC_ERR_INVALID_ARG;
+    if (n_nodes < 2 || N < 2 || n_variants < 1 || n_variants > 2) return UNIFRAC_ERR_INVALID_ARG;
+    for (int k = 0; k < n_variants; ++k)
+        if (!outs_host[k] || (variants[k] != UNIFRAC_UNWEIGHTED && variants[k] != UNIFRAC_WEIGHTED_NORMALIZED)) return UNIFRAC_ERR_INVALID_ARG;
     if (precision != UNIFRAC_FP32 && precision != UNIFRAC_FP64) return UNIFRAC_ERR_INVALID_ARG;
     const int64_t nnz = th.indptr[N];
     if (nnz < 0) return UNIFRAC_ERR_INVALID_TABLE;
     const size_t esz = precision == UNIFRAC_FP32 ? 4 : 8;
     const size_t n_out = (size_t)N * (N - 1) / 2;
-    cudaStream_t st = nullptr;
-    void *d_parent = nullptr, *d_len = nullptr, *d_post = nullptr, *d_indptr = nullptr, *d_idx = nullptr, *d_cnt = nullptr, *d_out = nullptr;
+    cudaStream_t st = nullptr, cs = nullptr;
+    cudaEvent_t done[2] = {nullptr, nullptr};
+    void *d_parent = nullptr, *d_len = nullptr, *d_post = nullptr, *d_indptr = nullptr, *d_idx = nullptr, *d_cnt = nullptr;
+    void* d_out[2] = {nullptr, nullptr};
     int rc = UNIFRAC_OK;
     auto ok = [&](cudaError_t e) { if (e != cudaSuccess && rc == UNIFRAC_OK) { g_cuda_err = cudaGetErrorString(e); cudaGetLastError(); rc = e == cudaErrorMemoryAllocation ? UNIFRAC_ERR_WORKSPACE : UNIFRAC_ERR_CUDA; } return rc == UNIFRAC_OK; };
-    ok(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
-    // All device memory of this call (inputs, output, workspace) comes from the device's stream-ordered pool; the pool keeps
-    // what it has mapped between calls (release threshold = max), so repeated calls do not pay for mapping ~20 GB again.
-    {
-        int dev = 0; cudaMemPool_t pool = nullptr;
-        if (ok(cudaGetDevice(&dev)) && ok(cudaDeviceGetDefaultMemPool(&pool, dev))) {
-            uint64_t keep = UINT64_MAX;
-            ok(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
-        }
+    int dev = 0;
+    ok(cudaGetDevice(&dev));
+    cudaMemPool_t pool = host_pool(dev);
+    if (!pool && rc == UNIFRAC_OK) { rc = UNIFRAC_ERR_CUDA; g_cuda_err = "cudaMemPoolCreate failed"; }
+    ok(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));        // compute (and the input copies)
+    ok(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));        // result copies: overlap the next variant's compute
+    auto dalloc = [&](void** p, size_t bytes) { return ok(cudaMallocFromPoolAsync(p, bytes ? bytes : 256, pool, st)); };
+    if (rc == UNIFRAC_OK) {
+        dalloc(&d_parent, sizeof(int32_t) * n_nodes) && dalloc(&d_len, sizeof(double) * n_nodes) &&
+        dalloc(&d_post, sizeof(int32_t) * n_nodes) && dalloc(&d_indptr, sizeof(int64_t) * ((size_t)N + 1)) &&
+        dalloc(&d_idx, sizeof(int32_t) * (size_t)nnz) && dalloc(&d_cnt, sizeof(int32_t) * (size_t)nnz);
+        for (int k = 0; k < n_variants; ++k) dalloc(&d_out[k], esz * n_out);
     }
-    auto dalloc = [&](void** p, size_t bytes) { return ok(cudaMallocAsync(p, bytes ? bytes : 256, st)); };
-    dalloc(&d_parent, sizeof(int32_t) * n_nodes) && dalloc(&d_len, sizeof(double) * n_nodes) &&
-    dalloc(&d_post, sizeof(int32_t) * n_nodes) && dalloc(&d_indptr, sizeof(int64_t) * ((size_t)N + 1)) &&
-    dalloc(&d_idx, sizeof(int32_t) * (size_t)nnz) && dalloc(&d_cnt, sizeof(int32_t) * (size_t)nnz) &&
-    dalloc(&d_out, esz * n_out);
     if (rc == UNIFRAC_OK) {
         ok(cudaMemcpyAsync(d_parent, tree_parent, sizeof(int32_t) * n_nodes, cudaMemcpyHostToDevice, st));
         ok(cudaMemcpyAsync(d_len, branch_len, sizeof(double) * n_nodes, cudaMemcpyHostToDevice, st));
@@ -1106,16 +1135,42 @@ int unifrac_dm_host(int32_t n_nodes, const int32_t* tree_parent, const double* b
         ok(cudaMemcpyAsync(d_idx, th.indices, sizeof(int32_t) * (size_t)nnz, cudaMemcpyHostToDevice, st));
         ok(cudaMemcpyAsync(d_cnt, th.counts, sizeof(int32_t) * (size_t)nnz, cudaMemcpyHostToDevice, st));
     }
-    if (rc == UNIFRAC_OK) {
+    for (int k = 0; k < n_variants && rc == UNIFRAC_OK; ++k) {
         unifrac_csr_t td{reinterpret_cast<const int64_t*>(d_indptr), reinterpret_cast<const int32_t*>(d_idx), reinterpret_cast<const int32_t*>(d_cnt)};
         rc = guarded(n_nodes, reinterpret_cast<const int32_t*>(d_parent), reinterpret_cast<const double*>(d_len),
-                     reinterpret_cast<const int32_t*>(d_post), td, N, variant, precision, d_out, nullptr, nullptr, flags, st);
+                     reinterpret_cast<const int32_t*>(d_post), td, N, (unifrac_variant_t)variants[k], precision, d_out[k], nullptr, nullptr,
+                     flags, st, 0, 1, pool);
+        if (rc != UNIFRAC_OK) break;
+        // unifrac_dm returns once the a-5 kernels are enqueued: the copy waits for them on its own stream
+        ok(cudaEventCreateWithFlags(&done[k], cudaEventDisableTiming));
+        if (rc == UNIFRAC_OK) {
+            ok(cudaEventRecord(done[k], st));
+            ok(cudaStreamWaitEvent(cs, done[k], 0));
+            ok(cudaMemcpyAsync(outs_host[k], d_out[k], esz * n_out, cudaMemcpyDeviceToHost, cs));
+        }
     }
-    if (rc == UNIFRAC_OK) {
-        ok(cudaMemcpyAsync(out_host, d_out, esz * n_out, cudaMemcpyDeviceToHost, st));
-    }
-    for (void* p : {d_parent, d_len, d_post, d_indptr, d_idx, d_cnt, d_out}) if (p && st) cudaFreeAsync(p, st);
+    if (cs) ok(cudaStreamSynchronize(cs));
+    for (void* p : {d_parent, d_len, d_post, d_indptr, d_idx, d_cnt, d_out[0], d_out[1]}) if (p && st) cudaFreeAsync(p, st);
     if (st) { ok(cudaStreamSynchronize(st)); cudaStreamDestroy(st); }
+    if (cs) cudaStreamDestroy(cs);
+    for (auto& e : done) if (e) cudaEventDestroy(e);
+    return rc;
+}
+
+int unifrac_dm_host(int32_t n_nodes, const int32_t* tree_parent, const double* branch_len, const int32_t* postorder,
+                    unifrac_csr_t th, int32_t N, unifrac_variant_t variant, unifrac_precision_t precision,
+                    void* out_host, uint32_t flags)
+{
+    const int32_t v = (int32_t)variant;
+    void* outs[1] = {out_host};
+    return unifrac_dm_host_multi(n_nodes, tree_parent, branch_len, postorder, th, N, 1, &v, precision, outs, flags);
+}
+
+int unifrac_release_host_pool(void)
+{
+    int rc = UNIFRAC_OK;
+    for (int d = 0; d < 64; ++d)
+        if (g_host_pool[d] && cudaMemPoolTrimTo(g_host_pool[d], 0) != cudaSuccess) { cudaGetLastError(); rc = UNIFRAC_ERR_CUDA; }
     return rc;
 }
 
@@ -1285,6 +1340,6 @@ const char* unifrac_status_string(int status)
 }
 
 const char* unifrac_last_cuda_error(void) { return g_cuda_err.c_str(); }
-int unifrac_abi_version(void) { return 6; }
+int unifrac_abi_version(void) { return 7; }
 
 }  // extern "C"

@@ -331,3 +331,38 @@ def test_two_shards_on_two_streams_merge_to_the_oracle_matrix(B, O, variant):
     assert int(torch.count_nonzero((a != 0) & (b != 0))) == 0          # disjoint owners
     assert int(torch.count_nonzero(a)) > 0 and int(torch.count_nonzero(b)) > 0
     check((a + b).cpu().numpy().astype(np.float64), want, 0)
+
+
+def test_unifrac_dm_returns_before_the_stripe_kernel_finishes(B):
+    """include/unifrac_b200.h: "after planning and embedding the stripe kernel is enqueued asynchronously and the call returns
+    without waiting for it".  Medium-sized weighted call (~100 ms of a-5 kernels): an event recorded right after the call
+    returns has not completed yet; the result is still correct once it has."""
+    import torch
+    cfg = synth.CONFIGS["medium"]
+    p = synth.make_problem(30000, 6000, 0.05, 1.05, cfg[4], cfg[5], seed=2)
+    args = B.to_device(p)
+    B.unifrac_dm(*args, p.n_samples, W, B.FP32)                      # warm-up (module load, allocator)
+    torch.cuda.synchronize()
+    ev = torch.cuda.Event()
+    out = B.unifrac_dm(*args, p.n_samples, W, B.FP32)
+    ev.record()
+    pending = not ev.query()
+    torch.cuda.synchronize()
+    assert pending, "unifrac_dm waited for its a-5 kernels"
+    assert bool(torch.isfinite(out).all()) and float(out.max()) <= 1.0
+
+
+def test_host_multi_matches_device_entry_point(B, O):
+    """unifrac_dm_host_multi (both variants, inputs uploaded once, result copies overlapping the next variant's compute)
+    returns what unifrac_dm returns; unifrac_release_host_pool afterwards."""
+    import torch
+    cfg = synth.CONFIGS["small"]
+    p = synth.make_problem(3000, 300, 0.1, 1.1, cfg[4], cfg[5], seed=4)
+    outs = B.unifrac_dm_host_multi(p.parent, p.branch_len, p.postorder, p.indptr, p.indices, p.counts, p.n_samples, [U, W], B.FP32)
+    for v, got in zip((U, W), outs):
+        dev = gpu_dm(B, p, v, 0)
+        assert np.array_equal(got.astype(np.float64), dev)
+        check(got.astype(np.float64), O.all_pairs(p.parent, p.branch_len, p.indptr, p.indices, p.counts, v), 0)
+    one = B.unifrac_dm_host(p.parent, p.branch_len, p.postorder, p.indptr, p.indices, p.counts, p.n_samples, W, B.FP64)
+    check(one, O.all_pairs(p.parent, p.branch_len, p.indptr, p.indices, p.counts, W), 1)
+    B.unifrac_release_host_pool()

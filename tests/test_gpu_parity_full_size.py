@@ -1,7 +1,9 @@
 """Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (device
 entry point, fp32, default flags): sampled outputs the oracle computes one by one (pair-list
-driver) plus structured pairs (first/last rows, tile-boundary neighbours, last condensed
-element), and properties that hold at any size (range, no NaN)."""
+driver): 200,000 seeded pairs, ALL 32,640 pairs among 256 seeded samples (a clique: it puts
+many pairs into the same tile pairs, which is what catches a wrong cell inside one tile pair),
+structured pairs (first/last rows, tile-boundary neighbours, last condensed element) -- SURVEY
+8(c) "Large configs" -- and properties that hold at any size (range, no NaN)."""
 import numpy as np
 import pytest
 
@@ -16,7 +18,13 @@ def _structured_pairs(n):
     return np.array([p for p in e if 0 <= p[0] < p[1] < n], dtype=np.int32)
 
 
-@pytest.mark.parametrize("name,n_pairs", [("medium", 20000), ("emp", 20000), ("large", 20000)])
+def _clique_pairs(n, k=256, seed=17):
+    members = np.sort(np.random.default_rng(seed).choice(n, size=min(k, n), replace=False))
+    i, j = np.triu_indices(len(members), 1)
+    return np.stack([members[i], members[j]], 1).astype(np.int32)
+
+
+@pytest.mark.parametrize("name,n_pairs", [("medium", 200000), ("emp", 200000), ("large", 200000)])
 def test_full_size_sampled_pairs(name, n_pairs):
     import torch
     from paper_2107_05397_b200 import binding as B
@@ -26,7 +34,7 @@ def test_full_size_sampled_pairs(name, n_pairs):
         pytest.skip("needs ~80 GB of free HBM")
     p = synth.make_config(name, seed=0)
     n = p.n_samples
-    pairs = np.concatenate([synth.sample_pairs(n, n_pairs, seed=1), _structured_pairs(n)])
+    pairs = np.concatenate([synth.sample_pairs(n, n_pairs, seed=1), _clique_pairs(n), _structured_pairs(n)])
     idx = torch.from_numpy(synth.condensed_index(n, pairs[:, 0], pairs[:, 1])).cuda()
     args = B.to_device(p)
     variants = (0,) if name == "medium" else (0, 1)
