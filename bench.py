@@ -42,8 +42,8 @@ SMEM_ATOMIC_PER_S, L2_RED_PER_S = 8.84 * SM_COUNT * SM_MAX_GHZ * 1e9, 1.94e11
 # dram__bytes_read.sum + dram__bytes_write.sum per launch, copied from the ncu --set full captures summarised in the file
 # TRAFFIC_SOURCE names (default flags, seed 0; k_mid: mean of the unweighted and the weighted launch); not measured by this
 # run -- other workloads and kernels that changed since the capture report null
-TRAFFIC_SOURCE = "profiles/r01_summary.md (ncu --set full, round-1 kernels)"
-NCU_TRAFFIC_BYTES = {"large": {"k_gram": 300.1e9, "k_mid": 240.2e9}}
+TRAFFIC_SOURCE = "profiles/r02_summary.md (ncu --set full captures of this round's kernels, Large, seed 0)"
+NCU_TRAFFIC_BYTES = {"large": {"k_dense16": 225.3e9, "k_gram": 300.1e9, "k_mid": 240.1e9, "k_zone": 307.1e9}}
 
 WORKLOADS = {   # name -> (variants, precision)    BASELINE.json:7-11
     "tiny": ((0, 1), 1), "small": ((0, 1), 1), "medium": ((0,), 0), "emp": ((0, 1), 0), "large": ((0, 1), 0),
@@ -430,7 +430,8 @@ def main():
     # (1) k_dense (default) / k_stripe (debug forms): CUDA-core register-tile kernel (head branches; weighted, fp64, or NO_TENSOR)
     ss = [s for s in flat if not s["gram"]]
     if ss:
-        kname = ("k_dense16" if precision == 0 else "k_dense") if all(s["dense"] for s in ss) else "k_stripe"
+        kname = "k_zone" if all(s["skip"] for s in ss) else \
+                ("k_dense16" if precision == 0 else "k_dense") if all(s["dense"] for s in ss) else "k_stripe"
         t = sum(s["ms_stripe"] for s in ss) * 1e-3
         w_exec = sum(s["updates_executed_head"] for s in ss)
         nl = sum(s["stripe_launches"] for s in ss)
