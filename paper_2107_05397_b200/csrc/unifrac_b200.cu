@@ -139,6 +139,34 @@ struct Timer {
     float ms(int a, int b) { float m = 0; if (on && b < n) cudaEventElapsedTime(&m, ev[a], ev[b]); return m; }
 };
 
+// per-device scale factors of the cost-model rates (see run(): "The kernel rates below ...")
+struct Calib { double f_atom = 1.0, f_red = 1.0, f_alu = 1.0; };
+Calib calibration(int dev, cudaStream_t st)
+{
+    static std::mutex mu;
+    static Calib cache[64];
+    static bool have[64] = {};
+    if (dev < 0 || dev >= 64) return Calib{};
+    std::lock_guard<std::mutex> lock(mu);
+    if (!have[dev]) {
+        have[dev] = true;                                   // a failed probe leaves the reference rates in place
+        const char* e = getenv("UNIFRAC_B200_CALIBRATE");
+        if (!e || atoi(e) != 0) {
+            unifrac_rates_t r{};
+            if (unifrac_measure_rates(&r, st) == UNIFRAC_OK) {
+                auto q = [](double measured, double ref) {
+                    const double f = std::round(4.0 * measured / ref) / 4.0;
+                    return f < 0.25 ? 0.25 : f > 4.0 ? 4.0 : f;
+                };
+                cache[dev].f_atom = q(r.smem_atomic_random_per_s, 2.57e12);     // 8.84 lanes/clk/SM x 148 SMs x 1.965 GHz
+                cache[dev].f_red = q(r.l2_red_random_per_s, 1.94e11);
+                cache[dev].f_alu = q(r.fmnmx_fadd_per_s, 3.48e13);
+            }
+        }
+    }
+    return cache[dev];
+}
+
 // stable LSD radix sort of (key, position) pairs (rank.cuh); the sort buffers are shared between the sorts of a call
 struct RankBufs { void* keys[2]; uint32_t* idx[2]; uint32_t* hist; uint32_t* offs; uint32_t* blast; unsigned nb; unsigned long long per_block; };
 template <typename T>
@@ -332,11 +360,15 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     const int n_tiles = cdiv(N, TILE);
     const double Pd = 0.5 * (double)N * (double)(N - 1), n_tp = 0.5 * (double)n_tiles * (n_tiles + 1);
     auto envd = [](const char* k, double d) { const char* e = getenv(k); return e ? atof(e) : d; };
-    const double R_tail = envd("UNIFRAC_B200_R_TAIL", 1.6e11), R_mid = envd("UNIFRAC_B200_R_MID", 1.6e12);
-    const double R_head = envd("UNIFRAC_B200_R_HEAD", std::is_same<T, float>::value ? 1.4e13 : 3.3e12), gram_Bps = envd("UNIFRAC_B200_GRAM_BPS", 1.15e13);
+    // The kernel rates below were measured on this pool's B200.  Once per process and device the unit rates they rest on
+    // (shared-memory atomics, L2 REDs, the FMNMX + FADD mix) are probed (unifrac_measure_rates, ~20 ms) and the kernel rates
+    // are scaled by measured / reference, in steps of 1/4 so that probe noise cannot move the split (on a B200: all 1.0).
+    const Calib cal = calibration(dev_id, st);
+    const double R_tail = envd("UNIFRAC_B200_R_TAIL", 1.6e11 * cal.f_red), R_mid = envd("UNIFRAC_B200_R_MID", 1.6e12 * cal.f_atom);
+    const double R_head = envd("UNIFRAC_B200_R_HEAD", (std::is_same<T, float>::value ? 1.4e13 : 3.3e12) * cal.f_alu), gram_Bps = envd("UNIFRAC_B200_GRAM_BPS", 1.15e13);
     // the rows that compete with the Gram kernel are sparse (a few entries per tile), where k_mid's per-entry overhead
     // halves its update rate (measured 5.9e11 /s at Large against 1.3e12 - 1.6e12 /s for the denser rows of the weighted variant)
-    const double R_mid_head = gram ? envd("UNIFRAC_B200_R_MID_SPARSE", 5.5e11) : R_mid;
+    const double R_mid_head = gram ? envd("UNIFRAC_B200_R_MID_SPARSE", 5.5e11 * cal.f_atom) : R_mid;
     const double c_ent = envd("UNIFRAC_B200_MID_ENT_S", 3e-12);         // seconds per (mid entry, tile pair) visit of the join kernel
     const double head_s = gram ? n_tp * 512.0 / gram_Bps : Pd / R_head;  // seconds per head branch
     double c2_head, c2_mid;
