@@ -93,3 +93,30 @@ def test_full_size_sample_permutation_property(name):
         ok = (err <= 2e-5 * dp.abs()) | (err <= 2e-7)
         assert bool(ok.all()), f"{name} variant {variant}: max rel diff {float((err / dp.abs().clamp_min(1e-30)).max()):.3e}"
         print(f"{name} variant {variant}: permuted run max rel diff {float((err / dp.abs().clamp_min(1e-30)).max()):.3e}")
+
+
+def test_full_size_richness_zones_flag_emp_weighted():
+    """UNIFRAC_FLAG_RICHNESS_ZONES at the EMP-shaped size (196 tiles: permuted samples, 120k+ rows with a dense zone, k_zone +
+    join + tail + un-permute): 20,000 sampled + clique + structured pairs against the oracle, and agreement with the default
+    path on 5e6 pairs."""
+    import torch
+    from paper_2107_05397_b200 import binding as B
+    from oracle import oracle as O
+    p = synth.make_config("emp", seed=0)
+    n = p.n_samples
+    pairs = np.concatenate([synth.sample_pairs(n, 20000, seed=2), _clique_pairs(n, 128, seed=3), _structured_pairs(n)])
+    idx = torch.from_numpy(synth.condensed_index(n, pairs[:, 0], pairs[:, 1])).cuda()
+    want = O.pair_list(p.parent, p.branch_len, p.indptr, p.indices, p.counts, 1, pairs)
+    args = B.to_device(p)
+    out = B.unifrac_dm(*args, n, 1, B.FP32, flags=B.FLAG_RICHNESS_ZONES)
+    torch.cuda.synchronize()
+    st = B.unifrac_last_stats()
+    assert st["skip"] == 1 and st["skip_row_pair_visits"] > 0 and st["mid_updates"] > 0
+    got = out[idx].cpu().numpy().astype(np.float64)
+    err = np.abs(got - want)
+    assert ((err <= 1e-5 * np.abs(want)) | (err <= 1e-7)).all(), f"max rel err {(err / np.maximum(want, 1e-30)).max():.3e}"
+    ref = B.unifrac_dm(*args, n, 1, B.FP32)
+    big = torch.from_numpy(synth.condensed_index(n, *synth.sample_pairs(n, 5_000_000, seed=6).T)).cuda()
+    d = (out[big].double() - ref[big].double()).abs()
+    assert bool(((d <= 2e-5 * ref[big].double()) | (d <= 2e-7)).all())
+    print(f"zones vs oracle max rel err {(err / np.maximum(want, 1e-30)).max():.3e}; vs default path max abs diff {float(d.max()):.3e}")
