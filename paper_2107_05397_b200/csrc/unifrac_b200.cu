@@ -487,7 +487,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     const bool dense16 = dense_head && std::is_same<T, float>::value && envd("UNIFRAC_B200_DENSE16", 1) != 0;   // fp32: 16 consumer warps, mixed forms
     // skip path (zone.cuh)
     uint32_t sk_n = 0, sk_KE = 0;
-    int32_t* sk_rows = nullptr; uint32_t* sk_base = nullptr; uint32_t* sk_len = nullptr; uint32_t* sk_cut = nullptr; float* sk_E = nullptr;
+    int32_t* sk_rows = nullptr; uint32_t* sk_base = nullptr; uint32_t* sk_len = nullptr; uint32_t* sk_cut = nullptr; float* sk_E = nullptr; double* sk_H = nullptr;
     std::vector<uint32_t> h_cut;
     unsigned long long h_skstat[2] = {0, 0};
     double* hsum = nullptr;
@@ -538,7 +538,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         unsigned long long* keys = A.get_n<unsigned long long>(sk_n);
         // cost model of k_row_cut in SM-clocks (measured on B200, sweeps in profiles/r02_summary.md; overridable for tuning):
         // one (row, tile pair) of k_zone, pair updates per clock of the join, one (entry, tile pair) visit of the join
-        CutModel CM{(float)env_double("UNIFRAC_B200_ZONE_C0", 330.0), (float)(0.5 / env_double("UNIFRAC_B200_JOIN_RATE", 4.64)),
+        CutModel CM{(float)env_double("UNIFRAC_B200_ZONE_C0", 310.0), (float)(0.5 / env_double("UNIFRAC_B200_JOIN_RATE", 4.64)),
                     (float)env_double("UNIFRAC_B200_JOIN_ENT", 0.87)};
         k_row_cut<<<cdiv(sk_n, ROWCUT_WARPS), ROWCUT_WARPS * 32, 0, st>>>(sk_n, lnode, bits, NW, n_tiles, (uint32_t)N, CM, keys); CU_LAUNCH(); ++launches;
         RankBufs RB = make_rank_bufs<unsigned long long>(A, sk_n, n_sm_dev);
@@ -565,6 +565,8 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             k_E_scatter<<<cdiv((long long)sk_KE * 32, TB), TB, 0, st>>>(sk_KE, sk_base, sk_len, ts, reinterpret_cast<const float*>(tv), sk_E, Npad);
             CU_LAUNCH(); ++launches;
         }
+        sk_H = A.get_n<double>((size_t)n_tiles * Npad);
+        k_zone_hsum<<<cdiv((long long)Npad, 128), 128, 0, st>>>(sk_E, Npad, n_tiles, sk_cut, sk_H); CU_LAUNCH(); ++launches;
         embed_rows = (uint64_t)sk_KE * n_tiles;
     } else if (!use_gram) {
         rflags = A.get_n<uint32_t>((size_t)n_tiles * nwords);
@@ -793,7 +795,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             CUtensorMap tmE = make_rowmajor_map(sk_E, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, sizeof(float), Npad, sk_KE ? sk_KE : ZONE_BK, TILE, ZONE_BK,
                                                 CU_TENSOR_MAP_SWIZZLE_NONE);
             ZoneParams SP{};
-            SP.pairs = pairs; SP.cta_off = cta_off; SP.cut = sk_cut; SP.sums = sums; SP.n_samples = N;
+            SP.pairs = pairs; SP.cta_off = cta_off; SP.cut = sk_cut; SP.H = sk_H; SP.Npad = Npad; SP.sums = sums; SP.n_samples = N;
             SP.out = reinterpret_cast<float*>(out); SP.add_out = 1; SP.guard = GL;
             SP.scratch = A.get_n<double>((size_t)grid * 32 * 512);
             CU(cudaFuncSetAttribute(k_zone, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZONE_SMEM));

@@ -139,12 +139,37 @@ k_E_scatter(uint32_t K_E, const uint32_t* __restrict__ mbase, const uint32_t* __
 }
 
 
+// H[I][s] = sum over the rows r < cut[I] of E[r][s] (fp64): the half-sum k_zone's "direct" cells need back (see k_zone).
+// One thread per sample column walks the rows in groups of 32 (cut[] are multiples of 32, non-decreasing in I).
+__global__ void __launch_bounds__(128)
+k_zone_hsum(const float* __restrict__ E, size_t Npad, int n_tiles, const uint32_t* __restrict__ cut, double* __restrict__ H)
+{
+    const size_t s = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= Npad) return;
+    double run = 0.0;
+    uint32_t r = 0;
+    for (int I = 0; I < n_tiles; ++I) {
+        const uint32_t c = cut[I];
+        for (; r < c; r += 32) {
+            float v[32];
+#pragma unroll
+            for (int j = 0; j < 32; ++j) v[j] = E[(size_t)(r + j) * Npad + s];
+            double g = 0.0;
+#pragma unroll
+            for (int j = 0; j < 32; ++j) g += (double)v[j];
+            run += g;
+        }
+        H[(size_t)I * Npad + s] = run;
+    }
+}
+
 // ------------------------------------------------------------------ k_zone
 // Same TMA / mbarrier pipeline as k_dense16 (dense.cuh): one persistent CTA per SM, 16 consumer warps + 1 producer warp,
 // BK = 32 rows of the two 128-sample column blocks per stage; the number of stages is per tile pair: cut[I] / 32.
 // Consumer warp w owns the 8 samples 8w .. 8w+7 of tile I (rows of the output tile; two broadcast LDS.128 per staged row)
-// against all 128 samples of tile J: lane l holds columns 4l .. 4l+3 (one LDS.128), acc[8][4]: 32 FMNMX (ALU pipe) + 16
-// packed adds (add.f32x2 -> FADD2, FMA pipe) per staged row and warp; the epilogue writes 512 contiguous bytes per row.
+// against all 128 samples of tile J: lane l holds columns 4l .. 4l+3 (one LDS.128), acc[8][4]: 24 FMNMX (ALU pipe) + 12
+// packed adds (add.f32x2 -> FADD2) + 8 FADD + 8 FFMA (direct cells) per staged row and warp; the epilogue writes 512
+// contiguous bytes per row.
 // The tile pairs of a CTA are a host-balanced list (least-loaded CTA first over cut[I] stages), cta_off[b] .. cta_off[b+1].
 constexpr int ZONE_THREADS = 544;
 constexpr int ZONE_BK = 32, ZONE_STAGES = 4, ZONE_FLUSH = 16, ZONE_FIRST_EVERY = 8;
@@ -158,8 +183,19 @@ struct ZoneParams {
     float* out;                   // condensed (position space); holds the join / tail sums when add_out
     int add_out;
     double* scratch;              // [grid][32][512] fp64 partial sums
+    const double* H;              // [n_tiles][Npad] H[I][s] = sum_{r < cut[I]} E[r][s] (k_zone_hsum)
+    size_t Npad;
     GuardList guard;
 };
+
+// the warp's samples 6 and 7 ("direct" cells, 8 of a thread's 32): acc += -1/2 |a - b|  (FADD + FFMA, both on the FMA pipe);
+// min(p, q) = (p + q) / 2 - |p - q| / 2, so the epilogue adds (H[I][i] + H[I][j]) / 2 back.  The other 24 cells take FMNMX on
+// the half-rate ALU pipe + packed adds: the same pipe balance as k_dense16 (dense.cuh).
+__device__ __forceinline__ void zone_row4_direct(float (&acc)[4], float a, const float4& b) {
+    acc[0] = fmaf(fabsf(a - b.x), -0.5f, acc[0]); acc[1] = fmaf(fabsf(a - b.y), -0.5f, acc[1]);
+    acc[2] = fmaf(fabsf(a - b.z), -0.5f, acc[2]); acc[3] = fmaf(fabsf(a - b.w), -0.5f, acc[3]);
+}
+__device__ __forceinline__ constexpr bool zone_direct_row(int a) { return a >= 6; }
 
 __device__ __forceinline__ void zone_row4(float (&acc)[4], float a, const float4& b) {
     add2(acc[0], acc[1], fminf(a, b.x), fminf(a, b.y));
@@ -230,7 +266,7 @@ k_zone(const __grid_constant__ CUtensorMap tmE, const ZoneParams P)
                 const float4 a1 = *reinterpret_cast<const float4*>(row + i_off + 4);
                 const float4 b = *reinterpret_cast<const float4*>(row + j_off);
                 zone_row4(acc[0], a0.x, b); zone_row4(acc[1], a0.y, b); zone_row4(acc[2], a0.z, b); zone_row4(acc[3], a0.w, b);
-                zone_row4(acc[4], a1.x, b); zone_row4(acc[5], a1.y, b); zone_row4(acc[6], a1.z, b); zone_row4(acc[7], a1.w, b);
+                zone_row4(acc[4], a1.x, b); zone_row4(acc[5], a1.y, b); zone_row4_direct(acc[6], a1.z, b); zone_row4_direct(acc[7], a1.w, b);
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(empty(stage));
@@ -254,17 +290,20 @@ k_zone(const __grid_constant__ CUtensorMap tmE, const ZoneParams P)
         }
         // ----------------------------------------------------------- a-6 finalize (epilogue of the tile pair)
         const long long N = P.n_samples;
-        double sj[4];
+        double sj[4], hj[4];
+        const double* Hrow = P.H + (size_t)ij.x * P.Npad;            // sums over the rows [0, cut[I]) this pair ran
 #pragma unroll
-        for (int b = 0; b < 4; ++b) sj[b] = P.sums[ij.y * TILE + lane * 4 + b];
+        for (int b = 0; b < 4; ++b) { sj[b] = P.sums[ij.y * TILE + lane * 4 + b]; hj[b] = Hrow[ij.y * TILE + lane * 4 + b]; }
 #pragma unroll
         for (int a = 0; a < 8; ++a) {
             const long long gi = (long long)ij.x * TILE + i_off + a;
             const double si = P.sums[gi];
+            const double hi = zone_direct_row(a) ? Hrow[gi] : 0.0;
             const long long rowbase = gi * (2 * N - gi - 1) / 2 - gi - 1;
 #pragma unroll
             for (int b = 0; b < 4; ++b) {
                 double tot = (double)acc[a][b];
+                if (zone_direct_row(a)) tot += 0.5 * (hi + hj[b]);
                 if (scratch_live) tot += my_scratch[(size_t)(a * 4 + b) * 512];
                 acc[a][b] = 0.f;
                 const long long gj = (long long)ij.y * TILE + lane * 4 + b;
