@@ -476,7 +476,10 @@ def main():
         rl.append(dict(bound="smem_atomic", achieved=mu / t / 1e9 if t > 0 else 0.0, peak=ATOMS_PEAK / 1e9, unit="GATOM/s",
                        frac=mu / t / ATOMS_PEAK if t > 0 else 0.0, traffic=None, kernel="k_mid", launches=nl,
                        ms_per_launch=1e3 * t / max(1, nl), seconds=t, share_of_step=t / step_s,
-                       note="ms_mid also covers the mid list preparation kernels (k_mid_seg/off/pack)",
+                       frac_of_fp32_lane_roofline=(2.0 * mu / t / (ALU_PEAK_TFLOPS * 1e12)) if t > 0 else 0.0,
+                       note="ms_mid also covers the mid list preparation kernels (k_mid_seg/off/pack); frac_of_fp32_lane_roofline = "
+                            "2 lane-ops per update against the FP32-lane peak of SURVEY 8(d): the atomic unit retires 8.8 of 128 lanes "
+                            "per clock, so this design cannot exceed 0.069 there",
                        peak_source=f"shared-memory u32 atomic adds on random cells of a 128 x 128 tile, 3 CTAs/SM x 512 threads "
                                    f"(= {ATOMS_PEAK / SM_COUNT / SM_MAX_GHZ / 1e9:.2f} lane-ops/clk/SM; same rate conflict-free), {rates_src}"))
     for r in rl:
