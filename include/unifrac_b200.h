@@ -231,9 +231,9 @@ int unifrac_mantel_pearson(int32_t n_samples, const void *x_condensed, const voi
  * two condensed vectors, tied values sharing the mean of the ranks they span (1-based fractional ranking, DESIGN.md readings
  * M5-M6); a permutation of the objects only moves entries around, so every rho_k is Pearson's r between the permuted rank
  * matrix of X and the ranks of y.  Arguments, output layout, p-values and error behaviour are those of unifrac_mantel_pearson.
- * The ranks come from a stable LSD radix sort of (value, position) pairs on the device (no library sort); they are held in
- * fp64.  Workspace: ~2 x (key + position) x n(n-1)/2 for the sort, 2 x 8 x n(n-1)/2 for the ranks, 8 n^2 for the square copy.
- * n(n-1)/2 >= 2^32 - 1: UNIFRAC_ERR_UNSUPPORTED.  NaNs are not supported.  Asynchronous on `stream`.
+ * The ranks come from a stable LSD radix sort of (value, position) pairs on the device (no library sort); they are held as
+ * exact 32-bit integers (twice the average rank).  Workspace: ~2 x (key + position) x n(n-1)/2 for the sort, 2 x 4 x n(n-1)/2
+ * for the ranks, 4 n^2 for the square copy.  n(n-1)/2 >= 2^31 - 1 (n > 65,535): UNIFRAC_ERR_UNSUPPORTED.  NaNs are not supported.  Asynchronous on `stream`.
  */
 int unifrac_mantel_spearman(int32_t n_samples, const void *x_condensed, const void *y_condensed,
                             unifrac_precision_t precision, const int32_t *perms, int32_t n_perms, double *out,

@@ -3,8 +3,8 @@
 // minutes", readings M5-M6).  Spearman's rho is Pearson's r of the RANKS, ties sharing the mean of the
 // ranks they span, so the device path is: a stable LSD radix sort of (key, position) pairs -- hand-written, 8-bit digits,
 // no cub / thrust --, a prefix-max scan that gives every sorted position the start of its run of equal keys, and a scatter
-// of  rank = start + (run length - 1) / 2 + 1  (1-based, fp64: half-integers up to 2^32 are exact) back to the original
-// positions.  k_mantel_perm (mantel.cuh) then runs unchanged on the two rank vectors.
+// of  2 x rank = 2 start + (run length - 1) + 2  (1-based average ranks are half-integers, so twice the rank is an exact uint32)
+// back to the original positions.  k_mantel_perm (mantel.cuh) then runs unchanged on the two integer vectors (fp64 sums).
 // Bound: HBM.  One pass moves 4 + 8 + 8 bytes per element (histogram read, scatter read + write of key and position).
 #pragma once
 #include "common.cuh"
@@ -206,14 +206,16 @@ k_rank_starts(const K* __restrict__ keys, unsigned long long P, unsigned long lo
     }
 }
 
-// rank[idx[p]] = start[p] + (rlen[start[p]] - 1) / 2 + 1     (1-based average rank, exact in fp64)
+// rank2[idx[p]] = 2 * (average rank) = 2 start[p] + (rlen[start[p]] - 1) + 2     (1-based average ranks are half-integers:
+// twice the rank is an exact 32-bit integer for n(n-1)/2 < 2^31 - 1, half the bytes of an fp64 rank, and Pearson's r does
+// not see the factor 2)
 __global__ void __launch_bounds__(256)
 k_rank_write(const uint32_t* __restrict__ idx, const uint32_t* __restrict__ start, const uint32_t* __restrict__ rlen,
-             unsigned long long P, double* __restrict__ rank)
+             unsigned long long P, uint32_t* __restrict__ rank2)
 {
     for (unsigned long long p = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; p < P; p += (unsigned long long)gridDim.x * blockDim.x) {
         const uint32_t s = start[p];
-        rank[idx[p]] = (double)s + 0.5 * (double)(rlen[s] - 1u) + 1.0;
+        rank2[idx[p]] = 2u * s + (rlen[s] - 1u) + 2u;
     }
 }
 

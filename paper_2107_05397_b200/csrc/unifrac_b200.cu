@@ -202,9 +202,9 @@ int radix_sort(const T* v, unsigned long long P, const RankBufs& B, cudaStream_t
     }
     return src;
 }
-// average ranks (fp64, 1-based) of the P values v[] -> rank[]
+// twice the 1-based average ranks of the P values v[] (exact 32-bit integers) -> rank2[]
 template <typename T>
-void rank_transform(const T* v, unsigned long long P, double* rank, const RankBufs& B, cudaStream_t st)
+void rank_transform(const T* v, unsigned long long P, uint32_t* rank2, const RankBufs& B, cudaStream_t st)
 {
     using K = typename RankKey<T>::K;
     const int src = radix_sort<T>(v, P, B, st);
@@ -213,7 +213,7 @@ void rank_transform(const T* v, unsigned long long P, double* rank, const RankBu
     uint32_t* rlen = B.idx[src ^ 1];
     k_rank_block_heads<K><<<B.nb, RADIX_THREADS, 0, st>>>(keys[src], P, B.per_block, B.blast); CU_LAUNCH();
     k_rank_starts<K><<<B.nb, RADIX_THREADS, 0, st>>>(keys[src], P, B.per_block, B.blast, start, rlen); CU_LAUNCH();
-    k_rank_write<<<B.nb * 4, 256, 0, st>>>(B.idx[src], start, rlen, P, rank); CU_LAUNCH();
+    k_rank_write<<<B.nb * 4, 256, 0, st>>>(B.idx[src], start, rlen, P, rank2); CU_LAUNCH();
 }
 
 template <typename T>
@@ -995,16 +995,16 @@ template <typename T>
 void run_spearman(int32_t N, const T* x, const T* y, const int32_t* perms, int32_t K, double* out, Arena& A, cudaStream_t st)
 {
     const unsigned long long P = (unsigned long long)N * (N - 1) / 2;
-    if (P >= (1ull << 32) - 1) throw StatusFail{UNIFRAC_ERR_UNSUPPORTED};      // positions and ranks are kept in 32 bits
+    if (P >= (1ull << 31) - 1) throw StatusFail{UNIFRAC_ERR_UNSUPPORTED};      // positions and 2 x rank are kept in 32 bits
     int dev = 0, n_sm = 0;
     CU(cudaGetDevice(&dev));
     CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
     RankBufs B = make_rank_bufs<T>(A, P, n_sm);
-    double* rx = A.get_n<double>(P);
-    double* ry = A.get_n<double>(P);
+    uint32_t* rx = A.get_n<uint32_t>(P);
+    uint32_t* ry = A.get_n<uint32_t>(P);
     rank_transform<T>(x, P, rx, B, st);
     rank_transform<T>(y, P, ry, B, st);
-    run_mantel<double>(N, rx, ry, perms, K, out, A, st);
+    run_mantel<uint32_t>(N, rx, ry, perms, K, out, A, st);
 }
 
 // PCoA: block subspace iteration with Rayleigh-Ritz (pcoa.cuh).  Synchronous: the Ritz values are read back every
