@@ -84,6 +84,10 @@ k_radix_hist(const T* __restrict__ raw, const typename RankKey<T>::K* __restrict
 // stable scatter of one digit: offs = exclusive scan of hist (digit-major), i.e. the global position of the first element
 // of block b with digit d.  Tiles of the block's range are processed in order; within a tile warp w owns 512 consecutive
 // elements and handles them in 16 rounds of 32 (lane order = element order), so equal digits keep their input order.
+// The tile is first put into digit order in shared memory (local position = digit's offset in the tile + rank inside the
+// digit) and then written out by position: elements of one digit are adjacent there and go to adjacent global addresses, so
+// the stores are runs of ~16 elements instead of 32 unrelated words per warp instruction.
+template <typename K> constexpr size_t radix_scatter_smem() { return (size_t)RADIX_TILE * (sizeof(K) + sizeof(uint32_t)); }
 template <typename T, bool FIRST>
 __global__ void __launch_bounds__(RADIX_THREADS)
 k_radix_scatter(const T* __restrict__ raw, const typename RankKey<T>::K* __restrict__ keys_in, const uint32_t* __restrict__ idx_in,
@@ -91,8 +95,13 @@ k_radix_scatter(const T* __restrict__ raw, const typename RankKey<T>::K* __restr
                 typename RankKey<T>::K* __restrict__ keys_out, uint32_t* __restrict__ idx_out)
 {
     using K = typename RankKey<T>::K;
-    __shared__ uint32_t gbase[256];
+    extern __shared__ __align__(16) unsigned char rsm[];
+    K* skey = reinterpret_cast<K*>(rsm);
+    uint32_t* sidx = reinterpret_cast<uint32_t*>(rsm + (size_t)RADIX_TILE * sizeof(K));
+    __shared__ uint32_t gbase[256];               // global position of the block's next element of digit d
+    __shared__ uint32_t gdelta[256];              // global position - local position of the tile's elements of digit d
     __shared__ uint32_t wh[RADIX_WARPS][256];
+    __shared__ uint32_t wsum[RADIX_WARPS];
     gbase[threadIdx.x] = offs[(size_t)threadIdx.x * gridDim.x + blockIdx.x];
     unsigned long long lo, hi;
     radix_range(P, per_block, lo, hi);
@@ -122,10 +131,21 @@ k_radix_scatter(const T* __restrict__ raw, const typename RankKey<T>::K* __restr
             __syncwarp();
         }
         __syncthreads();
-        {   // thread d: positions of digit d for warp 0, 1, ... of this tile, then the block's running offset moves on
-            uint32_t run = gbase[threadIdx.x];
+        {   // thread d: the tile's count of digit d -> exclusive scan over the digits = local offset of digit d in the tile;
+            // wh[w][d] becomes the local position of warp w's first element of digit d
+            uint32_t tc = 0;
+            for (int w = 0; w < RADIX_WARPS; ++w) tc += wh[w][threadIdx.x];
+            uint32_t incl = tc;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { const uint32_t x = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += x; }
+            if (lane == 31) wsum[warp] = incl;
+            __syncthreads();
+            uint32_t pre = 0;
+            for (int w = 0; w < warp; ++w) pre += wsum[w];
+            uint32_t run = pre + incl - tc;                                   // local offset of digit d
+            gdelta[threadIdx.x] = gbase[threadIdx.x] - run;
+            gbase[threadIdx.x] += tc;
             for (int w = 0; w < RADIX_WARPS; ++w) { const uint32_t t = wh[w][threadIdx.x]; wh[w][threadIdx.x] = run; run += t; }
-            gbase[threadIdx.x] = run;
         }
         __syncthreads();
 #pragma unroll
@@ -134,13 +154,21 @@ k_radix_scatter(const T* __restrict__ raw, const typename RankKey<T>::K* __restr
             const uint32_t d = ok ? (uint32_t)((k[r] >> shift) & 255u) : 256u;
             const uint32_t peers = __match_any_sync(0xffffffffu, d);
             if (ok) {
-                const uint32_t pos = wh[warp][d] + (uint32_t)__popc(peers & lt);
-                keys_out[pos] = k[r];
-                idx_out[pos] = id[r];
+                const uint32_t lp = wh[warp][d] + (uint32_t)__popc(peers & lt);
+                skey[lp] = k[r];
+                sidx[lp] = id[r];
             }
             __syncwarp();
             if (ok && lane == __ffs(peers) - 1) wh[warp][d] += (uint32_t)__popc(peers);
             __syncwarp();
+        }
+        __syncthreads();
+        const uint32_t n_tile = (uint32_t)min((unsigned long long)RADIX_TILE, hi - tile);
+        for (uint32_t p = threadIdx.x; p < n_tile; p += RADIX_THREADS) {
+            const K kk = skey[p];
+            const uint32_t pos = p + gdelta[(uint32_t)((kk >> shift) & 255u)];
+            keys_out[pos] = kk;
+            idx_out[pos] = sidx[p];
         }
         __syncthreads();
     }

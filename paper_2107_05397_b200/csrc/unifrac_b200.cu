@@ -195,8 +195,14 @@ int radix_sort(const T* v, unsigned long long P, const RankBufs& B, cudaStream_t
         else k_radix_hist<T, false><<<B.nb, RADIX_THREADS, 0, st>>>(nullptr, keys[src], P, B.per_block, shift, B.hist);
         CU_LAUNCH();
         k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>((int)(256 * B.nb), B.hist, B.offs); CU_LAUNCH();
-        if (pass == 0) k_radix_scatter<T, true><<<B.nb, RADIX_THREADS, 0, st>>>(v, nullptr, nullptr, P, B.per_block, shift, B.offs, keys[dst], B.idx[dst]);
-        else k_radix_scatter<T, false><<<B.nb, RADIX_THREADS, 0, st>>>(nullptr, keys[src], B.idx[src], P, B.per_block, shift, B.offs, keys[dst], B.idx[dst]);
+        constexpr size_t ssm = radix_scatter_smem<K>();
+        if (pass == 0) {
+            CU(cudaFuncSetAttribute(k_radix_scatter<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ssm));
+            k_radix_scatter<T, true><<<B.nb, RADIX_THREADS, ssm, st>>>(v, nullptr, nullptr, P, B.per_block, shift, B.offs, keys[dst], B.idx[dst]);
+        } else {
+            CU(cudaFuncSetAttribute(k_radix_scatter<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ssm));
+            k_radix_scatter<T, false><<<B.nb, RADIX_THREADS, ssm, st>>>(nullptr, keys[src], B.idx[src], P, B.per_block, shift, B.offs, keys[dst], B.idx[dst]);
+        }
         CU_LAUNCH();
         src = dst;
     }
