@@ -89,14 +89,15 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
 CUtensorMap make_rowmajor_map(void* base, CUtensorMapDataType dt, size_t esz, uint64_t cols, uint64_t rows, uint32_t box_cols,
                               uint32_t box_rows, CUtensorMapSwizzle swz)
 {
-    static EncodeTiledFn fn = nullptr;
-    if (!fn) {
+    // resolved once (thread-safe static initialisation)
+    static EncodeTiledFn fn = []() -> EncodeTiledFn {
         void* p = nullptr;
         cudaDriverEntryPointQueryResult qr;
         cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr);
-        if (e != cudaSuccess || qr != cudaDriverEntryPointSuccess || !p) throw CudaFail{e != cudaSuccess ? e : cudaErrorUnknown, "cuTensorMapEncodeTiled entry point", __LINE__};
-        fn = reinterpret_cast<EncodeTiledFn>(p);
-    }
+        if (e != cudaSuccess || qr != cudaDriverEntryPointSuccess) { cudaGetLastError(); return nullptr; }
+        return reinterpret_cast<EncodeTiledFn>(p);
+    }();
+    if (!fn) throw CudaFail{cudaErrorUnknown, "cuTensorMapEncodeTiled entry point", __LINE__};
     CUtensorMap m;
     cuuint64_t dims[2] = {cols, rows};
     cuuint64_t strides[1] = {cols * esz};        // bytes, dimension 1
