@@ -120,3 +120,25 @@ def test_full_size_richness_zones_flag_emp_weighted():
     d = (out[big].double() - ref[big].double()).abs()
     assert bool(((d <= 2e-5 * ref[big].double()) | (d <= 2e-7)).all())
     print(f"zones vs oracle max rel err {(err / np.maximum(want, 1e-30)).max():.3e}; vs default path max abs diff {float(d.max()):.3e}")
+
+
+def test_full_size_other_seed_emp():
+    """DESIGN.md reading Q16: another seed at the EMP-shaped size (a different tree, table and split), both variants and the
+    RICHNESS_ZONES flag, 20,000 sampled pairs each against the oracle."""
+    import torch
+    from paper_2107_05397_b200 import binding as B
+    from oracle import oracle as O
+    p = synth.make_config("emp", seed=1)
+    n = p.n_samples
+    pairs = np.concatenate([synth.sample_pairs(n, 20000, seed=9), _structured_pairs(n)])
+    idx = torch.from_numpy(synth.condensed_index(n, pairs[:, 0], pairs[:, 1])).cuda()
+    args = B.to_device(p)
+    for variant, flags in ((0, 0), (1, 0), (1, B.FLAG_RICHNESS_ZONES)):
+        want = O.pair_list(p.parent, p.branch_len, p.indptr, p.indices, p.counts, variant, pairs)
+        out = B.unifrac_dm(*args, n, variant, B.FP32, flags=flags)
+        torch.cuda.synchronize()
+        got = out[idx].cpu().numpy().astype(np.float64)
+        del out
+        err = np.abs(got - want)
+        assert ((err <= 1e-5 * np.abs(want)) | (err <= 1e-7)).all(), (variant, flags, (err / np.maximum(want, 1e-30)).max())
+        assert B.unifrac_last_stats()["quant_fallback"] == 0
