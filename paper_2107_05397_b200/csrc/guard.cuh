@@ -33,6 +33,7 @@ struct GuardParams {
     long long N;
     int weighted;
     GuardList list;
+    unsigned int* done;                     // listed pairs already recomputed by an earlier launch of this call
     uint32_t* scratch;                      // [grid][3][n] zeroed: cntA, cntB, seen
     void* out;                              // condensed, T (in position space)
 };
@@ -47,7 +48,7 @@ k_guard(const GuardParams P)
     uint32_t* seen = cntB + P.n;
     const uint32_t total = min(*P.list.count, P.list.cap);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    for (uint32_t p = blockIdx.x; p < total; p += gridDim.x) {
+    for (uint32_t p = *P.done + blockIdx.x; p < total; p += gridDim.x) {
         const uint2 ab = P.list.pairs[p];
         const int sa = P.order ? P.order[ab.x] : (int)ab.x, sb = P.order ? P.order[ab.y] : (int)ab.y;
         // ---- 1. integer counts of both samples on every branch above their observed tips
@@ -107,5 +108,8 @@ k_guard(const GuardParams P)
         __syncthreads();
     }
 }
+
+// after a k_guard launch: everything listed so far has been recomputed
+__global__ void k_guard_mark(GuardList list, unsigned int* done) { *done = min(*list.count, list.cap); }
 
 }  // namespace ufb

@@ -43,6 +43,9 @@ struct CudaFail { cudaError_t e; const char* what; int line; };
 struct WorkspaceFail {};
 struct StatusFail { int status; };
 struct RetryExact {};        // the fixed-point error ratio is over budget: rerun without the fixed-point kernels
+// unifrac_dm_host_multi: called after each segment of the finalizing kernel with the number of condensed ROWS that are final
+// (rows [0, row_end) of out, guard included), so that their copy to the host can start while the rest is computed
+typedef void (*ProgressFn)(void* user, long long row_end, cudaStream_t st);
 // Fixed-point error ratio r (tail.cuh: k_quant_ratio): a distance d moves by at most ~2 r / d relative, so the guard
 // threshold is raised to theta = max(1/16, r / QUANT_REL) -- every pair below it is recomputed from the definition -- and
 // the call is rerun without the fixed-point kernels when theta would pass 1/2 (r > QUANT_RATIO_BUDGET).
@@ -225,7 +228,8 @@ void rank_transform(const T* v, unsigned long long P, uint32_t* rank2, const Ran
 
 template <typename T>
 void run(int32_t n, const int32_t* parent, const double* len, const int32_t* postorder, unifrac_csr_t tab,
-         int32_t N, int weighted, void* out, Arena& A, uint32_t flags, cudaStream_t st, int shard, int n_shards, bool is_retry)
+         int32_t N, int weighted, void* out, Arena& A, uint32_t flags, cudaStream_t st, int shard, int n_shards, bool is_retry,
+         ProgressFn progress = nullptr, void* progress_user = nullptr)
 {
     const bool validate = !(flags & UNIFRAC_FLAG_SKIP_VALIDATION);
     const bool timing = getenv("UNIFRAC_B200_TIMING") && atoi(getenv("UNIFRAC_B200_TIMING")) != 0;
@@ -741,10 +745,48 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         GL.pairs = A.get_n<uint2>(GL.cap);
         GL.count = reinterpret_cast<unsigned int*>(work + 18);         // zeroed with the other counters
     }
+    // ------------------------------------------------------------------ near-duplicate guard: listed pairs from the definition
+    // (launched after the finalizing kernel, or after each of its segments; `done` = listed pairs already recomputed)
+    GuardParams GP{};
+    unsigned ggrid = 0;
+    if (GL.pairs) {
+        ggrid = (unsigned)std::max(1, std::min(n_sm_dev, (int)std::min<unsigned long long>(GL.cap, 1u << 30)));
+        GP.n = n; GP.parent = parent; GP.len = len; GP.indptr = tab.indptr; GP.indices = tab.indices; GP.counts = tab.counts;
+        GP.Tsum = Tsum; GP.order = nullptr; GP.N = N; GP.weighted = weighted; GP.list = GL; GP.out = out;
+        GP.done = reinterpret_cast<unsigned int*>(work + 23);                // zeroed with the other counters
+        GP.scratch = A.get_n<uint32_t>((size_t)ggrid * 3 * n);
+        CU(cudaMemsetAsync(GP.scratch, 0, sizeof(uint32_t) * (size_t)ggrid * 3 * n, st));
+    }
+    auto run_guard = [&]() {
+        if (!GL.pairs) return;
+        k_guard<T><<<ggrid, GUARD_THREADS, 0, st>>>(GP); CU_LAUNCH(); ++launches;
+        k_guard_mark<<<1, 1, 0, st>>>(GL, GP.done); CU_LAUNCH(); ++launches;
+    };
+    // segments of the finalizing kernel's tile-pair list (blocked order: whole block rows of SHARD_BLOCK tiles): one segment
+    // unless the caller wants to be told about finished rows; {first pair, end pair, condensed rows final after it}
+    struct Seg { uint32_t p0, p1; long long row_end; };
+    auto make_segments = [&](const std::vector<int2>& pl, int BLK) {
+        std::vector<Seg> segs;
+        const uint32_t np = (uint32_t)pl.size();
+        const bool split = progress && n_shards == 1 && !inv_perm && np >= 64;
+        const int n_seg = split ? (int)env_double("UNIFRAC_B200_E2E_SEGMENTS", 4) : 1;
+        uint32_t begin = 0;
+        for (int k = 1; k <= n_seg && begin < np; ++k) {
+            uint32_t end = k == n_seg ? np : (uint32_t)((unsigned long long)np * k / n_seg);
+            while (end < np && end > begin && (uint32_t)pl[end].x / BLK == (uint32_t)pl[end - 1].x / BLK) ++end;   // to the block row's end
+            if (end <= begin) continue;
+            const long long row_end = end == np ? (long long)N : std::min<long long>(N, ((long long)pl[end - 1].x / BLK + 1) * BLK * TILE);
+            segs.push_back(Seg{begin, end, row_end});
+            begin = end;
+        }
+        if (segs.empty()) segs.push_back(Seg{0, np, (long long)N});
+        return segs;
+    };
     // ------------------------------------------------------------------ a-5 / a-6 stripe accumulation + finalize
     unsigned long long* kstats = work + 4;     // [0] rows executed, [1] rows staged (zeroed above)
     unsigned stripe_launches = 0;
     uint32_t n_pairs = 0;
+    bool guard_ran = false;
     int dev = 0, n_sm = 0;
     CU(cudaGetDevice(&dev));
     CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
@@ -762,19 +804,26 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             CUtensorMap tmB1 = make_u8_rowmajor_map(XG[2], Npad, K_pad, TILE, GRAM_BK);
             CUtensorMap tmB2 = make_u8_rowmajor_map(XG[3], Npad, K_pad, TILE, GRAM_BK);
             GramParams G{};
-            G.pairs = pairs; G.n_pairs = n_pairs; G.K_pad = K_pad; G.sums = sums; G.n_samples = N;
+            G.K_pad = K_pad; G.sums = sums; G.n_samples = N;
             G.out = reinterpret_cast<float*>(out); G.add_out = (tail_rows || mid_rows) ? 1 : 0; G.q = gram_q; G.guard = GL;
             CU(cudaFuncSetAttribute(k_gram, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GRAM_SMEM));
-            unsigned grid = (unsigned)std::min<long long>(n_sm, n_pairs);
             const int eshift = (int)envd("UNIFRAC_B200_GRAM_EPOCH_SHIFT", 5);
-            if (eshift >= 0 && grid) {
-                G.steps_per_cta = (uint32_t)((n_pairs + grid - 1) / grid) * (K_pad / GRAM_BK);
-                G.epoch_shift = (uint32_t)eshift;
-                const size_t n_ep = ((size_t)G.steps_per_cta >> eshift) + 2;
-                G.epoch_cnt = A.get_n<unsigned int>(n_ep);
-                CU(cudaMemsetAsync(G.epoch_cnt, 0, sizeof(unsigned int) * n_ep, st));
+            for (const Seg& sg : make_segments(h_pairs, 12)) {
+                G.pairs = pairs + sg.p0; G.n_pairs = sg.p1 - sg.p0;
+                unsigned grid = (unsigned)std::min<long long>(n_sm, G.n_pairs);
+                G.epoch_cnt = nullptr;
+                if (eshift >= 0 && grid) {
+                    G.steps_per_cta = (uint32_t)((G.n_pairs + grid - 1) / grid) * (K_pad / GRAM_BK);
+                    G.epoch_shift = (uint32_t)eshift;
+                    const size_t n_ep = ((size_t)G.steps_per_cta >> eshift) + 2;
+                    G.epoch_cnt = A.get_n<unsigned int>(n_ep);
+                    CU(cudaMemsetAsync(G.epoch_cnt, 0, sizeof(unsigned int) * n_ep, st));
+                }
+                if (grid) { k_gram<<<grid, GRAM_THREADS, GRAM_SMEM, st>>>(tmA, tmB0, tmB1, tmB2, G); CU_LAUNCH(); ++launches; ++stripe_launches; }
+                run_guard();
+                if (progress) progress(progress_user, sg.row_end, st);
             }
-            if (grid) { k_gram<<<grid, GRAM_THREADS, GRAM_SMEM, st>>>(tmA, tmB0, tmB1, tmB2, G); CU_LAUNCH(); ++launches; ++stripe_launches; }
+            guard_ran = true;
         }
     } else if (skip_on) {
         if constexpr (std::is_same<T, float>::value) {
@@ -817,19 +866,25 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         CUtensorMap tmE = make_rowmajor_map(Edense, f32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, sizeof(T), Npad, Kd_pad,
                                             TILE, DenseCfg<T>::BK, CU_TENSOR_MAP_SWIZZLE_NONE);
         DenseParams D{};
-        D.pairs = pairs; D.n_pairs = n_pairs; D.K_pad = Kd_pad; D.sums = sums; D.n_samples = N; D.weighted = weighted; D.out = out;
+        D.K_pad = Kd_pad; D.sums = sums; D.n_samples = N; D.weighted = weighted; D.out = out;
         D.add_out = (tail_rows || mid_rows) ? 1 : 0; D.guard = GL;
         const size_t smem = dense_smem_bytes<T>();
-        unsigned grid = (unsigned)std::min<long long>(n_sm, n_pairs);
-        D.scratch = A.get_n<double>((size_t)grid * 64 * 256);
+        D.scratch = A.get_n<double>((size_t)std::max(1, n_sm) * 64 * 256);
         D.hsum = hsum;
-        if (dense16) {
-            CU(cudaFuncSetAttribute(k_dense16, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            if (grid) { k_dense16<<<grid, DENSE16_THREADS, smem, st>>>(tmE, D); CU_LAUNCH(); ++launches; ++stripe_launches; }
-        } else {
-            CU(cudaFuncSetAttribute(k_dense<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            if (grid) { k_dense<T><<<grid, DENSE_THREADS, smem, st>>>(tmE, D); CU_LAUNCH(); ++launches; ++stripe_launches; }
+        if (dense16) CU(cudaFuncSetAttribute(k_dense16, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        else CU(cudaFuncSetAttribute(k_dense<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        for (const Seg& sg : make_segments(h_pairs, 12)) {
+            D.pairs = pairs + sg.p0; D.n_pairs = sg.p1 - sg.p0;
+            const unsigned grid = (unsigned)std::min<long long>(n_sm, D.n_pairs);
+            if (grid) {
+                if (dense16) k_dense16<<<grid, DENSE16_THREADS, smem, st>>>(tmE, D);
+                else k_dense<T><<<grid, DENSE_THREADS, smem, st>>>(tmE, D);
+                CU_LAUNCH(); ++launches; ++stripe_launches;
+            }
+            run_guard();
+            if (progress) progress(progress_user, sg.row_end, st);
         }
+        guard_ran = true;
     } else {
     std::vector<int2> h_pairs;
     h_pairs.reserve((size_t)n_tiles * (n_tiles + 1) / 2);
@@ -863,16 +918,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         kern<<<grid, STRIPE_THREADS, smem, st>>>(P); CU_LAUNCH(); ++launches; ++stripe_launches;
     }
     }
-    // ------------------------------------------------------------------ near-duplicate guard: listed pairs from the definition
-    if (GL.pairs) {
-        const unsigned ggrid = (unsigned)std::max(1, std::min(n_sm, (int)std::min<unsigned long long>(GL.cap, 1u << 30)));
-        GuardParams GP{};
-        GP.n = n; GP.parent = parent; GP.len = len; GP.indptr = tab.indptr; GP.indices = tab.indices; GP.counts = tab.counts;
-        GP.Tsum = Tsum; GP.order = nullptr; GP.N = N; GP.weighted = weighted; GP.list = GL; GP.out = out;
-        GP.scratch = A.get_n<uint32_t>((size_t)ggrid * 3 * n);
-        CU(cudaMemsetAsync(GP.scratch, 0, sizeof(uint32_t) * (size_t)ggrid * 3 * n, st));
-        k_guard<T><<<ggrid, GUARD_THREADS, 0, st>>>(GP); CU_LAUNCH(); ++launches;
-    }
+    if (!guard_ran) run_guard();
     if (inv_perm) {
         k_unpermute<T><<<dim3((unsigned)cdiv(N, 256), (unsigned)std::min(N, 65535)), 256, 0, st>>>((long long)N, inv_perm, reinterpret_cast<const T*>(out),
                                                                                                   reinterpret_cast<T*>(out_user));
@@ -917,7 +963,8 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
 
 int guarded(int32_t n_nodes, const int32_t* parent, const double* len, const int32_t* postorder, unifrac_csr_t tab,
             int32_t N, unifrac_variant_t variant, unifrac_precision_t precision, void* out, unifrac_alloc_fn alloc,
-            void* user, uint32_t flags, cudaStream_t st, int shard = 0, int n_shards = 1, cudaMemPool_t pool = nullptr)
+            void* user, uint32_t flags, cudaStream_t st, int shard = 0, int n_shards = 1, cudaMemPool_t pool = nullptr,
+            ProgressFn progress = nullptr, void* progress_user = nullptr)
 {
     if (n_shards < 1 || n_shards > 255 || shard < 0 || shard >= n_shards) return UNIFRAC_ERR_INVALID_ARG;
     if (n_shards > 1 && (flags & (UNIFRAC_FLAG_LITERAL | UNIFRAC_FLAG_ABSDIFF | UNIFRAC_FLAG_SPARSE_STRIPE | UNIFRAC_FLAG_NO_TAIL)))
@@ -937,12 +984,13 @@ int guarded(int32_t n_nodes, const int32_t* parent, const double* len, const int
     const bool w = variant == UNIFRAC_WEIGHTED_NORMALIZED;
     try {
         try {
-            if (precision == UNIFRAC_FP32) run<float>(n_nodes, parent, len, postorder, tab, N, w, out, A, flags, st, shard, n_shards, false);
-            else run<double>(n_nodes, parent, len, postorder, tab, N, w, out, A, flags, st, shard, n_shards, false);
+            if (precision == UNIFRAC_FP32) run<float>(n_nodes, parent, len, postorder, tab, N, w, out, A, flags, st, shard, n_shards, false, progress, progress_user);
+            else run<double>(n_nodes, parent, len, postorder, tab, N, w, out, A, flags, st, shard, n_shards, false, progress, progress_user);
         } catch (const RetryExact&) {
             // only the fp32 path has fixed-point kernels; head rows on the CUDA-core kernel, the rest on the fp32 scatter
             A.release();
-            run<float>(n_nodes, parent, len, postorder, tab, N, w, out, A, flags | UNIFRAC_FLAG_NO_TENSOR | UNIFRAC_FLAG_NO_MID, st, shard, n_shards, true);
+            run<float>(n_nodes, parent, len, postorder, tab, N, w, out, A, flags | UNIFRAC_FLAG_NO_TENSOR | UNIFRAC_FLAG_NO_MID, st, shard, n_shards, true,
+                       progress, progress_user);
         }
     } catch (const CudaFail& f) {
         char buf[512];
@@ -1113,6 +1161,18 @@ int32_t unifrac_shard_of_pair(int32_t i, int32_t j, int32_t shard_count)
     return shard_of_tiles(a / TILE, b / TILE, shard_count);
 }
 
+// Device -> host copy in pieces of 32 MB: the planning steps of the NEXT variant read a few words back at every synchronisation
+// point, and those small copies share the copy engine with this one -- behind a single 5 GB transfer they would wait ~190 ms.
+static cudaError_t copy_d2h_pieces(unsigned char* dst, const unsigned char* src, size_t bytes, cudaStream_t s)
+{
+    const size_t PIECE = (size_t)env_double("UNIFRAC_B200_E2E_PIECE_MB", 32) << 20;
+    for (size_t off = 0; off < bytes; off += PIECE) {
+        cudaError_t e = cudaMemcpyAsync(dst + off, src + off, std::min(PIECE, bytes - off), cudaMemcpyDeviceToHost, s);
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
+
 // the library's own stream-ordered pool for the host entry points (one per device, created on first use; it keeps what it
 // has mapped between calls -- release threshold = max -- and unifrac_release_host_pool gives it back)
 static cudaMemPool_t g_host_pool[64] = {};
@@ -1176,18 +1236,44 @@ int unifrac_dm_host_multi(int32_t n_nodes, const int32_t* tree_parent, const dou
         ok(cudaMemcpyAsync(d_idx, th.indices, sizeof(int32_t) * (size_t)nnz, cudaMemcpyHostToDevice, st));
         ok(cudaMemcpyAsync(d_cnt, th.counts, sizeof(int32_t) * (size_t)nnz, cudaMemcpyHostToDevice, st));
     }
+    // The LAST variant's result has nothing to hide behind, so its finalizing kernel runs in segments of whole block rows and
+    // every finished range of condensed rows starts travelling while the next segment is computed (ProgressFn).
+    struct Chunked {
+        cudaStream_t cs; unsigned char* host; const unsigned char* dev; size_t esz; long long N; long long rows_done; cudaError_t err;
+        std::vector<cudaEvent_t> events;
+    } ch{cs, nullptr, nullptr, esz, (long long)N, 0, cudaSuccess, {}};
+    auto on_rows = [](void* user, long long row_end, cudaStream_t s) {
+        Chunked* c = static_cast<Chunked*>(user);
+        if (row_end <= c->rows_done || c->err != cudaSuccess) return;
+        auto first = [&](long long r) { return (size_t)(r * (2 * c->N - r - 1) / 2); };      // condensed index of (r, r + 1)
+        const long long r1 = row_end >= c->N - 1 ? c->N - 1 : row_end;                         // row N - 1 has no element
+        const size_t e0 = first(c->rows_done), e1 = first(r1);
+        cudaEvent_t ev = nullptr;
+        if ((c->err = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming)) != cudaSuccess) return;
+        c->events.push_back(ev);
+        if ((c->err = cudaEventRecord(ev, s)) != cudaSuccess) return;
+        if ((c->err = cudaStreamWaitEvent(c->cs, ev, 0)) != cudaSuccess) return;
+        if (e1 > e0) c->err = copy_d2h_pieces(c->host + e0 * c->esz, c->dev + e0 * c->esz, (e1 - e0) * c->esz, c->cs);
+        c->rows_done = r1;
+    };
     for (int k = 0; k < n_variants && rc == UNIFRAC_OK; ++k) {
         unifrac_csr_t td{reinterpret_cast<const int64_t*>(d_indptr), reinterpret_cast<const int32_t*>(d_idx), reinterpret_cast<const int32_t*>(d_cnt)};
+        const bool last = k == n_variants - 1;
+        ch.host = static_cast<unsigned char*>(outs_host[k]); ch.dev = static_cast<const unsigned char*>(d_out[k]); ch.rows_done = 0;
         rc = guarded(n_nodes, reinterpret_cast<const int32_t*>(d_parent), reinterpret_cast<const double*>(d_len),
                      reinterpret_cast<const int32_t*>(d_post), td, N, (unifrac_variant_t)variants[k], precision, d_out[k], nullptr, nullptr,
-                     flags, st, 0, 1, pool);
+                     flags, st, 0, 1, pool, last ? +on_rows : nullptr, last ? &ch : nullptr);
         if (rc != UNIFRAC_OK) break;
-        // unifrac_dm returns once the a-5 kernels are enqueued: the copy waits for them on its own stream
+        if (last) ok(ch.err);
+        // unifrac_dm returns once the a-5 kernels are enqueued: the copy of whatever has not been sent yet waits for them on its own stream
         ok(cudaEventCreateWithFlags(&done[k], cudaEventDisableTiming));
         if (rc == UNIFRAC_OK) {
+            const long long r0 = last ? ch.rows_done : 0;
+            const size_t e0 = (size_t)(r0 * (2 * (long long)N - r0 - 1) / 2);
             ok(cudaEventRecord(done[k], st));
             ok(cudaStreamWaitEvent(cs, done[k], 0));
-            ok(cudaMemcpyAsync(outs_host[k], d_out[k], esz * n_out, cudaMemcpyDeviceToHost, cs));
+            if (n_out > e0) ok(copy_d2h_pieces(static_cast<unsigned char*>(outs_host[k]) + e0 * esz, static_cast<const unsigned char*>(d_out[k]) + e0 * esz,
+                                               (n_out - e0) * esz, cs));
         }
     }
     if (cs) ok(cudaStreamSynchronize(cs));
@@ -1195,6 +1281,7 @@ int unifrac_dm_host_multi(int32_t n_nodes, const int32_t* tree_parent, const dou
     if (st) { ok(cudaStreamSynchronize(st)); cudaStreamDestroy(st); }
     if (cs) cudaStreamDestroy(cs);
     for (auto& e : done) if (e) cudaEventDestroy(e);
+    for (auto& e : ch.events) cudaEventDestroy(e);
     return rc;
 }
 

@@ -116,3 +116,20 @@ def test_guard_in_shard_mode(B, O):
     got = total[torch.from_numpy(idx).cuda()].cpu().numpy().astype(np.float64)
     assert np.all(got[kinds < 2] == 0.0)
     assert (np.abs(got[kinds == 2] - want[kinds == 2]) / want[kinds == 2]).max() <= 1e-5
+
+
+def test_guard_with_segmented_finalize_in_host_multi(B, O):
+    """unifrac_dm_host_multi finalizes the last variant in segments of block rows (guard + result copy after each one): planted
+    duplicates stay exactly 0 and the host result equals the device entry point's bit for bit.  1,700 samples = 105 tile pairs,
+    enough for the segmentation to kick in."""
+    cfg = synth.CONFIGS["small"]
+    base = synth.make_problem(2000, 1700, 0.1, 1.1, cfg[4], cfg[5], seed=17)
+    p, pairs, kinds = synth.plant_near_duplicates(base, 8, seed=3)
+    n = p.n_samples
+    idx = synth.condensed_index(n, pairs[:, 0], pairs[:, 1])
+    for order in ([U, W], [W, U]):                       # either variant last
+        outs = B.unifrac_dm_host_multi(p.parent, p.branch_len, p.postorder, p.indptr, p.indices, p.counts, n, order, B.FP32)
+        for v, got in zip(order, outs):
+            assert np.all(got[idx[kinds < 2]] == 0.0)
+            assert np.array_equal(got.astype(np.float64), gpu_dm(B, p, v, 0))
+    B.unifrac_release_host_pool()
