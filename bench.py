@@ -353,7 +353,7 @@ def main():
             # the rank transform: 2 vectors x 4 radix passes x (4 + 8 + 8) bytes per element, then the fp64 rank vectors
             mantel["spearman"] = dict(ms=s_ms, rho=float(so[0]), p_two_sided=float(so[1]),
                                       ms_rank_transform_and_fp64_statistics=s_ms,
-                                      note="device radix-sort rank transform of both matrices + the same permutation kernel on fp64 ranks")
+                                      note="device radix-sort rank transform of both matrices + the same permutation kernel on the 32-bit 2 x rank vectors (fp64 sums)")
         except binding.UnifracError as e:                              # e.g. workspace
             mantel["spearman"] = dict(error=str(e))
         del perms, mo

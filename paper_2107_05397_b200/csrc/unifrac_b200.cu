@@ -1010,39 +1010,46 @@ void run_mantel(int32_t N, const T* x, const T* y, const int32_t* perms, int32_t
 {
     const unsigned long long P = (unsigned long long)N * (N - 1) / 2;
     double* mom = A.get_n<double>(8);
-    double* S = A.get_n<double>((size_t)K + 1);
     const long long pitch = ((long long)N + 3) & ~3ll;                      // rows start 16-byte aligned (bulk copies)
     T* Xs = A.get_n<T>((size_t)N * pitch);
     CU(cudaMemsetAsync(mom, 0, sizeof(double) * 8, st));
-    CU(cudaMemsetAsync(S, 0, sizeof(double) * ((size_t)K + 1), st));
-    CU(cudaMemsetAsync(Xs, 0, sizeof(T) * (size_t)N * pitch, st));         // pitch padding
+    if (pitch > N)                                                          // the padding columns are copied with the rows: keep them finite
+        CU(cudaMemset2DAsync(Xs + N, (size_t)pitch * sizeof(T), 0, (size_t)(pitch - N) * sizeof(T), (size_t)N, st));
     int dev = 0, n_sm = 0;
     CU(cudaGetDevice(&dev));
     CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
     k_mantel_moments<T><<<n_sm * 8, 256, 0, st>>>(x, y, P, mom); CU_LAUNCH();
     const unsigned nb = (unsigned)cdiv(N, 32);
     k_mantel_square<T><<<dim3(nb, nb), dim3(32, 8), 0, st>>>(x, N, pitch, Xs); CU_LAUNCH();
-    // two ring buffers of one column segment each: as few segments as fit in ~208 KB
-    const size_t budget = (size_t)208 * 1024 / 2 / sizeof(T);              // elements per buffer
-    const int n_split = cdiv(pitch, (long long)budget);
+    // staging of the gathered rows: two ring buffers of a whole row when two fit in ~208 KB (the next row is copied while this
+    // one is used); ONE whole-row buffer when only one fits (the SMs drift apart, so one SM's copy overlaps the others'
+    // multiply-adds -- measured 2x faster than two passes over half rows); column segments in two buffers beyond that
+    const size_t cap = (size_t)208 * 1024 / sizeof(T);                     // elements of staging space
+    int n_buf = 2, n_split = 1;
+    if (const char* e = getenv("UNIFRAC_B200_MANTEL_BUFS")) n_buf = atoi(e) == 1 ? 1 : 2;
+    else if ((size_t)pitch * 2 > cap && (size_t)pitch <= cap) n_buf = 1;
+    if ((size_t)pitch * n_buf > cap) n_split = cdiv(pitch, (long long)(cap / n_buf));
     const int seg = (int)(((pitch + n_split - 1) / n_split + 3) & ~3ll);
-    const size_t smem = 2 * (size_t)seg * sizeof(T);
-    CU(cudaFuncSetAttribute(k_mantel_perm<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    for (int k0 = 0; k0 <= K; k0 += 65535) {                              // grid.y limit
-        const int kn = std::min(65535, K + 1 - k0);
+    const size_t smem = (size_t)n_buf * seg * sizeof(T) + 16;              // + the zero element of the split kernel
+    auto kern = n_split > 1 ? k_mantel_perm<T, true> : k_mantel_perm<T, false>;
+    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int32_t* ident = A.get_n<int32_t>(N);
+    k_mantel_iota<<<cdiv(N, 256), 256, 0, st>>>(ident, N); CU_LAUNCH();
+    {
+        const int kn = K + 1;
         // row-strided CTAs per permutation: G * kn CTAs (one per SM at a time) should fill whole waves of n_sm
         int G = 1; double best = 0.0;
         for (int m = 1; m <= 8; ++m) {
-            const int g = std::min<long long>(N - 1, (long long)n_sm * m / kn);
-            if (g < 1) continue;
+            const int g = (int)std::min<long long>(std::min<long long>(N - 1, 65535), std::max<long long>(1, (long long)n_sm * m / kn));
             const double fill = (double)g * kn / ((double)n_sm * cdiv((long long)g * kn, n_sm));
             if (fill > best + 1e-9) { best = fill; G = g; }
         }
-        k_mantel_perm<T><<<dim3((unsigned)G, (unsigned)kn), MANTEL_THREADS, smem, st>>>(
-            Xs, pitch, y, perms, N, seg, n_split, k0, S);
+        double* S = A.get_n<double>((size_t)kn * G);                      // every CTA writes its own partial sum
+        kern<<<dim3((unsigned)kn, (unsigned)G), MANTEL_THREADS, smem, st>>>(
+            Xs, pitch, y, perms, ident, N, seg, n_split, n_buf, 0, S);
         CU_LAUNCH();
+        k_mantel_final<T><<<1, 256, 0, st>>>(mom, S, G, K, (double)P, x, y, out); CU_LAUNCH();
     }
-    k_mantel_final<T><<<1, 256, 0, st>>>(mom, S, K, (double)P, x, y, out); CU_LAUNCH();
     A.release();
 }
 

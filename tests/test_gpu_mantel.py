@@ -91,17 +91,23 @@ def test_mantel_on_unifrac_matrices_and_sampled_property_at_scale():
     assert abs(both[4] - base[0]) <= 1e-10
 
 
-def test_mantel_row_longer_than_one_shared_memory_segment():
-    """fp64, N = 14,000: a row of the square copy is 112 KB, more than one ring buffer holds, so every row is staged in two
-    column segments (the path N = 50,000 takes in fp32).  One permutation against the oracle, identity against r."""
+@pytest.mark.parametrize("bufs", ["", "2"])
+def test_mantel_row_longer_than_one_ring_buffer(bufs, monkeypatch):
+    """fp64, N = 14,000: a row of the square copy is 112 KB, so two whole rows do not fit in shared memory.  Default: ONE
+    whole-row buffer (the path N = 50,000 takes in fp32); UNIFRAC_B200_MANTEL_BUFS=2: two buffers of half a row, every row
+    staged in two column segments (the path of rows beyond 208 KB).  One permutation against the oracle, identity against r."""
     from paper_2107_05397_b200 import binding as B
     from oracle import mantel_oracle as M
+    if bufs:
+        monkeypatch.setenv("UNIFRAC_B200_MANTEL_BUFS", bufs)
+    else:
+        monkeypatch.delenv("UNIFRAC_B200_MANTEL_BUFS", raising=False)
     n = 14000
     x, y, perms = _case(n, 1, seed=4, dtype=np.float64)
     perms = np.concatenate([perms, np.arange(n, dtype=np.int32)[None, :]])
     got = _run(B, x, y, n, perms)
     r, _, _, _, rk = M.mantel_pearson(x, y, n, perms[:1])
-    assert abs(got[0] - r) <= 1e-10 and abs(got[4] - rk[0]) <= 1e-10 and abs(got[5] - got[0]) <= 1e-12
+    assert abs(got[0] - r) <= 1e-10 and abs(got[4] - rk[0]) <= 1e-10 and got[5] == got[0]
 
 
 # ------------------------------------------------------------------------------------------------ Spearman (PAPER.md:41-43)
