@@ -62,23 +62,36 @@ k_radix_hist(const T* __restrict__ raw, const typename RankKey<T>::K* __restrict
              unsigned long long per_block, int shift, uint32_t* __restrict__ hist)
 {
     using K = typename RankKey<T>::K;
-    __shared__ uint32_t h[256];
-    h[threadIdx.x] = 0;
+    __shared__ uint32_t wh[RADIX_WARPS][256];                          // per-warp counts
+    for (int w = 0; w < RADIX_WARPS; ++w) wh[w][threadIdx.x] = 0;
     __syncthreads();
     unsigned long long lo, hi;
     radix_range(P, per_block, lo, hi);
-    const int lane = threadIdx.x & 31;
-    for (unsigned long long base = lo; base < hi; base += RADIX_THREADS) {
-        const unsigned long long e = base + threadIdx.x;
-        const bool ok = e < hi;
-        K k = 0;
-        if (ok) k = FIRST ? RankKey<T>::make(raw[e]) : keys[e];
-        const uint32_t d = ok ? (uint32_t)((k >> shift) & 255u) : 256u;            // 256 = the inactive lanes' own group
-        const uint32_t peers = __match_any_sync(0xffffffffu, d);
-        if (ok && lane == __ffs(peers) - 1) atomicAdd(&h[d], (uint32_t)__popc(peers));
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (unsigned long long tile = lo; tile < hi; tile += RADIX_TILE) {
+        // the same element -> (warp, round, lane) map as the scatter kernel; RADIX_ITEMS independent loads in flight per thread
+        const unsigned long long wbase = tile + (unsigned long long)warp * (32 * RADIX_ITEMS) + lane;
+        K k[RADIX_ITEMS];
+        if (FIRST) {                                                   // all loads first, then the key map (a load inside the
+            T v[RADIX_ITEMS];                                          // conditional conversion is not hoisted by the compiler)
+#pragma unroll
+            for (int r = 0; r < RADIX_ITEMS; ++r) { const unsigned long long e = wbase + (unsigned long long)r * 32; v[r] = e < hi ? raw[e] : T(0); }
+#pragma unroll
+            for (int r = 0; r < RADIX_ITEMS; ++r) k[r] = RankKey<T>::make(v[r]);
+        } else {
+#pragma unroll
+            for (int r = 0; r < RADIX_ITEMS; ++r) { const unsigned long long e = wbase + (unsigned long long)r * 32; k[r] = e < hi ? keys[e] : K(0); }
+        }
+        // counting needs no order: shared-memory atomics on the warp's own histogram (one __match_any_sync per element, which
+        // the scatter kernel needs for its stable ranks, made this kernel 6x slower: 5.0 -> 0.82 ms per pass at N = 50,000)
+#pragma unroll
+        for (int r = 0; r < RADIX_ITEMS; ++r)
+            if (wbase + (unsigned long long)r * 32 < hi) atomicAdd(&wh[warp][(uint32_t)((k[r] >> shift) & 255u)], 1u);
     }
     __syncthreads();
-    hist[(size_t)threadIdx.x * gridDim.x + blockIdx.x] = h[threadIdx.x];
+    uint32_t t = 0;
+    for (int w = 0; w < RADIX_WARPS; ++w) t += wh[w][threadIdx.x];
+    hist[(size_t)threadIdx.x * gridDim.x + blockIdx.x] = t;
 }
 
 // stable scatter of one digit: offs = exclusive scan of hist (digit-major), i.e. the global position of the first element
@@ -113,23 +126,24 @@ k_radix_scatter(const T* __restrict__ raw, const typename RankKey<T>::K* __restr
         K k[RADIX_ITEMS];
         uint32_t id[RADIX_ITEMS];
         const unsigned long long wbase = tile + (unsigned long long)warp * (32 * RADIX_ITEMS) + lane;
+        if (FIRST) {                                                   // all loads first, then the key map
+            T v[RADIX_ITEMS];
 #pragma unroll
-        for (int r = 0; r < RADIX_ITEMS; ++r) {
-            const unsigned long long e = wbase + (unsigned long long)r * 32;
-            if (e < hi) {
-                if (FIRST) { k[r] = RankKey<T>::make(raw[e]); id[r] = (uint32_t)e; }
-                else { k[r] = keys_in[e]; id[r] = idx_in[e]; }
-            } else { k[r] = 0; id[r] = 0; }
-        }
-        // per-warp digit counts
+            for (int r = 0; r < RADIX_ITEMS; ++r) { const unsigned long long e = wbase + (unsigned long long)r * 32; v[r] = e < hi ? raw[e] : T(0); }
 #pragma unroll
-        for (int r = 0; r < RADIX_ITEMS; ++r) {
-            const bool ok = wbase + (unsigned long long)r * 32 < hi;
-            const uint32_t d = ok ? (uint32_t)((k[r] >> shift) & 255u) : 256u;
-            const uint32_t peers = __match_any_sync(0xffffffffu, d);
-            if (ok && lane == __ffs(peers) - 1) wh[warp][d] += (uint32_t)__popc(peers);
-            __syncwarp();
+            for (int r = 0; r < RADIX_ITEMS; ++r) { k[r] = RankKey<T>::make(v[r]); id[r] = (uint32_t)(wbase + (unsigned long long)r * 32); }
+        } else {
+#pragma unroll
+            for (int r = 0; r < RADIX_ITEMS; ++r) {
+                const unsigned long long e = wbase + (unsigned long long)r * 32;
+                k[r] = e < hi ? keys_in[e] : K(0);
+                id[r] = e < hi ? idx_in[e] : 0u;
+            }
         }
+        // per-warp digit counts (order does not matter here: shared-memory atomics on the warp's own histogram)
+#pragma unroll
+        for (int r = 0; r < RADIX_ITEMS; ++r)
+            if (wbase + (unsigned long long)r * 32 < hi) atomicAdd(&wh[warp][(uint32_t)((k[r] >> shift) & 255u)], 1u);
         __syncthreads();
         {   // thread d: the tile's count of digit d -> exclusive scan over the digits = local offset of digit d in the tile;
             // wh[w][d] becomes the local position of warp w's first element of digit d
@@ -148,11 +162,19 @@ k_radix_scatter(const T* __restrict__ raw, const typename RankKey<T>::K* __restr
             for (int w = 0; w < RADIX_WARPS; ++w) { const uint32_t t = wh[w][threadIdx.x]; wh[w][threadIdx.x] = run; run += t; }
         }
         __syncthreads();
+        // the lanes with the same digit in each round: all RADIX_ITEMS matches are issued back to back (MATCH has a long
+        // latency; one match followed by its dependent shared-memory update per round left the warp waiting 16 times)
+        uint32_t pm[RADIX_ITEMS];
+#pragma unroll
+        for (int r = 0; r < RADIX_ITEMS; ++r) {
+            const bool ok = wbase + (unsigned long long)r * 32 < hi;
+            pm[r] = __match_any_sync(0xffffffffu, ok ? (uint32_t)((k[r] >> shift) & 255u) : 256u);
+        }
 #pragma unroll
         for (int r = 0; r < RADIX_ITEMS; ++r) {
             const bool ok = wbase + (unsigned long long)r * 32 < hi;
             const uint32_t d = ok ? (uint32_t)((k[r] >> shift) & 255u) : 256u;
-            const uint32_t peers = __match_any_sync(0xffffffffu, d);
+            const uint32_t peers = pm[r];
             if (ok) {
                 const uint32_t lp = wh[warp][d] + (uint32_t)__popc(peers & lt);
                 skey[lp] = k[r];
@@ -234,17 +256,40 @@ k_rank_starts(const K* __restrict__ keys, unsigned long long P, unsigned long lo
     }
 }
 
-// rank2[idx[p]] = 2 * (average rank) = 2 start[p] + (rlen[start[p]] - 1) + 2     (1-based average ranks are half-integers:
-// twice the rank is an exact 32-bit integer for n(n-1)/2 < 2^31 - 1, half the bytes of an fp64 rank, and Pearson's r does
-// not see the factor 2)
+// val[p] = 2 * (average rank) of sorted position p = 2 start[p] + (rlen[start[p]] - 1) + 2     (1-based average ranks are
+// half-integers: twice the rank is an exact 32-bit integer for n(n-1)/2 < 2^31 - 1, half the bytes of an fp64 rank, and
+// Pearson's r does not see the factor 2)
 __global__ void __launch_bounds__(256)
-k_rank_write(const uint32_t* __restrict__ idx, const uint32_t* __restrict__ start, const uint32_t* __restrict__ rlen,
-             unsigned long long P, uint32_t* __restrict__ rank2)
+k_rank_value(const uint32_t* __restrict__ start, const uint32_t* __restrict__ rlen, unsigned long long P, uint32_t* __restrict__ val)
 {
     for (unsigned long long p = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; p < P; p += (unsigned long long)gridDim.x * blockDim.x) {
         const uint32_t s = start[p];
-        rank2[idx[p]] = 2u * s + (rlen[s] - 1u) + 2u;
+        val[p] = 2u * s + (rlen[s] - 1u) + 2u;
     }
+}
+
+// rank2[pos[p]] = val[p].  The caller has partitioned the (pos, val) pairs by the top bits of pos (one more radix scatter, on
+// the positions), so the blocks that run together write into one window of rank2 that stays in L2 until its sectors are
+// complete; scattering straight from the sorted order costs a 32-byte read-modify-write per 4-byte rank (56.7 ms per vector
+// at N = 50,000 against 0.5 + 4.5 + 9.5 ms for histogram + partition + this kernel).
+// NOT a grid-stride loop: block b owns the RANK_PLACE_PER_BLOCK pairs behind b * RANK_PLACE_PER_BLOCK and blocks are scheduled
+// in order, so the blocks in flight stay within one or two windows (persistent blocks drift apart by several windows over
+// 10^9 elements and the windows' sectors leave L2 half-written: 45 ms).
+constexpr int RANK_PLACE_PER_BLOCK = 2048;
+__global__ void __launch_bounds__(256)
+k_rank_place(const uint32_t* __restrict__ pos, const uint32_t* __restrict__ val, unsigned long long P, uint32_t* __restrict__ rank2)
+{
+    const unsigned long long base = (unsigned long long)blockIdx.x * RANK_PLACE_PER_BLOCK + threadIdx.x;
+    uint32_t q[RANK_PLACE_PER_BLOCK / 256], v[RANK_PLACE_PER_BLOCK / 256];
+#pragma unroll
+    for (int u = 0; u < RANK_PLACE_PER_BLOCK / 256; ++u) {
+        const unsigned long long p = base + (unsigned long long)u * 256;
+        q[u] = 0xffffffffu;
+        if (p < P) { q[u] = pos[p]; v[u] = val[p]; }
+    }
+#pragma unroll
+    for (int u = 0; u < RANK_PLACE_PER_BLOCK / 256; ++u)
+        if (q[u] != 0xffffffffu) rank2[q[u]] = v[u];
 }
 
 }  // namespace ufb

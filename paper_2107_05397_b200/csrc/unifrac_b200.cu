@@ -213,6 +213,7 @@ int radix_sort(const T* v, unsigned long long P, const RankBufs& B, cudaStream_t
     return src;
 }
 // twice the 1-based average ranks of the P values v[] (exact 32-bit integers) -> rank2[]
+constexpr int RANK_WINDOW_BITS = 23;                                 // P < 2^31: at most 256 windows
 template <typename T>
 void rank_transform(const T* v, unsigned long long P, uint32_t* rank2, const RankBufs& B, cudaStream_t st)
 {
@@ -223,7 +224,24 @@ void rank_transform(const T* v, unsigned long long P, uint32_t* rank2, const Ran
     uint32_t* rlen = B.idx[src ^ 1];
     k_rank_block_heads<K><<<B.nb, RADIX_THREADS, 0, st>>>(keys[src], P, B.per_block, B.blast); CU_LAUNCH();
     k_rank_starts<K><<<B.nb, RADIX_THREADS, 0, st>>>(keys[src], P, B.per_block, B.blast, start, rlen); CU_LAUNCH();
-    k_rank_write<<<B.nb * 4, 256, 0, st>>>(B.idx[src], start, rlen, P, rank2); CU_LAUNCH();
+    // back to the original positions: rank values in sorted order, then the (position, value) pairs partitioned by the top
+    // 8 bits of the position (windows of 2^RANK_WINDOW_BITS ranks = 32 MB, L2-resident), then the scatter inside the windows
+    uint32_t* val = reinterpret_cast<uint32_t*>(keys[src]);           // the sorted keys are no longer needed
+    k_rank_value<<<B.nb * 4, 256, 0, st>>>(start, rlen, P, val); CU_LAUNCH();
+    if ((P >> RANK_WINDOW_BITS) == 0) {                               // one window: scatter directly
+        k_rank_place<<<(unsigned)cdiv((long long)P, RANK_PLACE_PER_BLOCK), 256, 0, st>>>(B.idx[src], val, P, rank2); CU_LAUNCH();
+        return;
+    }
+    uint32_t* pos_out = start;                                        // start / rlen are free once val is written
+    uint32_t* val_out = rlen;
+    k_radix_hist<uint32_t, false><<<B.nb, RADIX_THREADS, 0, st>>>(nullptr, B.idx[src], P, B.per_block, RANK_WINDOW_BITS, B.hist); CU_LAUNCH();
+    k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>((int)(256 * B.nb), B.hist, B.offs); CU_LAUNCH();
+    constexpr size_t ssm = radix_scatter_smem<uint32_t>();
+    CU(cudaFuncSetAttribute(k_radix_scatter<uint32_t, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ssm));
+    k_radix_scatter<uint32_t, false><<<B.nb, RADIX_THREADS, ssm, st>>>(nullptr, B.idx[src], val, P, B.per_block, RANK_WINDOW_BITS, B.offs,
+                                                                       pos_out, val_out);
+    CU_LAUNCH();
+    k_rank_place<<<(unsigned)cdiv((long long)P, RANK_PLACE_PER_BLOCK), 256, 0, st>>>(pos_out, val_out, P, rank2); CU_LAUNCH();
 }
 
 template <typename T>
