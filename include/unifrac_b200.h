@@ -226,6 +226,27 @@ int unifrac_mantel_pearson(int32_t n_samples, const void *x_condensed, const voi
                            unifrac_alloc_fn alloc, void *alloc_user, void *stream);
 
 /*
+ * unifrac_mantel_pearson_noalloc -- unifrac_mantel_pearson for callers that cannot allocate (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc): the same kernels and the same result, with the workspace (square
+ * copy of X, per-CTA partial sums, moments) in a static device array of UNIFRAC_NOALLOC_SCRATCH_BYTES inside the library
+ * instead of an allocator.  Every GPU that loads the library holds that array until the process exits.  The call makes no
+ * cudaMalloc / cudaFree / cudaMallocAsync and calls no allocating library routine; the caller passes inputs and `out`
+ * (4 + n_perms doubles), all DEVICE pointers, as for unifrac_mantel_pearson.
+ * Limits: n_samples <= UNIFRAC_NOALLOC_MAX_SAMPLES and n_perms <= UNIFRAC_NOALLOC_MAX_PERMS, else UNIFRAC_ERR_UNSUPPORTED
+ * (unifrac_last_cuda_error() then names the limit that was exceeded); other argument errors as unifrac_mantel_pearson.
+ * The array is SHARED by every call on the device and keeps the last call's contents (the call clears what must start at
+ * zero): two calls that overlap on the GPU -- different streams, or different host threads -- race on it; serialise them.
+ * Asynchronous on `stream`, which must belong to the current device.  The first call of a process also loads the kernels
+ * (driver-internal); make one warm-up call before a region that must not allocate at all.
+ */
+#define UNIFRAC_NOALLOC_MAX_SAMPLES 1024
+#define UNIFRAC_NOALLOC_MAX_PERMS 999
+#define UNIFRAC_NOALLOC_SCRATCH_BYTES (8u * 1024u * 1024u + 64u * 1024u)   /* 1024 x 1024 fp64 square copy + 64 KB */
+int unifrac_mantel_pearson_noalloc(int32_t n_samples, const void *x_condensed, const void *y_condensed,
+                                   unifrac_precision_t precision, const int32_t *perms, int32_t n_perms, double *out,
+                                   void *stream);
+
+/*
  * unifrac_mantel_spearman -- the same test with Spearman's rank correlation ("either Pearson's product-moment
  * correlation coefficient or Spearman's rank correlation coefficient").  rho = Pearson's r of the RANKS of the
  * two condensed vectors, tied values sharing the mean of the ranks they span (1-based fractional ranking, DESIGN.md readings
@@ -281,7 +302,7 @@ int unifrac_measure_rates(unifrac_rates_t *out, void *stream);
 
 const char *unifrac_status_string(int status);
 const char *unifrac_last_cuda_error(void);   /* text of the last CUDA error seen by this thread  */
-int unifrac_abi_version(void);               /* 7                                                */
+int unifrac_abi_version(void);               /* 8                                                */
 
 #ifdef __cplusplus
 }

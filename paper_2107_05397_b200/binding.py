@@ -19,12 +19,12 @@ FP32, FP64 = 0, 1
 FLAG_LITERAL, FLAG_TENSOR_GRAM, FLAG_SKIP_VALIDATION, FLAG_ABSDIFF = 1, 2, 4, 8
 FLAG_NO_TAIL, FLAG_ALL_TAIL, FLAG_NO_TENSOR, FLAG_NO_MID, FLAG_SPARSE_STRIPE, FLAG_RICHNESS_ZONES = 16, 32, 64, 128, 256, 512
 
-ABI_VERSION = 7          # unifrac_abi_version() of the header this binding was written against
+ABI_VERSION = 8          # unifrac_abi_version() of the header this binding was written against
 OK = 0
 ERR_INVALID_ARG, ERR_INVALID_TREE, ERR_INVALID_TABLE, ERR_EMPTY_SAMPLE = -1, -2, -3, -4
 ERR_WORKSPACE, ERR_CUDA, ERR_UNSUPPORTED = -5, -6, -7
 
-EXPORTS = ("unifrac_dm", "unifrac_dm_shard", "unifrac_shard_of_pair", "unifrac_dm_host", "unifrac_dm_host_multi", "unifrac_release_host_pool", "unifrac_mantel_pearson", "unifrac_mantel_spearman", "unifrac_pcoa", "unifrac_measure_rates", "unifrac_last_stats", "unifrac_status_string",
+EXPORTS = ("unifrac_dm", "unifrac_dm_shard", "unifrac_shard_of_pair", "unifrac_dm_host", "unifrac_dm_host_multi", "unifrac_release_host_pool", "unifrac_mantel_pearson", "unifrac_mantel_pearson_noalloc", "unifrac_mantel_spearman", "unifrac_pcoa", "unifrac_measure_rates", "unifrac_last_stats", "unifrac_status_string",
            "unifrac_last_cuda_error", "unifrac_abi_version")
 
 
@@ -99,6 +99,8 @@ def load(build_if_missing: bool = True) -> C.CDLL:
                                            ALLOC_FN, C.c_void_p, C.c_void_p]
     lib.unifrac_mantel_spearman.restype = C.c_int
     lib.unifrac_mantel_spearman.argtypes = lib.unifrac_mantel_pearson.argtypes
+    lib.unifrac_mantel_pearson_noalloc.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
+    lib.unifrac_mantel_pearson_noalloc.restype = C.c_int
     lib.unifrac_pcoa.restype = C.c_int
     lib.unifrac_pcoa.argtypes = [C.c_int32, C.c_void_p, C.c_int, C.c_int32, C.c_int32, C.c_double, C.c_void_p,
                                  C.POINTER(C.c_int32), ALLOC_FN, C.c_void_p, C.c_void_p]
@@ -255,6 +257,36 @@ def unifrac_mantel_pearson(x_condensed, y_condensed, n_samples: int, perms, stre
                                             perms.data_ptr() if K else None, K, out.data_ptr(), cb, None,
                                             C.c_void_p(s.cuda_stream))
     del held
+    _check(lib, rc)
+    return out
+
+
+NOALLOC_MAX_SAMPLES = 1024       # UNIFRAC_NOALLOC_MAX_SAMPLES / _PERMS of the header
+NOALLOC_MAX_PERMS = 999
+
+
+def unifrac_mantel_pearson_noalloc(x_condensed, y_condensed, n_samples: int, perms, out, stream=None):
+    """unifrac_mantel_pearson through the library's static device workspace: no allocation anywhere in the call, so `out`
+    (CUDA float64 [4 + K]) is the caller's too.  n_samples <= 1024, K <= 999 (UnifracError otherwise).  Calls that overlap
+    on the GPU race on the shared workspace.  Returns `out`.  Asynchronous on the stream."""
+    import torch
+    lib = load()
+    dev = x_condensed.device
+    n = int(n_samples)
+    assert dev.type == "cuda" and y_condensed.device == dev and perms.device == dev and out.device == dev
+    assert x_condensed.dtype == y_condensed.dtype and x_condensed.dtype in (torch.float32, torch.float64)
+    assert x_condensed.is_contiguous() and y_condensed.is_contiguous() and perms.is_contiguous() and perms.dtype == torch.int32
+    assert x_condensed.numel() == n * (n - 1) // 2 == y_condensed.numel()
+    K = int(perms.numel() // n) if perms.numel() else 0
+    assert out.dtype == torch.float64 and out.is_contiguous() and out.numel() == 4 + K
+    with torch.cuda.device(dev):
+        s = stream if stream is not None else torch.cuda.current_stream(dev)
+        rc = lib.unifrac_mantel_pearson_noalloc(n, C.c_void_p(x_condensed.data_ptr()), C.c_void_p(y_condensed.data_ptr()),
+                                                FP32 if x_condensed.dtype == torch.float32 else FP64,
+                                                C.c_void_p(perms.data_ptr()) if K else None, K, C.c_void_p(out.data_ptr()),
+                                                C.c_void_p(s.cuda_stream))
+    if rc == ERR_UNSUPPORTED:
+        raise UnifracError(rc, lib.unifrac_status_string(rc).decode() + ": " + lib.unifrac_last_cuda_error().decode())
     _check(lib, rc)
     return out
 

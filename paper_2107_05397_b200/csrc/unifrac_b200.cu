@@ -1366,6 +1366,70 @@ int unifrac_mantel_pearson(int32_t N, const void* x, const void* y, unifrac_prec
     return rc;
 }
 
+// ---- unifrac_mantel_pearson_noalloc (header): run_mantel with its workspace bumped out of a static device array ----------
+// In host code the array's NAME is a host-side stand-in, not a device address: the address the kernels get comes from
+// cudaGetSymbolAddress, once per device, with that device current.
+}  // extern "C"
+static __device__ __align__(256) unsigned char g_noalloc_scratch[UNIFRAC_NOALLOC_SCRATCH_BYTES];
+namespace {
+struct NoAllocBump { unsigned char* base; size_t cap; size_t used; };
+void* noalloc_bump(size_t bytes, void* user)            // Arena::get has rounded bytes up to a multiple of 256
+{
+    NoAllocBump* b = static_cast<NoAllocBump*>(user);
+    if (bytes > b->cap - b->used) return nullptr;       // -> UNIFRAC_ERR_WORKSPACE (the limits below keep a call within cap)
+    void* p = b->base + b->used;
+    b->used += bytes;
+    return p;
+}
+unsigned char* noalloc_scratch_of_current_device()
+{
+    constexpr int MAX_DEV = 64;
+    static std::mutex mu;
+    static unsigned char* ptrs[MAX_DEV] = {};
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= MAX_DEV) throw StatusFail{UNIFRAC_ERR_UNSUPPORTED};
+    std::lock_guard<std::mutex> g(mu);
+    if (!ptrs[dev]) {
+        void* p = nullptr;
+        CU(cudaGetSymbolAddress(&p, g_noalloc_scratch));
+        ptrs[dev] = static_cast<unsigned char*>(p);
+    }
+    return ptrs[dev];
+}
+}  // namespace
+extern "C" {
+
+int unifrac_mantel_pearson_noalloc(int32_t N, const void* x, const void* y, unifrac_precision_t precision, const int32_t* perms,
+                                   int32_t K, double* out, void* stream)
+{
+    if (!x || !y || !out || K < 0 || (K > 0 && !perms) || N < 3) return UNIFRAC_ERR_INVALID_ARG;
+    if (precision != UNIFRAC_FP32 && precision != UNIFRAC_FP64) return UNIFRAC_ERR_INVALID_ARG;
+    if (N > UNIFRAC_NOALLOC_MAX_SAMPLES || K > UNIFRAC_NOALLOC_MAX_PERMS) {
+        char b[256];
+        snprintf(b, sizeof(b), "unifrac_mantel_pearson_noalloc: n_samples = %d, n_perms = %d beyond the static workspace "
+                 "(UNIFRAC_NOALLOC_MAX_SAMPLES = %d, UNIFRAC_NOALLOC_MAX_PERMS = %d); use unifrac_mantel_pearson",
+                 (int)N, (int)K, UNIFRAC_NOALLOC_MAX_SAMPLES, UNIFRAC_NOALLOC_MAX_PERMS);
+        g_cuda_err = b;
+        return UNIFRAC_ERR_UNSUPPORTED;
+    }
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    int rc = UNIFRAC_OK;
+    try {
+        NoAllocBump bump{noalloc_scratch_of_current_device(), (size_t)UNIFRAC_NOALLOC_SCRATCH_BYTES, 0};
+        Arena A{noalloc_bump, &bump, st};               // fn != NULL: the arena owns nothing and release() frees nothing
+        if (precision == UNIFRAC_FP32) run_mantel<float>(N, reinterpret_cast<const float*>(x), reinterpret_cast<const float*>(y), perms, K, out, A, st);
+        else run_mantel<double>(N, reinterpret_cast<const double*>(x), reinterpret_cast<const double*>(y), perms, K, out, A, st);
+    } catch (const CudaFail& f) {
+        char b[512];
+        snprintf(b, sizeof(b), "%s: %s (unifrac_b200.cu:%d)", f.what, cudaGetErrorString(f.e), f.line);
+        g_cuda_err = b; cudaGetLastError(); rc = UNIFRAC_ERR_CUDA;
+    } catch (const WorkspaceFail&) { rc = UNIFRAC_ERR_WORKSPACE; g_cuda_err = "unifrac_mantel_pearson_noalloc: static workspace exhausted"; }
+    catch (const StatusFail& f) { rc = f.status; }
+    catch (...) { rc = UNIFRAC_ERR_CUDA; g_cuda_err = "unexpected C++ exception"; }
+    return rc;
+}
+
 int unifrac_mantel_spearman(int32_t N, const void* x, const void* y, unifrac_precision_t precision, const int32_t* perms,
                             int32_t K, double* out, unifrac_alloc_fn alloc, void* user, void* stream)
 {
@@ -1493,6 +1557,6 @@ const char* unifrac_status_string(int status)
 }
 
 const char* unifrac_last_cuda_error(void) { return g_cuda_err.c_str(); }
-int unifrac_abi_version(void) { return 7; }
+int unifrac_abi_version(void) { return 8; }
 
 }  // extern "C"
