@@ -201,6 +201,8 @@ typedef struct {
     uint32_t guard_pairs;        /* pairs with d < 1/16 that the near-duplicate guard recomputed from the definition */
     uint32_t guard_capacity;     /* size of the guard's pair list: min(P, max(2^22, 64 N)); pairs listed beyond it keep
                                     their separable-form value (absolute error ~1e-7 in fp32)                           */
+    uint32_t mid_groups;         /* grouped join (k_midg): groups of nested mid branches ...                          */
+    uint32_t mid_group_rows;     /* ... and the mid rows in them (the other mid_rows - mid_group_rows rows go through k_mid) */
     uint32_t quant_fallback;     /* 1 if the fixed-point error ratio was over budget and the call was rerun without
                                     the fixed-point kernels (tensor-core Gram, shared-memory mid)                       */
     float guard_theta;           /* the guard's threshold of this call: max(1/16, quant_err_ratio / 2.5e-6)            */

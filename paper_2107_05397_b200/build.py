@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libunifrac_b200.so")
 SOURCES = ["unifrac_b200.cu"]
-HEADERS = ["common.cuh", "rank.cuh", "perm.cuh", "zone.cuh", "pcoa.cuh", "guard.cuh", "plan.cuh", "embed.cuh", "tail.cuh", "stripe.cuh", "gram.cuh", "mid.cuh", "dense.cuh", "rates.cuh", "mantel.cuh"]
+HEADERS = ["common.cuh", "rank.cuh", "perm.cuh", "zone.cuh", "pcoa.cuh", "guard.cuh", "plan.cuh", "embed.cuh", "tail.cuh", "stripe.cuh", "gram.cuh", "mid.cuh", "midg.cuh", "dense.cuh", "rates.cuh", "mantel.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "--expt-relaxed-constexpr"]
 

@@ -31,17 +31,18 @@ constexpr size_t MID_SMEM = (size_t)TILE * TILE * sizeof(uint32_t) + 512 /*align
 // mid rows ordered by n_v (counting sort: histogram, scan, scatter) so that the rows a warp handles together
 // have similar list lengths; mbase[r] = list offset of row r.  The order inside a bucket is arbitrary --
 // harmless, integer accumulation commutes.
-__global__ void k_mid_hist(int n, const uint8_t* __restrict__ cls, const uint32_t* __restrict__ nv, uint32_t* __restrict__ hist)
+__global__ void k_mid_hist(int n, const uint8_t* __restrict__ cls, const uint32_t* __restrict__ nv, uint32_t* __restrict__ hist,
+                           uint8_t want /* class of the rows: CLS_MID, or CLS_MIDG_ROOT (midg.cuh) */)
 {
     int v = blockIdx.x * blockDim.x + threadIdx.x;
-    if (v < n && cls[v] == CLS_MID) atomicAdd(&hist[nv[v]], 1u);
+    if (v < n && cls[v] == want) atomicAdd(&hist[nv[v]], 1u);
 }
 __global__ void k_mid_rows(int n, const uint8_t* __restrict__ cls, const uint32_t* __restrict__ nv, uint32_t* __restrict__ cursor,
                            const uint32_t* __restrict__ tptr, int32_t* __restrict__ mrows, uint32_t* __restrict__ mbase,
-                           uint32_t* __restrict__ mlen)
+                           uint32_t* __restrict__ mlen, uint8_t want)
 {
     int v = blockIdx.x * blockDim.x + threadIdx.x;
-    if (v < n && cls[v] == CLS_MID) {
+    if (v < n && cls[v] == want) {
         uint32_t r = atomicAdd(&cursor[nv[v]], 1u);
         mrows[r] = v;
         mbase[r] = tptr[v];

@@ -1,0 +1,244 @@
+// midg.cuh -- step a-5 for the mid branches, GROUPED join (fp32 mode).  PAPER.md:23 "sparse-aware optimizations"; the
+// mechanism is ours.
+//
+// The samples in which a branch is present are a SUBSET of the samples in which its parent branch is present (a-2: a parent's
+// bit row is the OR of its children's, its counts their sum).  So for a group of mid branches below a group ROOT r -- r itself
+// and up to MIDG_L - 1 descendants connected to it -- every pair of samples (a, b) that any member touches is a pair of r, and
+//     sum over the members v of min(u~_va, u~_vb)        (u~ = 0 where v is absent: min(0, x) = 0 adds nothing)
+// can be formed in registers and added to the tile pair's accumulator with ONE shared-memory atomic per pair of r instead of
+// one per member.  The atomic unit is what bounds k_mid (8.8 lanes/clk/SM); at Large / weighted the groups chosen below need
+// 0.38 of k_mid's atomics for the same sums (profiles/r02_summary.md 4d).
+//
+// Grouping (k_midg_level, top-down by tree level): a mid branch c whose parent belongs to the group of root r joins that group
+// if n_c > theta n_r and the group still has a free slot; otherwise c starts a group of its own.  Groups that stay alone
+// (one member) remain ordinary k_mid rows.  Which of several competing children gets the last slot depends on the order of
+// atomics; the RESULT does not: all sums are exact integer sums of the same fixed-point values q = round(u~ 2^F) that k_mid uses.
+//
+// Layout: the root's entries are packed tile-major exactly like k_mid's rows (k_mid_seg / k_mid_off on the root list);
+// position p holds  ex[p] = g << 9 | (sample - 128 t) << 2  and  eq[p] = the MIDG_L fixed-point values of the members at
+// that sample (slot 0 = the root; 0 where a member is absent or the slot is unused).
+#pragma once
+#include "mid.cuh"
+
+namespace ufb {
+
+constexpr int MIDG_L = 4;
+constexpr uint8_t CLS_MIDG_ROOT = 4, CLS_MIDG_MEMBER = 5;
+constexpr int MIDG_THREADS = 384;
+constexpr int MIDG_MINB = 3;
+
+// children of the internal nodes of one tree level: groot[c] = root of c's group, gslot[c] = its slot, gcnt[r] = members so far
+__global__ void k_midg_level(uint32_t n_lv, const int32_t* __restrict__ level_nodes, const uint32_t* __restrict__ child_off,
+                             const int32_t* __restrict__ child_idx, const uint8_t* __restrict__ cls, const uint32_t* __restrict__ nv,
+                             uint32_t theta_256, int32_t* __restrict__ groot, uint8_t* __restrict__ gslot, uint32_t* __restrict__ gcnt)
+{
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_lv) return;
+    const int u = level_nodes[i];
+    const int r = cls[u] == CLS_MID ? groot[u] : -1;
+    const unsigned long long lim = r >= 0 ? (unsigned long long)theta_256 * nv[r] : 0ull;
+    for (uint32_t k = child_off[u]; k < child_off[u + 1]; ++k) {
+        const int c = child_idx[k];
+        if (cls[c] != CLS_MID) continue;
+        int g = c; uint32_t slot = 0;
+        if (r >= 0 && (unsigned long long)nv[c] * 256ull > lim) {
+            slot = atomicAdd(&gcnt[r], 1u);
+            if (slot < (uint32_t)MIDG_L) g = r; else slot = 0;
+        }
+        groot[c] = g;
+        gslot[c] = (uint8_t)slot;
+        if (g == c) gcnt[c] = 1u;
+    }
+}
+
+// members of groups with at least two members leave the k_mid rows: cnt[0] += roots, cnt[1] += rows (roots + members),
+// cnt[2] += entries of the roots, cnt[3] += sum of n_v (n_v - 1) / 2 over the rows that left
+__global__ void k_midg_classify(int n, uint8_t* __restrict__ cls, const uint32_t* __restrict__ nv, const int32_t* __restrict__ groot,
+                                const uint32_t* __restrict__ gcnt, unsigned long long* __restrict__ cnt)
+{
+    const int v = blockIdx.x * blockDim.x + threadIdx.x;
+    if (v >= n || cls[v] != CLS_MID) return;
+    const int r = groot[v];
+    if (gcnt[r] < 2u) return;
+    const bool is_root = r == v;
+    cls[v] = is_root ? CLS_MIDG_ROOT : CLS_MIDG_MEMBER;
+    const unsigned long long k = nv[v];
+    if (is_root) { atomicAdd(&cnt[0], 1ull); atomicAdd(&cnt[2], k); }
+    atomicAdd(&cnt[1], 1ull);
+    atomicAdd(&cnt[3], k * (k - 1) / 2);
+}
+
+// per-sample sums over the grouped rows (they count toward the bound of the fixed-point accumulators like k_mid's rows)
+__global__ void __launch_bounds__(256)
+k_midg_sums(int n, const uint8_t* __restrict__ cls, const uint32_t* __restrict__ tptr, const uint32_t* __restrict__ nv,
+            const uint32_t* __restrict__ ts, const float* __restrict__ tv, double* __restrict__ midsum)
+{
+    const int v = (int)((blockIdx.x * (unsigned)blockDim.x + threadIdx.x) >> 5);
+    const int lane = threadIdx.x & 31;
+    if (v >= n || (cls[v] != CLS_MIDG_ROOT && cls[v] != CLS_MIDG_MEMBER)) return;
+    const uint32_t base = tptr[v], m = nv[v];
+    for (uint32_t k = lane; k < m; k += 32) atomicAdd(&midsum[ts[base + k]], (double)tv[base + k]);
+}
+
+__global__ void k_midg_index(uint32_t n_g, const int32_t* __restrict__ grows, int32_t* __restrict__ rootidx)
+{
+    const uint32_t g = blockIdx.x * blockDim.x + threadIdx.x;
+    if (g < n_g) rootidx[grows[g]] = (int32_t)g;
+}
+
+// fixed-point value of an entry and the correction of the sample's side sum (the same bookkeeping as k_mid_pack)
+__device__ __forceinline__ uint32_t midg_quant(float u, uint32_t s, float qscale, double inv_qscale, double* __restrict__ sums,
+                                               double* __restrict__ qerr)
+{
+    const uint32_t q = __float2uint_rn(u * qscale);
+    const double c = (double)q * inv_qscale - (double)u;
+    if (c != 0.0) { atomicAdd(&sums[s], c); atomicAdd(&qerr[2 * s], c); atomicAdd(&qerr[2 * s + 1], c * c); }
+    return q;
+}
+
+// roots: one warp per group g.  ex / eq of the padding position of an odd (group, tile) list: ex repeats a valid cell, eq = 0.
+__global__ void __launch_bounds__(256)
+k_midg_pack_roots(uint32_t n_g, const uint32_t* __restrict__ gbase, const uint32_t* __restrict__ glen,
+                  const uint32_t* __restrict__ ts, const float* __restrict__ tv, const uint32_t* __restrict__ seg,
+                  const uint32_t* __restrict__ off, const uint32_t* __restrict__ tbase, float qscale, double inv_qscale,
+                  double* __restrict__ sums, double* __restrict__ qerr, uint32_t* __restrict__ ex, uint32_t* __restrict__ eq)
+{
+    const uint32_t g = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (g >= n_g) return;
+    const uint32_t base = gbase[g], m = glen[g];
+    for (uint32_t k = lane; k < m; k += 32) {
+        const uint32_t s = ts[base + k];
+        const uint32_t t = s >> 7;
+        const uint32_t g0 = seg[(size_t)t * n_g + g], g1 = seg[(size_t)(t + 1) * n_g + g];
+        const uint32_t pos = tbase[t] + off[(size_t)t * (n_g + 1) + g] + (k - g0);
+        const uint32_t x = (g << 9) | ((s & 127u) << 2);
+        ex[pos] = x;
+        eq[(size_t)pos * MIDG_L] = midg_quant(tv[base + k], s, qscale, inv_qscale, sums, qerr);
+        if (k + 1 == g1 && ((g1 - g0) & 1u)) ex[pos + 1] = x;
+    }
+}
+
+// members: one warp per tree node (only CLS_MIDG_MEMBER nodes do anything).  Every sample of the member is a sample of its
+// root: its position in the root's sorted list comes from a binary search; a miss (never, by the subset property) is counted.
+__global__ void __launch_bounds__(256)
+k_midg_pack_members(int n, const uint8_t* __restrict__ cls, const int32_t* __restrict__ groot, const uint8_t* __restrict__ gslot,
+                    const int32_t* __restrict__ rootidx, const uint32_t* __restrict__ tptr, const uint32_t* __restrict__ nv,
+                    const uint32_t* __restrict__ ts, const float* __restrict__ tv, uint32_t n_g, const uint32_t* __restrict__ seg,
+                    const uint32_t* __restrict__ off, const uint32_t* __restrict__ tbase, float qscale, double inv_qscale,
+                    double* __restrict__ sums, double* __restrict__ qerr, uint32_t* __restrict__ eq, unsigned long long* __restrict__ misses)
+{
+    const int v = (int)((blockIdx.x * (unsigned)blockDim.x + threadIdx.x) >> 5);
+    const int lane = threadIdx.x & 31;
+    if (v >= n || cls[v] != CLS_MIDG_MEMBER) return;
+    const int r = groot[v];
+    const uint32_t g = (uint32_t)rootidx[r], slot = gslot[v];
+    const uint32_t base = tptr[v], m = nv[v], rbase = tptr[r], rm = nv[r];
+    for (uint32_t k = lane; k < m; k += 32) {
+        const uint32_t s = ts[base + k];
+        uint32_t lo = 0, hi = rm;                                 // first root entry with sample >= s
+        while (lo < hi) { const uint32_t mid = (lo + hi) >> 1; if (ts[rbase + mid] < s) lo = mid + 1; else hi = mid; }
+        if (lo >= rm || ts[rbase + lo] != s) { atomicAdd(misses, 1ull); continue; }
+        const uint32_t t = s >> 7;
+        const uint32_t pos = tbase[t] + off[(size_t)t * (n_g + 1) + g] + (lo - seg[(size_t)t * n_g + g]);
+        eq[(size_t)pos * MIDG_L + slot] = midg_quant(tv[base + k], s, qscale, inv_qscale, sums, qerr);
+    }
+}
+
+struct MidgParams {
+    const int2* pairs; uint32_t n_pairs;
+    unsigned int* counter;        // dynamic tile-pair queue
+    uint32_t n_g;
+    const uint32_t* off;          // [n_tiles][n_g+1]
+    const uint32_t* tbase;        // [n_tiles+1]
+    const uint32_t* ex;           // packed positions, tile-major, groups ascending within a tile
+    const uint4* eq;              // MIDG_L = 4 values per position
+    int n_samples;
+    float* out;
+    double inv_qscale;            // 2^-F
+};
+
+__device__ __forceinline__ uint32_t midg_dot(const uint4& a, const uint4& b) {
+    return min(a.x, b.x) + min(a.y, b.y) + min(a.z, b.z) + min(a.w, b.w);
+}
+
+// The grouped join: every position (group g, sample a, values qa[]) of tile I meets the positions (g, b, qb[]) of the same
+// group in tile J; one lane per I position, chunks of 32 consecutive I positions per warp, software pipelined like k_mid.
+__global__ void __launch_bounds__(MIDG_THREADS, MIDG_MINB)
+k_midg(const MidgParams P)
+{
+    extern __shared__ uint32_t macc_raw[];
+    __shared__ int s_pair;
+    const uint32_t raw_s = smem_u32(macc_raw);
+    const uint32_t macc_s = (raw_s + 511u) & ~511u;                    // 512-byte aligned rows: row a at macc_s + 512 a
+    uint32_t* macc = macc_raw + ((macc_s - raw_s) >> 2);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    constexpr int NWARP = MIDG_THREADS / 32;
+    const long long N = P.n_samples;
+    const size_t pitch = (size_t)P.n_g + 1;
+    const uint32_t* __restrict__ ex = P.ex;
+    const uint4* __restrict__ eq = P.eq;
+
+    for (;;) {
+        if (threadIdx.x == 0) s_pair = (int)atomicAdd(P.counter, 1u);
+        for (int i = threadIdx.x; i < TILE * TILE; i += MIDG_THREADS) macc[i] = 0u;
+        __syncthreads();
+        const int pi = s_pair;
+        if ((uint32_t)pi >= P.n_pairs) break;
+        const int2 ij = P.pairs[pi];
+        const uint32_t eI0 = P.tbase[ij.x], eI1 = P.tbase[ij.x + 1], eJ0 = P.tbase[ij.y];
+        const uint32_t* offJ = P.off + (size_t)ij.y * pitch;
+        const uint32_t nchunk = (eI1 - eI0 + 31u) >> 5;
+
+        // pipeline: stage B = position + J range of chunk c+1, stage C = current
+        uint32_t xB = 0, xC; uint4 qB = make_uint4(0u, 0u, 0u, 0u), qC;
+        uint32_t jB0 = 0, jB1 = 0, jC0, jC1;
+        auto load_pos = [&](uint32_t c, uint32_t& x, uint4& q, uint32_t& j0, uint32_t& j1) {
+            const uint32_t e = eI0 + c * 32u + lane;
+            j0 = j1 = 0; x = 0; q = make_uint4(0u, 0u, 0u, 0u);
+            if (c < nchunk && e < eI1) {
+                x = __ldg(ex + e); q = __ldg(eq + e);
+                if (q.x | q.y | q.z | q.w) {                 // all-zero (padding) positions contribute nothing
+                    const uint32_t g = x >> 9;
+                    j0 = eJ0 + offJ[g];                      // both even
+                    j1 = eJ0 + offJ[g + 1];
+                }
+            }
+        };
+        uint32_t c = warp;
+        load_pos(c, xB, qB, jB0, jB1);
+        for (; c < nchunk; c += NWARP) {
+            xC = xB; qC = qB; jC0 = jB0; jC1 = jB1;
+            load_pos(c + NWARP, xB, qB, jB0, jB1);
+            const uint32_t a4 = xC & 0x1fcu;                                      // 4 a
+            const uint32_t arow = (macc_s + (a4 << 7)) | (a4 & 0x7cu);            // row base | (a & 31) << 2
+            uint32_t l = jC0;
+            while (__any_sync(0xffffffffu, l < jC1)) {
+                const bool p0 = l < jC1, p1 = l + 2u < jC1;
+                uint2 x0, x1; uint4 b0, b1, b2, b3;
+                if (p0) { x0 = __ldg(reinterpret_cast<const uint2*>(ex + l)); b0 = __ldg(eq + l); b1 = __ldg(eq + l + 1); }
+                if (p1) { x1 = __ldg(reinterpret_cast<const uint2*>(ex + l + 2)); b2 = __ldg(eq + l + 2); b3 = __ldg(eq + l + 3); }
+                if (p0) { mid_red(arow ^ (x0.x & 0x1fcu), midg_dot(qC, b0)); mid_red(arow ^ (x0.y & 0x1fcu), midg_dot(qC, b1)); }
+                if (p1) { mid_red(arow ^ (x1.x & 0x1fcu), midg_dot(qC, b2)); mid_red(arow ^ (x1.y & 0x1fcu), midg_dot(qC, b3)); }
+                l += 4;
+            }
+        }
+        __syncthreads();
+        // ---- epilogue: add the tile pair's fixed-point sums to the condensed matrix (exclusive owner, after k_mid's)
+        const uint32_t sI = (uint32_t)ij.x * TILE, sJ = (uint32_t)ij.y * TILE;
+        for (int e = threadIdx.x; e < TILE * TILE; e += MIDG_THREADS) {
+            const int a = e >> 7, b = (e & 127) ^ (a & 31);
+            const uint32_t q = macc[e];
+            if (q) {
+                const long long gi = (long long)sI + a, gj = (long long)sJ + b;
+                if (gi < gj && gj < N) {
+                    float* o = P.out + (gi * (2 * N - gi - 1) / 2 - gi - 1 + gj);
+                    *o = (float)((double)*o + (double)q * P.inv_qscale);
+                }
+            }
+        }
+        __syncthreads();
+    }
+}
+
+}  // namespace ufb

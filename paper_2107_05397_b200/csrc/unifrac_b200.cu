@@ -17,6 +17,7 @@
 #include "zone.cuh"
 #include "pcoa.cuh"
 #include "guard.cuh"
+#include "midg.cuh"
 
 #include <cstdio>
 #include <cstdlib>
@@ -362,8 +363,8 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     uint8_t* cls = A.get_n<uint8_t>(n);
     uint32_t* tcnt = A.get_n<uint32_t>(n);
     uint32_t* tptr = A.get_n<uint32_t>((size_t)n + 1);
-    unsigned long long* work = A.get_n<unsigned long long>(24);
-    CU(cudaMemsetAsync(work, 0, sizeof(unsigned long long) * 24, st));
+    unsigned long long* work = A.get_n<unsigned long long>(28);
+    CU(cudaMemsetAsync(work, 0, sizeof(unsigned long long) * 28, st));
     uint32_t* bits = A.get_n<uint32_t>((size_t)n * NW);
     {
         CU(cudaMemsetAsync(bits, 0, sizeof(uint32_t) * (size_t)n * NW, st));
@@ -676,6 +677,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     unsigned mid_launches = 0;
     int mid_F = 0;
     bool mid_packed = false;
+    uint32_t midg_groups = 0, midg_rows = 0;
     double quant_ratio = 0.0;
     // fixed-point error ratio (Gram head lengths + mid entries): over budget => rerun without the fixed-point kernels
     auto check_quant_ratio = [&]() {
@@ -690,64 +692,144 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     if (mid_rows || skip_on) {
         if constexpr (std::is_same<T, float>::value) {
             if (mid_rows >= (1ull << 23)) throw StatusFail{UNIFRAC_ERR_UNSUPPORTED};     // packed entries keep the row in 23 bits
-            const uint32_t n_mid = skip_on ? sk_n : (uint32_t)mid_rows;
-            int32_t* mrows = sk_rows; uint32_t* mbase = sk_base; uint32_t* mlen = sk_len;
-            if (!skip_on) {
-                uint32_t* mhist = A.get_n<uint32_t>((size_t)N + 2);
-                uint32_t* mcur = A.get_n<uint32_t>((size_t)N + 2);
-                mrows = A.get_n<int32_t>(n_mid);
-                mbase = A.get_n<uint32_t>(n_mid);
-                mlen = A.get_n<uint32_t>(n_mid);
-                CU(cudaMemsetAsync(mhist, 0, sizeof(uint32_t) * ((size_t)N + 2), st));
-                k_mid_hist<<<cdiv(n, TB), TB, 0, st>>>(n, cls, nv, mhist); CU_LAUNCH(); ++launches;
-                k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>(N + 1, mhist, mcur); CU_LAUNCH(); ++launches;
-                k_mid_rows<<<cdiv(n, TB), TB, 0, st>>>(n, cls, nv, mcur, tptr, mrows, mbase, mlen); CU_LAUNCH(); ++launches;
+            // ---- grouped join (midg.cuh): mid branches whose presence sets nest are joined with one atomic per pair of the
+            // group's root; rows that end up alone stay k_mid rows
+            uint32_t n_g = 0;
+            unsigned long long g_rows = 0;
+            int32_t* groot = nullptr; uint8_t* gslot = nullptr;
+            const bool groups_on = !skip_on && mid_rows >= 2 && envd("UNIFRAC_B200_MID_GROUPS", 1.0) != 0.0;
+            if (groups_on) {
+                groot = A.get_n<int32_t>(n); gslot = A.get_n<uint8_t>(n);
+                uint32_t* gcnt = A.get_n<uint32_t>(n);
+                unsigned long long* gc = A.get_n<unsigned long long>(4);
+                CU(cudaMemsetAsync(gcnt, 0, sizeof(uint32_t) * n, st));
+                CU(cudaMemsetAsync(gc, 0, sizeof(unsigned long long) * 4, st));
+                const uint32_t theta_256 = (uint32_t)std::lround(256.0 * envd("UNIFRAC_B200_MID_GROUP_THETA", 0.5));
+                for (int d = 0; d < n_levels; ++d)
+                    if (h_hist[d]) {
+                        k_midg_level<<<cdiv(h_hist[d], TB), TB, 0, st>>>(h_hist[d], level_nodes + h_off[d], child_off, child_idx, cls, nv,
+                                                                         theta_256, groot, gslot, gcnt);
+                        CU_LAUNCH(); ++launches;
+                    }
+                k_midg_classify<<<cdiv(n, TB), TB, 0, st>>>(n, cls, nv, groot, gcnt, gc); CU_LAUNCH(); ++launches;
+                unsigned long long h_gc[4] = {0, 0, 0, 0};
+                CU(cudaMemcpyAsync(h_gc, gc, sizeof(h_gc), cudaMemcpyDeviceToHost, st));
+                CU(cudaStreamSynchronize(st));
+                n_g = (uint32_t)h_gc[0]; g_rows = h_gc[1];
+                midg_groups = n_g; midg_rows = (uint32_t)g_rows;
             }
-            uint32_t* mseg = A.get_n<uint32_t>((size_t)(n_tiles + 1) * n_mid);
-            k_mid_seg<<<cdiv((long long)n_mid * 32, TB), TB, 0, st>>>(n_mid, mrows, tptr, ts, n_tiles, mseg); CU_LAUNCH(); ++launches;
-            uint32_t* moff = A.get_n<uint32_t>((size_t)n_tiles * ((size_t)n_mid + 1));
-            uint32_t* ttot = A.get_n<uint32_t>(n_tiles);
-            uint32_t* tbase = A.get_n<uint32_t>((size_t)n_tiles + 1);
-            k_mid_off<<<n_tiles, 1024, 0, st>>>(n_mid, mseg, moff, ttot, sk_cut); CU_LAUNCH(); ++launches;
-            k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>(n_tiles, ttot, tbase); CU_LAUNCH(); ++launches;
+            const uint32_t n_mid = skip_on ? sk_n : (uint32_t)(mid_rows - g_rows);
+            // row lists of one class ordered by n_v (counting sort)
+            auto class_rows = [&](uint8_t want, uint32_t count, int32_t*& rows, uint32_t*& base, uint32_t*& len) {
+                uint32_t* hh = A.get_n<uint32_t>((size_t)N + 2);
+                uint32_t* cc = A.get_n<uint32_t>((size_t)N + 2);
+                rows = A.get_n<int32_t>(count ? count : 1);
+                base = A.get_n<uint32_t>(count ? count : 1);
+                len = A.get_n<uint32_t>(count ? count : 1);
+                CU(cudaMemsetAsync(hh, 0, sizeof(uint32_t) * ((size_t)N + 2), st));
+                k_mid_hist<<<cdiv(n, TB), TB, 0, st>>>(n, cls, nv, hh, want); CU_LAUNCH(); ++launches;
+                k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>(N + 1, hh, cc); CU_LAUNCH(); ++launches;
+                k_mid_rows<<<cdiv(n, TB), TB, 0, st>>>(n, cls, nv, cc, tptr, rows, base, len, want); CU_LAUNCH(); ++launches;
+            };
+            // tile-major offsets of the rows' (row, tile) lists
+            struct TileLists { uint32_t* seg; uint32_t* off; uint32_t* tbase; };
+            auto tile_lists = [&](uint32_t count, const int32_t* rows, const uint32_t* cut) {
+                TileLists L{};
+                L.seg = A.get_n<uint32_t>((size_t)(n_tiles + 1) * std::max<uint32_t>(count, 1u));
+                L.off = A.get_n<uint32_t>((size_t)n_tiles * ((size_t)count + 1));
+                uint32_t* ttot = A.get_n<uint32_t>(n_tiles);
+                L.tbase = A.get_n<uint32_t>((size_t)n_tiles + 1);
+                if (count) { k_mid_seg<<<cdiv((long long)count * 32, TB), TB, 0, st>>>(count, rows, tptr, ts, n_tiles, L.seg); CU_LAUNCH(); ++launches; }
+                k_mid_off<<<n_tiles, 1024, 0, st>>>(count, L.seg, L.off, ttot, cut); CU_LAUNCH(); ++launches;
+                k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>(n_tiles, ttot, L.tbase); CU_LAUNCH(); ++launches;
+                return L;
+            };
+            int32_t* mrows = sk_rows; uint32_t* mbase = sk_base; uint32_t* mlen = sk_len;
+            if (!skip_on) class_rows(CLS_MID, n_mid, mrows, mbase, mlen);
+            const TileLists ML = tile_lists(n_mid, mrows, sk_cut);
+            int32_t* grows = nullptr; uint32_t* gbase = nullptr; uint32_t* glen = nullptr;
+            TileLists GLs{};
+            if (n_g) { class_rows(CLS_MIDG_ROOT, n_g, grows, gbase, glen); GLs = tile_lists(n_g, grows, nullptr); }
             unsigned long long* smax = work + 15;
             double* midsum = A.get_n<double>((size_t)n_tiles * TILE);
             CU(cudaMemsetAsync(midsum, 0, sizeof(double) * (size_t)n_tiles * TILE, st));
-            k_mid_sums<<<cdiv((long long)n_mid * 32, TB), TB, 0, st>>>(n_mid, mbase, mlen, ts, reinterpret_cast<const float*>(tv), midsum, sk_cut); CU_LAUNCH(); ++launches;
+            if (n_mid) { k_mid_sums<<<cdiv((long long)n_mid * 32, TB), TB, 0, st>>>(n_mid, mbase, mlen, ts, reinterpret_cast<const float*>(tv), midsum, sk_cut); CU_LAUNCH(); ++launches; }
+            if (n_g) { k_midg_sums<<<cdiv((long long)n * 32, TB), TB, 0, st>>>(n, cls, tptr, nv, ts, reinterpret_cast<const float*>(tv), midsum); CU_LAUNCH(); ++launches; }
             k_max_positive<<<cdiv((long long)n_tiles * TILE, TB), TB, 0, st>>>(n_tiles * TILE, midsum, smax); CU_LAUNCH(); ++launches;
             unsigned long long h_smax = 0;
             CU(cudaMemcpyAsync(&h_smax, smax, sizeof(h_smax), cudaMemcpyDeviceToHost, st));
-            uint32_t h_pk_total = 0;                            // packed entries incl. the even-length padding
-            CU(cudaMemcpyAsync(&h_pk_total, tbase + n_tiles, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+            uint32_t h_pk_total = 0, h_g_total = 0;             // packed entries / positions incl. the even-length padding
+            CU(cudaMemcpyAsync(&h_pk_total, ML.tbase + n_tiles, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+            if (n_g) CU(cudaMemcpyAsync(&h_g_total, GLs.tbase + n_tiles, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
             std::vector<int2> h_mp = blocked_pairs(n_tiles, 8, shard, n_shards);
+            const size_t n_all_pairs = h_mp.size();
+            int2* gpairs = A.get_n<int2>(n_all_pairs ? n_all_pairs : 1);     // the grouped join visits every tile pair of the shard
+            CU(cudaMemcpyAsync(gpairs, h_mp.data(), sizeof(int2) * n_all_pairs, cudaMemcpyHostToDevice, st));
             if (skip_on)                                          // pairs whose rows all go to k_zone have nothing to join
                 h_mp.erase(std::remove_if(h_mp.begin(), h_mp.end(), [&](const int2& q) { return h_cut[q.x] >= sk_n; }), h_mp.end());
-            int2* mpairs = A.get_n<int2>(h_mp.size());
+            int2* mpairs = A.get_n<int2>(h_mp.size() ? h_mp.size() : 1);
             CU(cudaMemcpyAsync(mpairs, h_mp.data(), sizeof(int2) * h_mp.size(), cudaMemcpyHostToDevice, st));
             CU(cudaStreamSynchronize(st));
             double sm; memcpy(&sm, &h_smax, sizeof(sm));
             int ex = 0; frexp(sm > 0 ? sm : 1.0, &ex);          // sm < 2^ex
             // unsigned 32-bit cells: acc <= min(R^mid_a, R^mid_b) * 2^F + (rounding: at most half a unit per mid row)
             mid_F = 32 - ex;
-            if (ldexp(sm, mid_F) + 0.5 * (double)n_mid + 1.0 > 4294967295.0) --mid_F;
+            if (ldexp(sm, mid_F) + 0.5 * (double)(n_mid + g_rows) + 1.0 > 4294967295.0) --mid_F;
             (void)mid_entries;
+            const float qscale = ldexpf(1.0f, mid_F);
+            const double inv_qscale = ldexp(1.0, -mid_F);
             uint2* pk = A.get_n<uint2>(h_pk_total ? h_pk_total : 1);
-            k_mid_pack<<<cdiv((long long)n_mid * 32, TB), TB, 0, st>>>(n_mid, mbase, mlen, ts, reinterpret_cast<const float*>(tv), mseg, moff, tbase,
-                                                                      ldexpf(1.0f, mid_F), ldexp(1.0, -mid_F), sums, qerr, pk, sk_cut); CU_LAUNCH(); ++launches;
+            if (n_mid) {
+                k_mid_pack<<<cdiv((long long)n_mid * 32, TB), TB, 0, st>>>(n_mid, mbase, mlen, ts, reinterpret_cast<const float*>(tv), ML.seg, ML.off, ML.tbase,
+                                                                          qscale, inv_qscale, sums, qerr, pk, sk_cut); CU_LAUNCH(); ++launches;
+            }
+            uint32_t* gex = nullptr; uint32_t* geq = nullptr;
+            unsigned long long* gmiss = work + 24;
+            if (n_g) {
+                gex = A.get_n<uint32_t>((size_t)h_g_total + 2);
+                geq = A.get_n<uint32_t>(((size_t)h_g_total + 2) * MIDG_L);
+                int32_t* rootidx = A.get_n<int32_t>(n);
+                CU(cudaMemsetAsync(gex, 0, sizeof(uint32_t) * ((size_t)h_g_total + 2), st));
+                CU(cudaMemsetAsync(geq, 0, sizeof(uint32_t) * ((size_t)h_g_total + 2) * MIDG_L, st));
+                k_midg_index<<<cdiv(n_g, TB), TB, 0, st>>>(n_g, grows, rootidx); CU_LAUNCH(); ++launches;
+                k_midg_pack_roots<<<cdiv((long long)n_g * 32, TB), TB, 0, st>>>(n_g, gbase, glen, ts, reinterpret_cast<const float*>(tv), GLs.seg, GLs.off,
+                                                                               GLs.tbase, qscale, inv_qscale, sums, qerr, gex, geq); CU_LAUNCH(); ++launches;
+                k_midg_pack_members<<<cdiv((long long)n * 32, TB), TB, 0, st>>>(n, cls, groot, gslot, rootidx, tptr, nv, ts, reinterpret_cast<const float*>(tv),
+                                                                               n_g, GLs.seg, GLs.off, GLs.tbase, qscale, inv_qscale, sums, qerr, geq, gmiss);
+                CU_LAUNCH(); ++launches;
+            }
             mid_packed = true;
             check_quant_ratio();
-            MidParams M{};
-            M.pairs = mpairs; M.n_pairs = (uint32_t)h_mp.size(); M.counter = reinterpret_cast<unsigned int*>(work + 7);
-            M.n_mid = n_mid; M.off = moff; M.tbase = tbase; M.pk = pk; M.cut = sk_cut;
-            M.n_samples = N; M.out = reinterpret_cast<float*>(out); M.inv_qscale = ldexp(1.0, -mid_F);
-            CU(cudaFuncSetAttribute(k_mid, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MID_SMEM));
-            int occ = 0, dev2 = 0, n_sm2 = 0;
+            if (n_g) {                                            // (the stream was just synchronised)
+                unsigned long long h_miss = 0;
+                CU(cudaMemcpy(&h_miss, gmiss, sizeof(h_miss), cudaMemcpyDeviceToHost));
+                if (h_miss) { g_cuda_err = "grouped join: a member branch has a sample its group root lacks"; throw StatusFail{UNIFRAC_ERR_CUDA}; }
+            }
+            int dev2 = 0, n_sm2 = 0;
             CU(cudaGetDevice(&dev2));
             CU(cudaDeviceGetAttribute(&n_sm2, cudaDevAttrMultiProcessorCount, dev2));
-            CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_mid, MID_THREADS, MID_SMEM));
-            if (occ < 1) occ = 1;
-            if (!h_mp.empty()) {                                  // a shard may own no tile pair of a small problem
+            if (n_mid && !h_mp.empty()) {                         // a shard may own no tile pair of a small problem
+                MidParams M{};
+                M.pairs = mpairs; M.n_pairs = (uint32_t)h_mp.size(); M.counter = reinterpret_cast<unsigned int*>(work + 7);
+                M.n_mid = n_mid; M.off = ML.off; M.tbase = ML.tbase; M.pk = pk; M.cut = sk_cut;
+                M.n_samples = N; M.out = reinterpret_cast<float*>(out); M.inv_qscale = inv_qscale;
+                CU(cudaFuncSetAttribute(k_mid, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MID_SMEM));
+                int occ = 0;
+                CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_mid, MID_THREADS, MID_SMEM));
+                if (occ < 1) occ = 1;
                 k_mid<<<(unsigned)std::min<long long>((long long)n_sm2 * occ, (long long)h_mp.size()), MID_THREADS, MID_SMEM, st>>>(M);
+                CU_LAUNCH(); ++launches; ++mid_launches;
+            }
+            if (n_g && n_all_pairs) {
+                MidgParams M{};
+                M.pairs = gpairs; M.n_pairs = (uint32_t)n_all_pairs; M.counter = reinterpret_cast<unsigned int*>(work + 25);
+                M.n_g = n_g; M.off = GLs.off; M.tbase = GLs.tbase; M.ex = gex; M.eq = reinterpret_cast<const uint4*>(geq);
+                M.n_samples = N; M.out = reinterpret_cast<float*>(out); M.inv_qscale = inv_qscale;
+                CU(cudaFuncSetAttribute(k_midg, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MID_SMEM));
+                int occ = 0;
+                CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_midg, MIDG_THREADS, MID_SMEM));
+                if (occ < 1) occ = 1;
+                k_midg<<<(unsigned)std::min<long long>((long long)n_sm2 * occ, (long long)n_all_pairs), MIDG_THREADS, MID_SMEM, st>>>(M);
                 CU_LAUNCH(); ++launches; ++mid_launches;
             }
         }
@@ -960,6 +1042,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     g_stats.embed_rows = embed_rows;
     g_stats.head_rows = head_rows; g_stats.tail_rows = tail_rows; g_stats.tail_updates = tail_updates; g_stats.tail_entries = tail_entries;
     g_stats.tail_launches = tail_launches;
+    g_stats.mid_groups = midg_groups; g_stats.mid_group_rows = midg_rows;
     g_stats.mid_rows = mid_rows; g_stats.mid_updates = mid_updates; g_stats.mid_launches = mid_launches; g_stats.mid_F = (uint32_t)mid_F;
     g_stats.skip = skip_on ? 1u : 0u; g_stats.skip_rows = sk_KE; g_stats.list_rows = sk_n;
     if (skip_on) { g_stats.mid_updates = h_skstat[0]; g_stats.skip_row_pair_visits = h_skstat[1]; g_stats.skip_updates_executed = h_skstat[1] * 16384ull; g_stats.mid_rows = sk_n; g_stats.head_rows = sk_KE; }
