@@ -74,7 +74,8 @@ k_mid_seg(uint32_t n_mid, const int32_t* __restrict__ mrows, const uint32_t* __r
 // off[t][n_mid] = ttot[t] = number of packed entries of tile t.  One CTA per tile (exclusive scan over rows).
 __global__ void __launch_bounds__(1024)
 k_mid_off(uint32_t n_mid, const uint32_t* __restrict__ seg, uint32_t* __restrict__ off, uint32_t* __restrict__ ttot,
-          const uint32_t* __restrict__ cut /* rows r < cut[0] are never joined (zone.cuh), or NULL */)
+          const uint32_t* __restrict__ cut /* rows r < cut[0] are never joined (zone.cuh), or NULL */,
+          uint32_t pad /* every (row, tile) list is padded to a multiple of this power of two: 2 (k_mid), 4 (k_midg) */)
 {
     __shared__ uint32_t part[1024];
     const uint32_t t = blockIdx.x;
@@ -83,7 +84,7 @@ k_mid_off(uint32_t n_mid, const uint32_t* __restrict__ seg, uint32_t* __restrict
     uint32_t* o = off + (size_t)t * (n_mid + 1);
     const int th = threadIdx.x;
     const uint32_t r0 = cut ? cut[0] : 0u;       // rows below cut[0] are in the dense zone of every tile
-    auto cnt = [&](uint32_t r) { return r >= r0 ? ((s1[r] - s0[r] + 1u) & ~1u) : 0u; };   // every (row, tile) list padded to an even length
+    auto cnt = [&](uint32_t r) { return r >= r0 ? ((s1[r] - s0[r] + pad - 1u) & ~(pad - 1u)) : 0u; };
     const uint32_t chunk = (n_mid + 1023u) / 1024u;
     uint32_t lo = th * chunk, hi = lo + chunk;
     if (lo > n_mid) lo = n_mid;

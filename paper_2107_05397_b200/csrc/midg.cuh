@@ -22,9 +22,10 @@
 
 namespace ufb {
 
-constexpr int MIDG_L = 4;
+constexpr int MIDG_L = 4;            // members per group = fixed-point values per position (one uint4)
+constexpr int MIDG_R = 2;            // I positions per lane of k_midg; every (group, tile) list is padded to a multiple of it
 constexpr uint8_t CLS_MIDG_ROOT = 4, CLS_MIDG_MEMBER = 5;
-constexpr int MIDG_THREADS = 384;
+constexpr int MIDG_THREADS = 384;       // x 3 CTAs per SM: 56 registers per thread
 constexpr int MIDG_MINB = 3;
 
 // children of the internal nodes of one tree level: groot[c] = root of c's group, gslot[c] = its slot, gcnt[r] = members so far
@@ -115,7 +116,8 @@ k_midg_pack_roots(uint32_t n_g, const uint32_t* __restrict__ gbase, const uint32
         const uint32_t x = (g << 9) | ((s & 127u) << 2);
         ex[pos] = x;
         eq[(size_t)pos * MIDG_L] = midg_quant(tv[base + k], s, qscale, inv_qscale, sums, qerr);
-        if (k + 1 == g1 && ((g1 - g0) & 1u)) ex[pos + 1] = x;
+        if (k + 1 == g1)                                          // padding positions: a valid cell, values 0 (memset)
+            for (uint32_t f = g1 - g0; f & (MIDG_R - 1); ++f) ex[pos + 1 + (f - (g1 - g0))] = x;
     }
 }
 
@@ -163,7 +165,10 @@ __device__ __forceinline__ uint32_t midg_dot(const uint4& a, const uint4& b) {
 }
 
 // The grouped join: every position (group g, sample a, values qa[]) of tile I meets the positions (g, b, qb[]) of the same
-// group in tile J; one lane per I position, chunks of 32 consecutive I positions per warp, software pipelined like k_mid.
+// group in tile J.  A lane owns MIDG_R = 4 consecutive I positions (same group: the lists are padded to multiples of 4), a warp
+// a chunk of 128; every J position a lane loads (20 bytes: cell + 4 values) feeds 4 atomics.  That ratio is the point: a
+// warp-wide 16-byte load occupies the L1 data pipe for 4 cycles whether or not the lanes read the same address, and with
+// one I position per lane those loads, not the atomics, bounded the kernel (ncu: data pipe 94 %, of it atomics 31 %).
 __global__ void __launch_bounds__(MIDG_THREADS, MIDG_MINB)
 k_midg(const MidgParams P)
 {
@@ -188,39 +193,57 @@ k_midg(const MidgParams P)
         const int2 ij = P.pairs[pi];
         const uint32_t eI0 = P.tbase[ij.x], eI1 = P.tbase[ij.x + 1], eJ0 = P.tbase[ij.y];
         const uint32_t* offJ = P.off + (size_t)ij.y * pitch;
-        const uint32_t nchunk = (eI1 - eI0 + 31u) >> 5;
+        const uint32_t nchunk = (eI1 - eI0 + 32u * MIDG_R - 1u) / (32u * MIDG_R);
 
-        // pipeline: stage B = position + J range of chunk c+1, stage C = current
-        uint32_t xB = 0, xC; uint4 qB = make_uint4(0u, 0u, 0u, 0u), qC;
+        // one chunk ahead: the cells of the lane and the J range of their group
+        uint32_t xB[MIDG_R], xC[MIDG_R];
         uint32_t jB0 = 0, jB1 = 0, jC0, jC1;
-        auto load_pos = [&](uint32_t c, uint32_t& x, uint4& q, uint32_t& j0, uint32_t& j1) {
-            const uint32_t e = eI0 + c * 32u + lane;
-            j0 = j1 = 0; x = 0; q = make_uint4(0u, 0u, 0u, 0u);
+        auto load_pos = [&](uint32_t c, uint32_t (&x)[MIDG_R], uint32_t& j0, uint32_t& j1) {
+            const uint32_t e = eI0 + (c * 32u + lane) * MIDG_R;
+            j0 = j1 = 0;
+#pragma unroll
+            for (int k = 0; k < MIDG_R; ++k) x[k] = 0u;
             if (c < nchunk && e < eI1) {
-                x = __ldg(ex + e); q = __ldg(eq + e);
-                if (q.x | q.y | q.z | q.w) {                 // all-zero (padding) positions contribute nothing
-                    const uint32_t g = x >> 9;
-                    j0 = eJ0 + offJ[g];                      // both even
-                    j1 = eJ0 + offJ[g + 1];
-                }
+                if (MIDG_R == 4) { const uint4 t = __ldg(reinterpret_cast<const uint4*>(ex + e)); x[0] = t.x; x[1] = t.y; x[MIDG_R - 2] = t.z; x[MIDG_R - 1] = t.w; }
+                else { const uint2 t = __ldg(reinterpret_cast<const uint2*>(ex + e)); x[0] = t.x; x[1] = t.y; }
+                const uint32_t g = x[0] >> 9;
+                j0 = eJ0 + offJ[g];                          // multiples of MIDG_R
+                j1 = eJ0 + offJ[g + 1];
             }
         };
         uint32_t c = warp;
-        load_pos(c, xB, qB, jB0, jB1);
+        load_pos(c, xB, jB0, jB1);
         for (; c < nchunk; c += NWARP) {
-            xC = xB; qC = qB; jC0 = jB0; jC1 = jB1;
-            load_pos(c + NWARP, xB, qB, jB0, jB1);
-            const uint32_t a4 = xC & 0x1fcu;                                      // 4 a
-            const uint32_t arow = (macc_s + (a4 << 7)) | (a4 & 0x7cu);            // row base | (a & 31) << 2
-            uint32_t l = jC0;
-            while (__any_sync(0xffffffffu, l < jC1)) {
+#pragma unroll
+            for (int k = 0; k < MIDG_R; ++k) xC[k] = xB[k];
+            jC0 = jB0; jC1 = jB1;
+            const uint32_t e = eI0 + (c * 32u + lane) * MIDG_R;
+            uint4 q[MIDG_R];
+            uint32_t row[MIDG_R];
+#pragma unroll
+            for (int k = 0; k < MIDG_R; ++k) {
+                q[k] = make_uint4(0u, 0u, 0u, 0u);
+                if (jC0 < jC1) q[k] = __ldg(eq + e + k);
+                const uint32_t a4 = xC[k] & 0x1fcu;
+                row[k] = (macc_s + (a4 << 7)) | (a4 & 0x7cu);              // row base | (a & 31) << 2
+            }
+            load_pos(c + NWARP, xB, jB0, jB1);
+            // 4 J positions per iteration (two independent pairs of loads in flight)
+            for (uint32_t l = jC0; __any_sync(0xffffffffu, l < jC1); l += 4) {
                 const bool p0 = l < jC1, p1 = l + 2u < jC1;
-                uint2 x0, x1; uint4 b0, b1, b2, b3;
-                if (p0) { x0 = __ldg(reinterpret_cast<const uint2*>(ex + l)); b0 = __ldg(eq + l); b1 = __ldg(eq + l + 1); }
-                if (p1) { x1 = __ldg(reinterpret_cast<const uint2*>(ex + l + 2)); b2 = __ldg(eq + l + 2); b3 = __ldg(eq + l + 3); }
-                if (p0) { mid_red(arow ^ (x0.x & 0x1fcu), midg_dot(qC, b0)); mid_red(arow ^ (x0.y & 0x1fcu), midg_dot(qC, b1)); }
-                if (p1) { mid_red(arow ^ (x1.x & 0x1fcu), midg_dot(qC, b2)); mid_red(arow ^ (x1.y & 0x1fcu), midg_dot(qC, b3)); }
-                l += 4;
+                uint2 xa, xb; uint4 b0, b1, b2, b3;
+                if (p0) { xa = __ldg(reinterpret_cast<const uint2*>(ex + l)); b0 = __ldg(eq + l); b1 = __ldg(eq + l + 1); }
+                if (p1) { xb = __ldg(reinterpret_cast<const uint2*>(ex + l + 2)); b2 = __ldg(eq + l + 2); b3 = __ldg(eq + l + 3); }
+                if (p0) {
+                    const uint32_t c0 = xa.x & 0x1fcu, c1 = xa.y & 0x1fcu;
+#pragma unroll
+                    for (int k = 0; k < MIDG_R; ++k) { mid_red(row[k] ^ c0, midg_dot(q[k], b0)); mid_red(row[k] ^ c1, midg_dot(q[k], b1)); }
+                }
+                if (p1) {
+                    const uint32_t c0 = xb.x & 0x1fcu, c1 = xb.y & 0x1fcu;
+#pragma unroll
+                    for (int k = 0; k < MIDG_R; ++k) { mid_red(row[k] ^ c0, midg_dot(q[k], b2)); mid_red(row[k] ^ c1, midg_dot(q[k], b3)); }
+                }
             }
         }
         __syncthreads();

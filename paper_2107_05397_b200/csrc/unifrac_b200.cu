@@ -704,7 +704,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
                 unsigned long long* gc = A.get_n<unsigned long long>(4);
                 CU(cudaMemsetAsync(gcnt, 0, sizeof(uint32_t) * n, st));
                 CU(cudaMemsetAsync(gc, 0, sizeof(unsigned long long) * 4, st));
-                const uint32_t theta_256 = (uint32_t)std::lround(256.0 * envd("UNIFRAC_B200_MID_GROUP_THETA", 0.5));
+                const uint32_t theta_256 = (uint32_t)std::lround(256.0 * envd("UNIFRAC_B200_MID_GROUP_THETA", 0.35));
                 for (int d = 0; d < n_levels; ++d)
                     if (h_hist[d]) {
                         k_midg_level<<<cdiv(h_hist[d], TB), TB, 0, st>>>(h_hist[d], level_nodes + h_off[d], child_off, child_idx, cls, nv,
@@ -733,23 +733,23 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             };
             // tile-major offsets of the rows' (row, tile) lists
             struct TileLists { uint32_t* seg; uint32_t* off; uint32_t* tbase; };
-            auto tile_lists = [&](uint32_t count, const int32_t* rows, const uint32_t* cut) {
+            auto tile_lists = [&](uint32_t count, const int32_t* rows, const uint32_t* cut, uint32_t pad) {
                 TileLists L{};
                 L.seg = A.get_n<uint32_t>((size_t)(n_tiles + 1) * std::max<uint32_t>(count, 1u));
                 L.off = A.get_n<uint32_t>((size_t)n_tiles * ((size_t)count + 1));
                 uint32_t* ttot = A.get_n<uint32_t>(n_tiles);
                 L.tbase = A.get_n<uint32_t>((size_t)n_tiles + 1);
                 if (count) { k_mid_seg<<<cdiv((long long)count * 32, TB), TB, 0, st>>>(count, rows, tptr, ts, n_tiles, L.seg); CU_LAUNCH(); ++launches; }
-                k_mid_off<<<n_tiles, 1024, 0, st>>>(count, L.seg, L.off, ttot, cut); CU_LAUNCH(); ++launches;
+                k_mid_off<<<n_tiles, 1024, 0, st>>>(count, L.seg, L.off, ttot, cut, pad); CU_LAUNCH(); ++launches;
                 k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>(n_tiles, ttot, L.tbase); CU_LAUNCH(); ++launches;
                 return L;
             };
             int32_t* mrows = sk_rows; uint32_t* mbase = sk_base; uint32_t* mlen = sk_len;
             if (!skip_on) class_rows(CLS_MID, n_mid, mrows, mbase, mlen);
-            const TileLists ML = tile_lists(n_mid, mrows, sk_cut);
+            const TileLists ML = tile_lists(n_mid, mrows, sk_cut, 2u);
             int32_t* grows = nullptr; uint32_t* gbase = nullptr; uint32_t* glen = nullptr;
             TileLists GLs{};
-            if (n_g) { class_rows(CLS_MIDG_ROOT, n_g, grows, gbase, glen); GLs = tile_lists(n_g, grows, nullptr); }
+            if (n_g) { class_rows(CLS_MIDG_ROOT, n_g, grows, gbase, glen); GLs = tile_lists(n_g, grows, nullptr, (uint32_t)MIDG_R); }
             unsigned long long* smax = work + 15;
             double* midsum = A.get_n<double>((size_t)n_tiles * TILE);
             CU(cudaMemsetAsync(midsum, 0, sizeof(double) * (size_t)n_tiles * TILE, st));
@@ -786,11 +786,11 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             uint32_t* gex = nullptr; uint32_t* geq = nullptr;
             unsigned long long* gmiss = work + 24;
             if (n_g) {
-                gex = A.get_n<uint32_t>((size_t)h_g_total + 2);
-                geq = A.get_n<uint32_t>(((size_t)h_g_total + 2) * MIDG_L);
+                gex = A.get_n<uint32_t>((size_t)h_g_total + 4);
+                geq = A.get_n<uint32_t>(((size_t)h_g_total + 4) * MIDG_L);
                 int32_t* rootidx = A.get_n<int32_t>(n);
-                CU(cudaMemsetAsync(gex, 0, sizeof(uint32_t) * ((size_t)h_g_total + 2), st));
-                CU(cudaMemsetAsync(geq, 0, sizeof(uint32_t) * ((size_t)h_g_total + 2) * MIDG_L, st));
+                CU(cudaMemsetAsync(gex, 0, sizeof(uint32_t) * ((size_t)h_g_total + 4), st));
+                CU(cudaMemsetAsync(geq, 0, sizeof(uint32_t) * ((size_t)h_g_total + 4) * MIDG_L, st));
                 k_midg_index<<<cdiv(n_g, TB), TB, 0, st>>>(n_g, grows, rootidx); CU_LAUNCH(); ++launches;
                 k_midg_pack_roots<<<cdiv((long long)n_g * 32, TB), TB, 0, st>>>(n_g, gbase, glen, ts, reinterpret_cast<const float*>(tv), GLs.seg, GLs.off,
                                                                                GLs.tbase, qscale, inv_qscale, sums, qerr, gex, geq); CU_LAUNCH(); ++launches;
