@@ -172,6 +172,79 @@ __device__ __forceinline__ void mid_red(uint32_t addr, uint32_t v) {
     asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
 }
 
+// the join of one tile pair into the CTA's accumulators (macc_s = shared-memory address of row 0); NWARP warps take the chunks
+template <int NWARP>
+__device__ __forceinline__ void mid_join_pair(const MidParams& P, const int2 ij, const uint32_t macc_s, const int warp, const int lane)
+{
+    const size_t pitch = (size_t)P.n_mid + 1;
+    const uint2* __restrict__ pk = P.pk;
+    const uint32_t eI1 = P.tbase[ij.x + 1], eJ0 = P.tbase[ij.y];
+    const uint32_t eI0 = P.tbase[ij.x] + (P.cut ? P.off[(size_t)ij.x * pitch + P.cut[ij.x]] : 0u);
+    const uint32_t* offJ = P.off + (size_t)ij.y * pitch;
+    const uint32_t nchunk = (eI1 - eI0 + 31u) >> 5;
+
+    // pipeline registers: stage A = entry of chunk c+2, stage B = entry + J range of chunk c+1, stage C = current
+    uint2 entA = make_uint2(0u, 0u), entB = make_uint2(0u, 0u), entC;
+    uint32_t jB0 = 0, jB1 = 0, jC0, jC1;
+    bool vA = false, vB = false;
+    auto load_ent = [&](uint32_t c, uint2& ent, bool& valid) {
+        const uint32_t e = eI0 + c * 32u + lane;
+        valid = c < nchunk && e < eI1;
+        if (valid) ent = __ldg(pk + e);
+    };
+    auto load_range = [&](const uint2& ent, bool valid, uint32_t& j0, uint32_t& j1) {
+        j0 = j1 = 0;
+        if (valid && ent.y != 0u) {                      // q = 0 (padding entries) contributes nothing
+            const uint32_t r = ent.x >> 9;
+            j0 = eJ0 + offJ[r];                          // both even: 16-byte aligned pairs of entries
+            j1 = eJ0 + offJ[r + 1];
+        }
+    };
+    // The diagonal tile pair (I == J) walks the row's full list as well: cells with a >= b receive sums that the
+    // epilogue never reads (it keeps gi < gj only).
+    uint32_t c = warp;
+    load_ent(c, entB, vB);
+    load_range(entB, vB, jB0, jB1);
+    load_ent(c + NWARP, entA, vA);
+    for (; c < nchunk; c += NWARP) {
+        entC = entB; jC0 = jB0; jC1 = jB1;
+        entB = entA; vB = vA;
+        load_range(entB, vB, jB0, jB1);
+        load_ent(c + 2 * NWARP, entA, vA);
+        const uint32_t a4 = entC.x & 0x1fcu;                                  // 4 a
+        const uint32_t arow = (macc_s + (a4 << 7)) | (a4 & 0x7cu);            // row base | (a & 31) << 2
+        const uint32_t qa = entC.y;
+        uint32_t l = jC0;
+        while (__any_sync(0xffffffffu, l < jC1)) {
+            uint4 f0, f1;
+            const bool p0 = l < jC1, p1 = l + 2u < jC1;
+            if (p0) f0 = __ldg(reinterpret_cast<const uint4*>(pk + l));
+            if (p1) f1 = __ldg(reinterpret_cast<const uint4*>(pk + l + 2));
+            if (p0) { mid_red(arow ^ (f0.x & 0x1fcu), min(qa, f0.y)); mid_red(arow ^ (f0.z & 0x1fcu), min(qa, f0.w)); }
+            if (p1) { mid_red(arow ^ (f1.x & 0x1fcu), min(qa, f1.y)); mid_red(arow ^ (f1.z & 0x1fcu), min(qa, f1.w)); }
+            l += 4;
+        }
+    }
+}
+
+// epilogue of a tile pair: add its fixed-point sums to the condensed matrix (exclusive owner; the tail REDs ran before)
+template <int NTHREADS>
+__device__ __forceinline__ void mid_epilogue(const uint32_t* macc, const int2 ij, const long long N, float* __restrict__ out, const double inv_qscale)
+{
+    const uint32_t sI = (uint32_t)ij.x * TILE, sJ = (uint32_t)ij.y * TILE;
+    for (int e = threadIdx.x; e < TILE * TILE; e += NTHREADS) {
+        const int a = e >> 7, b = (e & 127) ^ (a & 31);
+        const uint32_t q = macc[e];
+        if (q) {
+            const long long gi = (long long)sI + a, gj = (long long)sJ + b;
+            if (gi < gj && gj < N) {
+                float* o = out + (gi * (2 * N - gi - 1) / 2 - gi - 1 + gj);
+                *o = (float)((double)*o + (double)q * inv_qscale);
+            }
+        }
+    }
+}
+
 __global__ void __launch_bounds__(MID_THREADS, MID_MINB)
 k_mid(const MidParams P)
 {
@@ -181,11 +254,6 @@ k_mid(const MidParams P)
     const uint32_t macc_s = (raw_s + 511u) & ~511u;                    // 512-byte aligned rows: row a at macc_s + 512 a
     uint32_t* macc = macc_raw + ((macc_s - raw_s) >> 2);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    constexpr int NWARP = MID_THREADS / 32;
-    const long long N = P.n_samples;
-    const size_t pitch = (size_t)P.n_mid + 1;
-    const uint2* __restrict__ pk = P.pk;
-
     for (;;) {
         if (threadIdx.x == 0) s_pair = (int)atomicAdd(P.counter, 1u);
         for (int i = threadIdx.x; i < TILE * TILE; i += MID_THREADS) macc[i] = 0u;
@@ -193,67 +261,9 @@ k_mid(const MidParams P)
         const int pi = s_pair;
         if ((uint32_t)pi >= P.n_pairs) break;
         const int2 ij = P.pairs[pi];
-        const uint32_t eI1 = P.tbase[ij.x + 1], eJ0 = P.tbase[ij.y];
-        const uint32_t eI0 = P.tbase[ij.x] + (P.cut ? P.off[(size_t)ij.x * pitch + P.cut[ij.x]] : 0u);
-        const uint32_t* offJ = P.off + (size_t)ij.y * pitch;
-        const uint32_t nchunk = (eI1 - eI0 + 31u) >> 5;
-
-        // pipeline registers: stage A = entry of chunk c+2, stage B = entry + J range of chunk c+1, stage C = current
-        uint2 entA = make_uint2(0u, 0u), entB = make_uint2(0u, 0u), entC;
-        uint32_t jB0 = 0, jB1 = 0, jC0, jC1;
-        bool vA = false, vB = false;
-        auto load_ent = [&](uint32_t c, uint2& ent, bool& valid) {
-            const uint32_t e = eI0 + c * 32u + lane;
-            valid = c < nchunk && e < eI1;
-            if (valid) ent = __ldg(pk + e);
-        };
-        auto load_range = [&](const uint2& ent, bool valid, uint32_t& j0, uint32_t& j1) {
-            j0 = j1 = 0;
-            if (valid && ent.y != 0u) {                      // q = 0 (padding entries) contributes nothing
-                const uint32_t r = ent.x >> 9;
-                j0 = eJ0 + offJ[r];                          // both even: 16-byte aligned pairs of entries
-                j1 = eJ0 + offJ[r + 1];
-            }
-        };
-        // The diagonal tile pair (I == J) walks the row's full list as well: cells with a >= b receive sums that the
-        // epilogue never reads (it keeps gi < gj only).
-        uint32_t c = warp;
-        load_ent(c, entB, vB);
-        load_range(entB, vB, jB0, jB1);
-        load_ent(c + NWARP, entA, vA);
-        for (; c < nchunk; c += NWARP) {
-            entC = entB; jC0 = jB0; jC1 = jB1;
-            entB = entA; vB = vA;
-            load_range(entB, vB, jB0, jB1);
-            load_ent(c + 2 * NWARP, entA, vA);
-            const uint32_t a4 = entC.x & 0x1fcu;                                  // 4 a
-            const uint32_t arow = (macc_s + (a4 << 7)) | (a4 & 0x7cu);            // row base | (a & 31) << 2
-            const uint32_t qa = entC.y;
-            uint32_t l = jC0;
-            while (__any_sync(0xffffffffu, l < jC1)) {
-                uint4 f0, f1;
-                const bool p0 = l < jC1, p1 = l + 2u < jC1;
-                if (p0) f0 = __ldg(reinterpret_cast<const uint4*>(pk + l));
-                if (p1) f1 = __ldg(reinterpret_cast<const uint4*>(pk + l + 2));
-                if (p0) { mid_red(arow ^ (f0.x & 0x1fcu), min(qa, f0.y)); mid_red(arow ^ (f0.z & 0x1fcu), min(qa, f0.w)); }
-                if (p1) { mid_red(arow ^ (f1.x & 0x1fcu), min(qa, f1.y)); mid_red(arow ^ (f1.z & 0x1fcu), min(qa, f1.w)); }
-                l += 4;
-            }
-        }
+        mid_join_pair<MID_THREADS / 32>(P, ij, macc_s, warp, lane);
         __syncthreads();
-        // ---- epilogue: add the tile pair's fixed-point sums to the condensed matrix (exclusive owner)
-        const uint32_t sI = (uint32_t)ij.x * TILE, sJ = (uint32_t)ij.y * TILE;
-        for (int e = threadIdx.x; e < TILE * TILE; e += MID_THREADS) {
-            const int a = e >> 7, b = (e & 127) ^ (a & 31);
-            const uint32_t q = macc[e];
-            if (q) {
-                const long long gi = (long long)sI + a, gj = (long long)sJ + b;
-                if (gi < gj && gj < N) {
-                    float* o = P.out + (gi * (2 * N - gi - 1) / 2 - gi - 1 + gj);
-                    *o = (float)((double)*o + (double)q * P.inv_qscale);
-                }
-            }
-        }
+        mid_epilogue<MID_THREADS>(macc, ij, P.n_samples, P.out, P.inv_qscale);
         __syncthreads();
     }
 }

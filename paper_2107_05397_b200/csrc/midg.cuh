@@ -158,6 +158,7 @@ struct MidgParams {
     int n_samples;
     float* out;
     double inv_qscale;            // 2^-F
+    MidParams rows;               // the mid rows that stayed alone: joined by the same CTA into the same accumulators (n_mid = 0: none)
 };
 
 __device__ __forceinline__ uint32_t midg_dot(const uint4& a, const uint4& b) {
@@ -191,6 +192,9 @@ k_midg(const MidgParams P)
         const int pi = s_pair;
         if ((uint32_t)pi >= P.n_pairs) break;
         const int2 ij = P.pairs[pi];
+        // the rows that are in no group first, into the same integer accumulators: one conversion to fp32 per pair, and a
+        // result that does not depend on which rows the grouping picked (integer sums are exact)
+        if (P.rows.n_mid) mid_join_pair<NWARP>(P.rows, ij, macc_s, warp, lane);
         const uint32_t eI0 = P.tbase[ij.x], eI1 = P.tbase[ij.x + 1], eJ0 = P.tbase[ij.y];
         const uint32_t* offJ = P.off + (size_t)ij.y * pitch;
         const uint32_t nchunk = (eI1 - eI0 + 32u * MIDG_R - 1u) / (32u * MIDG_R);
@@ -247,19 +251,7 @@ k_midg(const MidgParams P)
             }
         }
         __syncthreads();
-        // ---- epilogue: add the tile pair's fixed-point sums to the condensed matrix (exclusive owner, after k_mid's)
-        const uint32_t sI = (uint32_t)ij.x * TILE, sJ = (uint32_t)ij.y * TILE;
-        for (int e = threadIdx.x; e < TILE * TILE; e += MIDG_THREADS) {
-            const int a = e >> 7, b = (e & 127) ^ (a & 31);
-            const uint32_t q = macc[e];
-            if (q) {
-                const long long gi = (long long)sI + a, gj = (long long)sJ + b;
-                if (gi < gj && gj < N) {
-                    float* o = P.out + (gi * (2 * N - gi - 1) / 2 - gi - 1 + gj);
-                    *o = (float)((double)*o + (double)q * P.inv_qscale);
-                }
-            }
-        }
+        mid_epilogue<MIDG_THREADS>(macc, ij, N, P.out, P.inv_qscale);
         __syncthreads();
     }
 }

@@ -394,11 +394,13 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     // (shared-memory atomics, L2 REDs, the FMNMX + FADD mix) are probed (unifrac_measure_rates, ~20 ms) and the kernel rates
     // are scaled by measured / reference, in steps of 1/4 so that probe noise cannot move the split (on a B200: all 1.0).
     const Calib cal = calibration(dev_id, st);
-    const double R_tail = envd("UNIFRAC_B200_R_TAIL", 1.6e11 * cal.f_red), R_mid = envd("UNIFRAC_B200_R_MID", 1.6e12 * cal.f_atom);
+    // with the grouped join (midg.cuh) a mid update costs about half of what it costs in k_mid alone (sweeps: profiles/r02_summary.md 4d)
+    const bool groups_expected = std::is_same<T, float>::value && !skip_path && envd("UNIFRAC_B200_MID_GROUPS", 1.0) != 0.0;
+    const double R_tail = envd("UNIFRAC_B200_R_TAIL", 1.6e11 * cal.f_red), R_mid = envd("UNIFRAC_B200_R_MID", (groups_expected ? 3.5e12 : 1.6e12) * cal.f_atom);
     const double R_head = envd("UNIFRAC_B200_R_HEAD", (std::is_same<T, float>::value ? 1.4e13 : 3.3e12) * cal.f_alu), gram_Bps = envd("UNIFRAC_B200_GRAM_BPS", 1.15e13);
     // the rows that compete with the Gram kernel are sparse (a few entries per tile), where k_mid's per-entry overhead
     // halves its update rate (measured 5.9e11 /s at Large against 1.3e12 - 1.6e12 /s for the denser rows of the weighted variant)
-    const double R_mid_head = gram ? envd("UNIFRAC_B200_R_MID_SPARSE", 5.5e11 * cal.f_atom) : R_mid;
+    const double R_mid_head = gram ? envd("UNIFRAC_B200_R_MID_SPARSE", (groups_expected ? 8e11 : 5.5e11) * cal.f_atom) : R_mid;
     const double c_ent = envd("UNIFRAC_B200_MID_ENT_S", 3e-12);         // seconds per (mid entry, tile pair) visit of the join kernel
     const double head_s = gram ? n_tp * 512.0 / gram_Bps : Pd / R_head;  // seconds per head branch
     double c2_head, c2_mid;
@@ -808,16 +810,16 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             int dev2 = 0, n_sm2 = 0;
             CU(cudaGetDevice(&dev2));
             CU(cudaDeviceGetAttribute(&n_sm2, cudaDevAttrMultiProcessorCount, dev2));
-            if (n_mid && !h_mp.empty()) {                         // a shard may own no tile pair of a small problem
-                MidParams M{};
-                M.pairs = mpairs; M.n_pairs = (uint32_t)h_mp.size(); M.counter = reinterpret_cast<unsigned int*>(work + 7);
-                M.n_mid = n_mid; M.off = ML.off; M.tbase = ML.tbase; M.pk = pk; M.cut = sk_cut;
-                M.n_samples = N; M.out = reinterpret_cast<float*>(out); M.inv_qscale = inv_qscale;
+            MidParams MP{};
+            MP.pairs = mpairs; MP.n_pairs = (uint32_t)h_mp.size(); MP.counter = reinterpret_cast<unsigned int*>(work + 7);
+            MP.n_mid = n_mid; MP.off = ML.off; MP.tbase = ML.tbase; MP.pk = pk; MP.cut = sk_cut;
+            MP.n_samples = N; MP.out = reinterpret_cast<float*>(out); MP.inv_qscale = inv_qscale;
+            if (!n_g && n_mid && !h_mp.empty()) {                 // a shard may own no tile pair of a small problem
                 CU(cudaFuncSetAttribute(k_mid, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MID_SMEM));
                 int occ = 0;
                 CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_mid, MID_THREADS, MID_SMEM));
                 if (occ < 1) occ = 1;
-                k_mid<<<(unsigned)std::min<long long>((long long)n_sm2 * occ, (long long)h_mp.size()), MID_THREADS, MID_SMEM, st>>>(M);
+                k_mid<<<(unsigned)std::min<long long>((long long)n_sm2 * occ, (long long)h_mp.size()), MID_THREADS, MID_SMEM, st>>>(MP);
                 CU_LAUNCH(); ++launches; ++mid_launches;
             }
             if (n_g && n_all_pairs) {
@@ -825,6 +827,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
                 M.pairs = gpairs; M.n_pairs = (uint32_t)n_all_pairs; M.counter = reinterpret_cast<unsigned int*>(work + 25);
                 M.n_g = n_g; M.off = GLs.off; M.tbase = GLs.tbase; M.ex = gex; M.eq = reinterpret_cast<const uint4*>(geq);
                 M.n_samples = N; M.out = reinterpret_cast<float*>(out); M.inv_qscale = inv_qscale;
+                M.rows = MP;                                      // (groups are off in the zones path: MP.cut = NULL here)
                 CU(cudaFuncSetAttribute(k_midg, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MID_SMEM));
                 int occ = 0;
                 CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_midg, MIDG_THREADS, MID_SMEM));
