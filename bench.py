@@ -40,10 +40,11 @@ ALU_PEAK_TFLOPS = SM_COUNT * FP32_LANES * SM_MAX_GHZ / 1e3    # FADD/FMNMX-class
 SMEM_ATOMIC_PER_S, L2_RED_PER_S = 8.84 * SM_COUNT * SM_MAX_GHZ * 1e9, 1.94e11
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch, copied from the ncu --set full captures summarised in the file
-# TRAFFIC_SOURCE names (default flags, seed 0; k_mid: mean of the unweighted and the weighted launch); not measured by this
+# TRAFFIC_SOURCE names (default flags, seed 0; k_midg / k_mid: mean of the unweighted and the weighted launch; k_mid and k_zone:
+# the earlier captures of section 2, for runs with UNIFRAC_B200_MID_GROUPS=0 / --flags 512); not measured by this
 # run -- other workloads and kernels that changed since the capture report null
-TRAFFIC_SOURCE = "profiles/r02_summary.md (ncu --set full captures of this round's kernels, Large, seed 0)"
-NCU_TRAFFIC_BYTES = {"large": {"k_dense16": 225.3e9, "k_gram": 300.1e9, "k_mid": 240.1e9, "k_zone": 307.1e9}}
+TRAFFIC_SOURCE = "profiles/r02_summary.md section 0 (ncu --set full captures of the final kernels of the round, Large, seed 0)"
+NCU_TRAFFIC_BYTES = {"large": {"k_dense16": 80.5e9, "k_gram": 260.8e9, "k_midg": 223.9e9, "k_mid": 240.1e9, "k_zone": 307.1e9}}
 
 WORKLOADS = {   # name -> (variants, precision)    BASELINE.json:7-11
     "tiny": ((0, 1), 1), "small": ((0, 1), 1), "medium": ((0,), 0), "emp": ((0, 1), 0), "large": ((0, 1), 0),
@@ -162,6 +163,7 @@ def wall_of(all_stats, variants, n_nodes, nnz):
             updates_executed_per_s=(s0["updates_executed"] / t_a5) if t_a5 > 0 else None,
             embed_gbs=(embed_bytes / (mean("ms_embed") * 1e-3) / 1e9) if mean("ms_embed") > 0 else None,
             mid_rows=s0["mid_rows"], mid_updates=s0["mid_updates"], mid_F=s0["mid_F"],
+            mid_groups=s0["mid_groups"], mid_group_rows=s0["mid_group_rows"], mid_atomics=s0["mid_atomics"],
             head_rows=s0["head_rows"], tail_rows=s0["tail_rows"], tail_updates=s0["tail_updates"],
             gram=s0["gram"], gram_k=s0["gram_k"], gram_q=s0["gram_q"], guard_pairs=s0["guard_pairs"],
             skip=s0["skip"], skip_rows=s0["skip_rows"], list_rows=s0["list_rows"], skip_row_pair_visits=s0["skip_row_pair_visits"],
@@ -468,19 +470,27 @@ def main():
                        frac=reds / t / RED_PEAK if t > 0 else 0.0, traffic=None, kernel="k_tail_scatter", launches=nl,
                        ms_per_launch=1e3 * t / max(1, nl), seconds=t, share_of_step=t / step_s,
                        peak_source=f"scattered RED.ADD.F32 into a 48 MB L2-resident footprint, {rates_src}"))
-    # (4) k_mid: tile-pair join with native shared-memory integer atomics (ATOMS.ADD), one per (pair, branch) update
+    # (4) the mid stage: tile-pair join with native shared-memory integer atomics (ATOMS.ADD).  k_mid: one atomic per
+    # (pair, branch) update; k_midg (grouped join, default): one atomic per pair of a group ROOT serves the update of every
+    # member, so the algorithmic update rate may pass the rate of the atomic unit
     t = sum(s["ms_mid"] for s in flat) * 1e-3
     mu = sum(s["mid_updates"] for s in flat)
+    ma = sum(s["mid_atomics"] for s in flat)
     nl = sum(s["mid_launches"] for s in flat)
+    grouped = any(s["mid_groups"] for s in flat)
     if nl:
         ATOMS_PEAK = rates["smem_atomic_random_per_s"]
         rl.append(dict(bound="smem_atomic", achieved=mu / t / 1e9 if t > 0 else 0.0, peak=ATOMS_PEAK / 1e9, unit="GATOM/s",
-                       frac=mu / t / ATOMS_PEAK if t > 0 else 0.0, traffic=None, kernel="k_mid", launches=nl,
+                       frac=mu / t / ATOMS_PEAK if t > 0 else 0.0, traffic=None, kernel="k_midg" if grouped else "k_mid", launches=nl,
                        ms_per_launch=1e3 * t / max(1, nl), seconds=t, share_of_step=t / step_s,
+                       updates_per_launch=mu / max(1, nl), atomics_executed_per_launch=ma / max(1, nl),
+                       frac_atomics_executed=(ma / t / ATOMS_PEAK) if t > 0 else 0.0,
                        frac_of_fp32_lane_roofline=(2.0 * mu / t / (ALU_PEAK_TFLOPS * 1e12)) if t > 0 else 0.0,
-                       note="ms_mid also covers the mid list preparation kernels (k_mid_seg/off/pack); frac_of_fp32_lane_roofline = "
-                            "2 lane-ops per update against the FP32-lane peak of SURVEY 8(d): the atomic unit retires 8.8 of 128 lanes "
-                            "per clock, so this design cannot exceed 0.069 there",
+                       note="achieved = algorithmic (pair, mid branch) updates per second against the rate of the shared-memory atomic unit "
+                            "(one atomic per update is what the ungrouped join k_mid needs); the grouped join executes atomics_executed "
+                            "atomics for them (frac_atomics_executed of the unit's rate).  ms_mid also covers the list preparation "
+                            "kernels (grouping, k_mid_seg/off/pack, k_midg_pack_*).  frac_of_fp32_lane_roofline = 2 lane-ops per update "
+                            "against the FP32-lane peak of SURVEY 8(d)",
                        peak_source=f"shared-memory u32 atomic adds on random cells of a 128 x 128 tile, 3 CTAs/SM x 512 threads "
                                    f"(= {ATOMS_PEAK / SM_COUNT / SM_MAX_GHZ / 1e9:.2f} lane-ops/clk/SM; same rate conflict-free), {rates_src}"))
     for r in rl:

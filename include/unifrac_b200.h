@@ -183,6 +183,8 @@ typedef struct {
     uint64_t workspace_bytes;    /* device bytes requested from the allocator                         */
     uint64_t skip_updates_executed; /* RICHNESS_ZONES (k_zone): 128 x 128 pair updates per (row, tile pair) visit           */
     uint64_t skip_row_pair_visits;  /* (row, tile pair) visits of k_zone                                                     */
+    uint64_t mid_atomics;        /* shared-memory atomics of the mid stage: one per (pair, lone mid row) and one per (pair, group root);
+                                    = mid_updates without the grouped join                                                  */
     uint32_t n_tile_pairs;       /* 128x128 tile pairs in the upper triangle                          */
     uint32_t n_levels;           /* tree depth levels                                                 */
     uint32_t stripe_launches;    /* stripe-kernel launches in this call                               */

@@ -39,7 +39,7 @@ class Stats(C.Structure):
                 ("tail_entries", C.c_uint64), ("mid_rows", C.c_uint64), ("mid_updates", C.c_uint64),
                 ("rows_staged", C.c_uint64),
                 ("embed_rows", C.c_uint64), ("workspace_bytes", C.c_uint64), ("skip_updates_executed", C.c_uint64),
-                ("skip_row_pair_visits", C.c_uint64), ("n_tile_pairs", C.c_uint32),
+                ("skip_row_pair_visits", C.c_uint64), ("mid_atomics", C.c_uint64), ("n_tile_pairs", C.c_uint32),
                 ("n_levels", C.c_uint32), ("stripe_launches", C.c_uint32), ("tail_launches", C.c_uint32),
                 ("kernel_launches", C.c_uint32), ("mid_launches", C.c_uint32), ("mid_F", C.c_uint32), ("gram", C.c_uint32), ("gram_k", C.c_uint32), ("gram_q", C.c_uint32), ("dense", C.c_uint32), ("skip", C.c_uint32), ("skip_rows", C.c_uint32), ("list_rows", C.c_uint32), ("guard_pairs", C.c_uint32), ("guard_capacity", C.c_uint32), ("mid_groups", C.c_uint32), ("mid_group_rows", C.c_uint32), ("quant_fallback", C.c_uint32), ("guard_theta", C.c_float), ("quant_err_ratio", C.c_float),
                 ("ms_plan", C.c_float), ("ms_embed", C.c_float), ("ms_tail", C.c_float), ("ms_mid", C.c_float), ("ms_stripe", C.c_float),

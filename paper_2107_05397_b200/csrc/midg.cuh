@@ -53,7 +53,7 @@ __global__ void k_midg_level(uint32_t n_lv, const int32_t* __restrict__ level_no
 }
 
 // members of groups with at least two members leave the k_mid rows: cnt[0] += roots, cnt[1] += rows (roots + members),
-// cnt[2] += entries of the roots, cnt[3] += sum of n_v (n_v - 1) / 2 over the rows that left
+// cnt[2] += entries of the roots, cnt[3] += sum of n_v (n_v - 1) / 2 over the rows that left, cnt[4] += the same over the roots only
 __global__ void k_midg_classify(int n, uint8_t* __restrict__ cls, const uint32_t* __restrict__ nv, const int32_t* __restrict__ groot,
                                 const uint32_t* __restrict__ gcnt, unsigned long long* __restrict__ cnt)
 {
@@ -64,7 +64,7 @@ __global__ void k_midg_classify(int n, uint8_t* __restrict__ cls, const uint32_t
     const bool is_root = r == v;
     cls[v] = is_root ? CLS_MIDG_ROOT : CLS_MIDG_MEMBER;
     const unsigned long long k = nv[v];
-    if (is_root) { atomicAdd(&cnt[0], 1ull); atomicAdd(&cnt[2], k); }
+    if (is_root) { atomicAdd(&cnt[0], 1ull); atomicAdd(&cnt[2], k); atomicAdd(&cnt[4], k * (k - 1) / 2); }
     atomicAdd(&cnt[1], 1ull);
     atomicAdd(&cnt[3], k * (k - 1) / 2);
 }

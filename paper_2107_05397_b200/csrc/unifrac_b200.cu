@@ -680,6 +680,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     int mid_F = 0;
     bool mid_packed = false;
     uint32_t midg_groups = 0, midg_rows = 0;
+    unsigned long long mid_atomics = mid_updates;
     double quant_ratio = 0.0;
     // fixed-point error ratio (Gram head lengths + mid entries): over budget => rerun without the fixed-point kernels
     auto check_quant_ratio = [&]() {
@@ -703,9 +704,9 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             if (groups_on) {
                 groot = A.get_n<int32_t>(n); gslot = A.get_n<uint8_t>(n);
                 uint32_t* gcnt = A.get_n<uint32_t>(n);
-                unsigned long long* gc = A.get_n<unsigned long long>(4);
+                unsigned long long* gc = A.get_n<unsigned long long>(8);
                 CU(cudaMemsetAsync(gcnt, 0, sizeof(uint32_t) * n, st));
-                CU(cudaMemsetAsync(gc, 0, sizeof(unsigned long long) * 4, st));
+                CU(cudaMemsetAsync(gc, 0, sizeof(unsigned long long) * 8, st));
                 const uint32_t theta_256 = (uint32_t)std::lround(256.0 * envd("UNIFRAC_B200_MID_GROUP_THETA", 0.35));
                 for (int d = 0; d < n_levels; ++d)
                     if (h_hist[d]) {
@@ -714,11 +715,12 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
                         CU_LAUNCH(); ++launches;
                     }
                 k_midg_classify<<<cdiv(n, TB), TB, 0, st>>>(n, cls, nv, groot, gcnt, gc); CU_LAUNCH(); ++launches;
-                unsigned long long h_gc[4] = {0, 0, 0, 0};
+                unsigned long long h_gc[5] = {0, 0, 0, 0, 0};
                 CU(cudaMemcpyAsync(h_gc, gc, sizeof(h_gc), cudaMemcpyDeviceToHost, st));
                 CU(cudaStreamSynchronize(st));
                 n_g = (uint32_t)h_gc[0]; g_rows = h_gc[1];
                 midg_groups = n_g; midg_rows = (uint32_t)g_rows;
+                mid_atomics = mid_updates - h_gc[3] + h_gc[4];    // one atomic per pair of a lone row / of a group root
             }
             const uint32_t n_mid = skip_on ? sk_n : (uint32_t)(mid_rows - g_rows);
             // row lists of one class ordered by n_v (counting sort)
@@ -1045,7 +1047,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     g_stats.embed_rows = embed_rows;
     g_stats.head_rows = head_rows; g_stats.tail_rows = tail_rows; g_stats.tail_updates = tail_updates; g_stats.tail_entries = tail_entries;
     g_stats.tail_launches = tail_launches;
-    g_stats.mid_groups = midg_groups; g_stats.mid_group_rows = midg_rows;
+    g_stats.mid_groups = midg_groups; g_stats.mid_group_rows = midg_rows; g_stats.mid_atomics = mid_atomics;
     g_stats.mid_rows = mid_rows; g_stats.mid_updates = mid_updates; g_stats.mid_launches = mid_launches; g_stats.mid_F = (uint32_t)mid_F;
     g_stats.skip = skip_on ? 1u : 0u; g_stats.skip_rows = sk_KE; g_stats.list_rows = sk_n;
     if (skip_on) { g_stats.mid_updates = h_skstat[0]; g_stats.skip_row_pair_visits = h_skstat[1]; g_stats.skip_updates_executed = h_skstat[1] * 16384ull; g_stats.mid_rows = sk_n; g_stats.head_rows = sk_KE; }
