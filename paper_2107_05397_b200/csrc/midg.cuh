@@ -97,10 +97,32 @@ __device__ __forceinline__ uint32_t midg_quant(float u, uint32_t s, float qscale
     return q;
 }
 
-// roots: one warp per group g.  ex / eq of the padding position of an odd (group, tile) list: ex repeats a valid cell, eq = 0.
+// Position of sample a (0..127 within its tile) in the (group, tile) list of a root whose presence bits in the tile are the
+// four words w[0..3] (bit r of w[j] = sample 32 j + r): the list is ordered by (a mod 32, a / 32), NOT by a.  A lane of k_midg
+// owns two consecutive positions and one ATOMS covers every second position of up to 32 lanes, all in the same column b of the
+// accumulator tile, whose bank is (a xor b) mod 32: in this order the rows a of one instruction differ mod 32 unless three
+// samples of the list share a residue, so the lanes of a group hit different banks (sorted by a they collided 3-fold:
+// ncu 3.06 shared-memory wavefronts per ATOMS).
+__device__ __forceinline__ uint32_t midg_rank(const uint4 w, uint32_t a)
+{
+    const uint32_t r = a & 31u, j = a >> 5, lt = (1u << r) - 1u;
+    uint32_t k = __popc(w.x & lt) + __popc(w.y & lt) + __popc(w.z & lt) + __popc(w.w & lt);
+    if (j > 0) k += (w.x >> r) & 1u;
+    if (j > 1) k += (w.y >> r) & 1u;
+    if (j > 2) k += (w.z >> r) & 1u;
+    return k;
+}
+__device__ __forceinline__ bool midg_has(const uint4 w, uint32_t a)
+{
+    const uint32_t j = a >> 5, x = j == 0 ? w.x : j == 1 ? w.y : j == 2 ? w.z : w.w;
+    return (x >> (a & 31u)) & 1u;
+}
+
+// roots: one warp per group g.  Padding positions of a (group, tile) list: ex repeats a valid cell, eq = 0 (memset).
+// bits4 = the presence bits of the tree nodes as uint4 (128 samples = one tile per element), NW4 elements per node.
 __global__ void __launch_bounds__(256)
-k_midg_pack_roots(uint32_t n_g, const uint32_t* __restrict__ gbase, const uint32_t* __restrict__ glen,
-                  const uint32_t* __restrict__ ts, const float* __restrict__ tv, const uint32_t* __restrict__ seg,
+k_midg_pack_roots(uint32_t n_g, const int32_t* __restrict__ grows, const uint32_t* __restrict__ gbase, const uint32_t* __restrict__ glen,
+                  const uint32_t* __restrict__ ts, const float* __restrict__ tv, const uint4* __restrict__ bits4, uint32_t NW4,
                   const uint32_t* __restrict__ off, const uint32_t* __restrict__ tbase, float qscale, double inv_qscale,
                   double* __restrict__ sums, double* __restrict__ qerr, uint32_t* __restrict__ ex, uint32_t* __restrict__ eq)
 {
@@ -108,26 +130,29 @@ k_midg_pack_roots(uint32_t n_g, const uint32_t* __restrict__ gbase, const uint32
     const int lane = threadIdx.x & 31;
     if (g >= n_g) return;
     const uint32_t base = gbase[g], m = glen[g];
+    const uint4* __restrict__ wrow = bits4 + (size_t)grows[g] * NW4;
     for (uint32_t k = lane; k < m; k += 32) {
         const uint32_t s = ts[base + k];
-        const uint32_t t = s >> 7;
-        const uint32_t g0 = seg[(size_t)t * n_g + g], g1 = seg[(size_t)(t + 1) * n_g + g];
-        const uint32_t pos = tbase[t] + off[(size_t)t * (n_g + 1) + g] + (k - g0);
-        const uint32_t x = (g << 9) | ((s & 127u) << 2);
+        const uint32_t t = s >> 7, a = s & 127u;
+        const uint4 w = wrow[t];
+        const uint32_t len = __popc(w.x) + __popc(w.y) + __popc(w.z) + __popc(w.w);
+        const uint32_t rk = midg_rank(w, a);
+        const uint32_t pos = tbase[t] + off[(size_t)t * (n_g + 1) + g] + rk;
+        const uint32_t x = (g << 9) | (a << 2);
         ex[pos] = x;
         eq[(size_t)pos * MIDG_L] = midg_quant(tv[base + k], s, qscale, inv_qscale, sums, qerr);
-        if (k + 1 == g1)                                          // padding positions: a valid cell, values 0 (memset)
-            for (uint32_t f = g1 - g0; f & (MIDG_R - 1); ++f) ex[pos + 1 + (f - (g1 - g0))] = x;
+        if (rk + 1 == len)
+            for (uint32_t f = len; f & (MIDG_R - 1); ++f) ex[pos + 1 + (f - len)] = x;
     }
 }
 
 // members: one warp per tree node (only CLS_MIDG_MEMBER nodes do anything).  Every sample of the member is a sample of its
-// root: its position in the root's sorted list comes from a binary search; a miss (never, by the subset property) is counted.
+// root: the position comes from the ROOT's presence bits; a miss (never, by the subset property) is counted.
 __global__ void __launch_bounds__(256)
 k_midg_pack_members(int n, const uint8_t* __restrict__ cls, const int32_t* __restrict__ groot, const uint8_t* __restrict__ gslot,
                     const int32_t* __restrict__ rootidx, const uint32_t* __restrict__ tptr, const uint32_t* __restrict__ nv,
-                    const uint32_t* __restrict__ ts, const float* __restrict__ tv, uint32_t n_g, const uint32_t* __restrict__ seg,
-                    const uint32_t* __restrict__ off, const uint32_t* __restrict__ tbase, float qscale, double inv_qscale,
+                    const uint32_t* __restrict__ ts, const float* __restrict__ tv, const uint4* __restrict__ bits4, uint32_t NW4,
+                    uint32_t n_g, const uint32_t* __restrict__ off, const uint32_t* __restrict__ tbase, float qscale, double inv_qscale,
                     double* __restrict__ sums, double* __restrict__ qerr, uint32_t* __restrict__ eq, unsigned long long* __restrict__ misses)
 {
     const int v = (int)((blockIdx.x * (unsigned)blockDim.x + threadIdx.x) >> 5);
@@ -135,14 +160,14 @@ k_midg_pack_members(int n, const uint8_t* __restrict__ cls, const int32_t* __res
     if (v >= n || cls[v] != CLS_MIDG_MEMBER) return;
     const int r = groot[v];
     const uint32_t g = (uint32_t)rootidx[r], slot = gslot[v];
-    const uint32_t base = tptr[v], m = nv[v], rbase = tptr[r], rm = nv[r];
+    const uint32_t base = tptr[v], m = nv[v];
+    const uint4* __restrict__ wrow = bits4 + (size_t)r * NW4;
     for (uint32_t k = lane; k < m; k += 32) {
         const uint32_t s = ts[base + k];
-        uint32_t lo = 0, hi = rm;                                 // first root entry with sample >= s
-        while (lo < hi) { const uint32_t mid = (lo + hi) >> 1; if (ts[rbase + mid] < s) lo = mid + 1; else hi = mid; }
-        if (lo >= rm || ts[rbase + lo] != s) { atomicAdd(misses, 1ull); continue; }
-        const uint32_t t = s >> 7;
-        const uint32_t pos = tbase[t] + off[(size_t)t * (n_g + 1) + g] + (lo - seg[(size_t)t * n_g + g]);
+        const uint32_t t = s >> 7, a = s & 127u;
+        const uint4 w = wrow[t];
+        if (!midg_has(w, a)) { atomicAdd(misses, 1ull); continue; }
+        const uint32_t pos = tbase[t] + off[(size_t)t * (n_g + 1) + g] + midg_rank(w, a);
         eq[(size_t)pos * MIDG_L + slot] = midg_quant(tv[base + k], s, qscale, inv_qscale, sums, qerr);
     }
 }

@@ -796,10 +796,11 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
                 CU(cudaMemsetAsync(gex, 0, sizeof(uint32_t) * ((size_t)h_g_total + 4), st));
                 CU(cudaMemsetAsync(geq, 0, sizeof(uint32_t) * ((size_t)h_g_total + 4) * MIDG_L, st));
                 k_midg_index<<<cdiv(n_g, TB), TB, 0, st>>>(n_g, grows, rootidx); CU_LAUNCH(); ++launches;
-                k_midg_pack_roots<<<cdiv((long long)n_g * 32, TB), TB, 0, st>>>(n_g, gbase, glen, ts, reinterpret_cast<const float*>(tv), GLs.seg, GLs.off,
-                                                                               GLs.tbase, qscale, inv_qscale, sums, qerr, gex, geq); CU_LAUNCH(); ++launches;
+                const uint4* bits4 = reinterpret_cast<const uint4*>(bits);
+                k_midg_pack_roots<<<cdiv((long long)n_g * 32, TB), TB, 0, st>>>(n_g, grows, gbase, glen, ts, reinterpret_cast<const float*>(tv), bits4, NW4,
+                                                                               GLs.off, GLs.tbase, qscale, inv_qscale, sums, qerr, gex, geq); CU_LAUNCH(); ++launches;
                 k_midg_pack_members<<<cdiv((long long)n * 32, TB), TB, 0, st>>>(n, cls, groot, gslot, rootidx, tptr, nv, ts, reinterpret_cast<const float*>(tv),
-                                                                               n_g, GLs.seg, GLs.off, GLs.tbase, qscale, inv_qscale, sums, qerr, geq, gmiss);
+                                                                               bits4, NW4, n_g, GLs.off, GLs.tbase, qscale, inv_qscale, sums, qerr, geq, gmiss);
                 CU_LAUNCH(); ++launches;
             }
             mid_packed = true;
