@@ -172,6 +172,53 @@ Calib calibration(int dev, cudaStream_t st)
     return cache[dev];
 }
 
+// Small device -> host read-backs of the planning steps.  A cudaMemcpyAsync would queue on the device-to-host copy engine BEHIND
+// every copy submitted before it, from any stream -- in unifrac_dm_host_multi that is the previous variant's 5 GB result, and the
+// next variant's planning (a dozen read-backs of a few words) then waited ~90 ms for it.  Here a one-block kernel writes the words
+// into page-locked MAPPED host memory instead, and sync() hands them to their destinations after the stream synchronisation.
+__global__ void k_readback(unsigned char* __restrict__ dst, const unsigned char* __restrict__ src, size_t bytes)
+{
+    for (size_t i = threadIdx.x; i < bytes; i += blockDim.x) dst[i] = src[i];
+}
+struct Readback {
+    static constexpr size_t CAP = 64 * 1024, MAX_ITEM = 16 * 1024;
+    struct Item { void* dst; size_t off, bytes; };
+    cudaStream_t st;
+    std::vector<Item> items;
+    size_t used = 0;
+    explicit Readback(cudaStream_t s) : st(s) {}
+    static unsigned char* stage() {                       // one buffer per host thread, kept for the life of the process
+        thread_local unsigned char* h = nullptr;
+        thread_local bool failed = false;
+        if (!h && !failed) {
+            void* p = nullptr;
+            if (cudaHostAlloc(&p, CAP, cudaHostAllocPortable | cudaHostAllocMapped) == cudaSuccess) h = static_cast<unsigned char*>(p);
+            else { cudaGetLastError(); failed = true; }
+        }
+        return h;
+    }
+    void get(void* dst, const void* src, size_t bytes) {
+        unsigned char* h = stage();
+        void* d = nullptr;
+        if (!h || bytes > MAX_ITEM || used + bytes > CAP || cudaHostGetDevicePointer(&d, h, 0) != cudaSuccess) {
+            cudaGetLastError();
+            CU(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, st));
+            return;
+        }
+        k_readback<<<1, 256, 0, st>>>(static_cast<unsigned char*>(d) + used, static_cast<const unsigned char*>(src), bytes);
+        CU_LAUNCH();
+        items.push_back({dst, used, bytes});
+        used += (bytes + 15) & ~(size_t)15;
+    }
+    void sync() {
+        CU(cudaStreamSynchronize(st));
+        unsigned char* h = stage();
+        for (const Item& it : items) memcpy(it.dst, h + it.off, it.bytes);
+        items.clear();
+        used = 0;
+    }
+};
+
 // stable LSD radix sort of (key, position) pairs (rank.cuh); the sort buffers are shared between the sorts of a call
 struct RankBufs { void* keys[2]; uint32_t* idx[2]; uint32_t* hist; uint32_t* offs; uint32_t* blast; unsigned nb; unsigned long long per_block; };
 template <typename T>
@@ -250,6 +297,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
          int32_t N, int weighted, void* out, Arena& A, uint32_t flags, cudaStream_t st, int shard, int n_shards, bool is_retry,
          ProgressFn progress = nullptr, void* progress_user = nullptr)
 {
+    Readback RDB(st);                   // the planning steps' small read-backs (no copy engine: see struct Readback)
     const bool validate = !(flags & UNIFRAC_FLAG_SKIP_VALIDATION);
     const bool timing = getenv("UNIFRAC_B200_TIMING") && atoi(getenv("UNIFRAC_B200_TIMING")) != 0;
     Timer tm(timing, st);
@@ -273,9 +321,9 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         CU(cudaMemsetAsync(bad, 0, sizeof(unsigned int), st));
         k_perm_keys<<<cdiv(N, TB), TB, 0, st>>>(N, tab.indptr, key, bad); CU_LAUNCH(); ++launches;
         unsigned int h_bad = 0; long long h_nnz = 0;
-        CU(cudaMemcpyAsync(&h_bad, bad, sizeof(h_bad), cudaMemcpyDeviceToHost, st));
-        CU(cudaMemcpyAsync(&h_nnz, tab.indptr + N, sizeof(h_nnz), cudaMemcpyDeviceToHost, st));
-        CU(cudaStreamSynchronize(st));
+        RDB.get(&h_bad, bad, sizeof(h_bad));
+        RDB.get(&h_nnz, tab.indptr + N, sizeof(h_nnz));
+        RDB.sync();
         if (!h_bad && h_nnz >= 0 && h_nnz < (1ll << 32)) {       // otherwise: validation below reports what is wrong
             RankBufs RB = make_rank_bufs<uint32_t>(A, (unsigned long long)N, n_sm_dev);
             const int src = radix_sort<uint32_t>(key, (unsigned long long)N, RB, st);
@@ -312,8 +360,8 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         k_post_check2<<<cdiv(n, TB), TB, 0, st>>>(n, parent, postorder, pos, pw); CU_LAUNCH(); ++launches;
     }
     PlanWords h{};
-    CU(cudaMemcpyAsync(&h, pw, sizeof(h), cudaMemcpyDeviceToHost, st));
-    CU(cudaStreamSynchronize(st));
+    RDB.get(&h, pw, sizeof(h));
+    RDB.sync();
     if (h.err & ERRBIT_TREE) throw StatusFail{UNIFRAC_ERR_INVALID_TREE};
 
     k_csr_check<<<cdiv((long long)N * 32, TB), TB, 0, st>>>(n, N, tab.indptr, tab.indices, tab.counts, child_count,
@@ -331,8 +379,8 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     uint32_t* hist = A.get_n<uint32_t>((size_t)n + 1);
     CU(cudaMemsetAsync(hist, 0, sizeof(uint32_t) * ((size_t)n + 1), st));
     k_level_hist<<<cdiv(n, TB), TB, 0, st>>>(n, depth, child_count, hist, pw); CU_LAUNCH(); ++launches;
-    CU(cudaMemcpyAsync(&h, pw, sizeof(h), cudaMemcpyDeviceToHost, st));
-    CU(cudaStreamSynchronize(st));
+    RDB.get(&h, pw, sizeof(h));
+    RDB.sync();
     if (h.err & ERRBIT_TABLE) throw StatusFail{UNIFRAC_ERR_INVALID_TABLE};
     if (h.err & ERRBIT_EMPTY) throw StatusFail{UNIFRAC_ERR_EMPTY_SAMPLE};
     if (h.err & ERRBIT_UNSUPPORTED) throw StatusFail{UNIFRAC_ERR_UNSUPPORTED};
@@ -340,8 +388,8 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     const int n_levels = h.max_depth + 1;
     const size_t n_internal = (size_t)h.n_internal;
     std::vector<uint32_t> h_hist(n_levels), h_off(n_levels + 1);
-    CU(cudaMemcpyAsync(h_hist.data(), hist, sizeof(uint32_t) * n_levels, cudaMemcpyDeviceToHost, st));
-    CU(cudaStreamSynchronize(st));
+    RDB.get(h_hist.data(), hist, sizeof(uint32_t) * n_levels);
+    RDB.sync();
     h_off[0] = 0;
     for (int d = 0; d < n_levels; ++d) h_off[d + 1] = h_off[d] + h_hist[d];
     uint32_t* cursor = A.get_n<uint32_t>(n_levels);
@@ -425,8 +473,8 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         k_exclusive_scan<uint32_t><<<1, 1024, 0, st>>>(n, tipc, cptr); CU_LAUNCH(); ++launches;
     }
     unsigned long long h_work[18];
-    CU(cudaMemcpyAsync(h_work, work, sizeof(h_work), cudaMemcpyDeviceToHost, st));
-    CU(cudaStreamSynchronize(st));
+    RDB.get(h_work, work, sizeof(h_work));
+    RDB.sync();
     const unsigned long long head_rows = h_work[8], tail_rows = h_work[9], tail_updates = h_work[10], tail_entries = h_work[11];
     const unsigned long long mid_rows = h_work[12], mid_updates = h_work[13], nnz_pos = h_work[16], mid_entries = h_work[17];
     if (tail_entries >= (1ull << 32) || nnz_pos >= (1ull << 32)) throw StatusFail{UNIFRAC_ERR_UNSUPPORTED};
@@ -456,8 +504,8 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         unsigned long long* lmax = work + 14;
         k_gram_lenmax<<<cdiv(n, TB), TB, 0, st>>>(n, cls, len, lmax); CU_LAUNCH(); ++launches;
         unsigned long long h_lmax = 0;
-        CU(cudaMemcpyAsync(&h_lmax, lmax, sizeof(h_lmax), cudaMemcpyDeviceToHost, st));
-        CU(cudaStreamSynchronize(st));
+        RDB.get(&h_lmax, lmax, sizeof(h_lmax));
+        RDB.sync();
         double lm; memcpy(&lm, &h_lmax, sizeof(lm));
         int ex = 0; frexp(lm, &ex);
         const uint32_t K = (uint32_t)head_rows;
@@ -586,9 +634,9 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         k_cut_table<<<cdiv(n_tiles + 1, TB), TB, 0, st>>>(n_tiles, sk_n, Dr, ZONE_BK, sk_cut); CU_LAUNCH(); ++launches;
         k_cut_stats<<<cdiv((long long)sk_n * 32, TB), TB, 0, st>>>(sk_n, sk_rows, bits, NW, n_tiles, sk_cut, work + 21); CU_LAUNCH(); ++launches;
         h_cut.resize((size_t)n_tiles + 1);
-        CU(cudaMemcpyAsync(h_cut.data(), sk_cut, sizeof(uint32_t) * ((size_t)n_tiles + 1), cudaMemcpyDeviceToHost, st));
-        CU(cudaMemcpyAsync(h_skstat, work + 21, sizeof(h_skstat), cudaMemcpyDeviceToHost, st));
-        CU(cudaStreamSynchronize(st));
+        RDB.get(h_cut.data(), sk_cut, sizeof(uint32_t) * ((size_t)n_tiles + 1));
+        RDB.get(h_skstat, work + 21, sizeof(h_skstat));
+        RDB.sync();
         sk_KE = h_cut[n_tiles - 1];                              // cut is non-decreasing in the tile index
         const size_t e_rows = sk_KE ? sk_KE : ZONE_BK;
         sk_E = A.get_n<float>(e_rows * Npad);
@@ -609,8 +657,8 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         k_head_flags<<<cdiv((long long)nwords * 32, TB), TB, 0, st>>>(n, cls, bits, NW, n_tiles, rflags, nwords); CU_LAUNCH(); ++launches;
         k_rank_scan<<<n_tiles, 1024, 0, st>>>(rflags, rrank, nwords, 0, rows); CU_LAUNCH(); ++launches;
         std::vector<uint32_t> h_rows(n_tiles);
-        CU(cudaMemcpyAsync(h_rows.data(), rows, sizeof(uint32_t) * n_tiles, cudaMemcpyDeviceToHost, st));
-        CU(cudaStreamSynchronize(st));
+        RDB.get(h_rows.data(), rows, sizeof(uint32_t) * n_tiles);
+        RDB.sync();
         for (int t = 0; t < n_tiles; ++t) embed_rows += h_rows[t];
         T* Eb = A.get_n<T>((embed_rows ? embed_rows : 1) * TILE);
         uint8_t* Qb = A.get_n<uint8_t>(embed_rows ? embed_rows : 1);
@@ -632,7 +680,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
                                                                                     weighted ? tv : nullptr, tileE, tileQ);
             CU_LAUNCH(); ++launches;
         }
-        CU(cudaStreamSynchronize(st));   // h_tileE / h_tileQ staging copies are done
+        RDB.sync();   // h_tileE / h_tileQ staging copies are done
     }
     tm.mark();
 
@@ -662,7 +710,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
                 for (int bi = 0; bi <= bj; ++bi) h_owner[(size_t)bj * (bj + 1) / 2 + bi] = (uint8_t)(((long long)bj * (bj + 1) / 2 + bi) % n_shards);
             uint8_t* owner = A.get_n<uint8_t>(h_owner.size());
             CU(cudaMemcpyAsync(owner, h_owner.data(), h_owner.size(), cudaMemcpyHostToDevice, st));
-            CU(cudaStreamSynchronize(st));
+            RDB.sync();
             TP.owner = owner; TP.shard = shard;
         }
         TP.tptr = tptr; TP.seg = seg; TP.ts = ts; TP.tv = tv; TP.cls = cls; TP.n = n; TP.nsup = nsup; TP.N = N; TP.out = out;
@@ -687,8 +735,8 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         unsigned long long* rbits = work + 19;
         k_quant_ratio<<<cdiv((long long)n_tiles * TILE, TB), TB, 0, st>>>(n_tiles * TILE, qerr, sums, rbits); CU_LAUNCH(); ++launches;
         unsigned long long h_r = 0;
-        CU(cudaMemcpyAsync(&h_r, rbits, sizeof(h_r), cudaMemcpyDeviceToHost, st));
-        CU(cudaStreamSynchronize(st));
+        RDB.get(&h_r, rbits, sizeof(h_r));
+        RDB.sync();
         memcpy(&quant_ratio, &h_r, sizeof(quant_ratio));
         if (quant_ratio > envd("UNIFRAC_B200_QUANT_BUDGET", QUANT_RATIO_BUDGET) && !is_retry) throw RetryExact{};
     };
@@ -716,8 +764,8 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
                     }
                 k_midg_classify<<<cdiv(n, TB), TB, 0, st>>>(n, cls, nv, groot, gcnt, gc); CU_LAUNCH(); ++launches;
                 unsigned long long h_gc[5] = {0, 0, 0, 0, 0};
-                CU(cudaMemcpyAsync(h_gc, gc, sizeof(h_gc), cudaMemcpyDeviceToHost, st));
-                CU(cudaStreamSynchronize(st));
+                RDB.get(h_gc, gc, sizeof(h_gc));
+                RDB.sync();
                 n_g = (uint32_t)h_gc[0]; g_rows = h_gc[1];
                 midg_groups = n_g; midg_rows = (uint32_t)g_rows;
                 mid_atomics = mid_updates - h_gc[3] + h_gc[4];    // one atomic per pair of a lone row / of a group root
@@ -761,10 +809,10 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             if (n_g) { k_midg_sums<<<cdiv((long long)n * 32, TB), TB, 0, st>>>(n, cls, tptr, nv, ts, reinterpret_cast<const float*>(tv), midsum); CU_LAUNCH(); ++launches; }
             k_max_positive<<<cdiv((long long)n_tiles * TILE, TB), TB, 0, st>>>(n_tiles * TILE, midsum, smax); CU_LAUNCH(); ++launches;
             unsigned long long h_smax = 0;
-            CU(cudaMemcpyAsync(&h_smax, smax, sizeof(h_smax), cudaMemcpyDeviceToHost, st));
+            RDB.get(&h_smax, smax, sizeof(h_smax));
             uint32_t h_pk_total = 0, h_g_total = 0;             // packed entries / positions incl. the even-length padding
-            CU(cudaMemcpyAsync(&h_pk_total, ML.tbase + n_tiles, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
-            if (n_g) CU(cudaMemcpyAsync(&h_g_total, GLs.tbase + n_tiles, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+            RDB.get(&h_pk_total, ML.tbase + n_tiles, sizeof(uint32_t));
+            if (n_g) RDB.get(&h_g_total, GLs.tbase + n_tiles, sizeof(uint32_t));
             std::vector<int2> h_mp = blocked_pairs(n_tiles, 8, shard, n_shards);
             const size_t n_all_pairs = h_mp.size();
             int2* gpairs = A.get_n<int2>(n_all_pairs ? n_all_pairs : 1);     // the grouped join visits every tile pair of the shard
@@ -773,7 +821,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
                 h_mp.erase(std::remove_if(h_mp.begin(), h_mp.end(), [&](const int2& q) { return h_cut[q.x] >= sk_n; }), h_mp.end());
             int2* mpairs = A.get_n<int2>(h_mp.size() ? h_mp.size() : 1);
             CU(cudaMemcpyAsync(mpairs, h_mp.data(), sizeof(int2) * h_mp.size(), cudaMemcpyHostToDevice, st));
-            CU(cudaStreamSynchronize(st));
+            RDB.sync();
             double sm; memcpy(&sm, &h_smax, sizeof(sm));
             int ex = 0; frexp(sm > 0 ? sm : 1.0, &ex);          // sm < 2^ex
             // unsigned 32-bit cells: acc <= min(R^mid_a, R^mid_b) * 2^F + (rounding: at most half a unit per mid row)
@@ -807,7 +855,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
             check_quant_ratio();
             if (n_g) {                                            // (the stream was just synchronised)
                 unsigned long long h_miss = 0;
-                CU(cudaMemcpy(&h_miss, gmiss, sizeof(h_miss), cudaMemcpyDeviceToHost));
+                RDB.get(&h_miss, gmiss, sizeof(h_miss)); RDB.sync();
                 if (h_miss) { g_cuda_err = "grouped join: a member branch has a sample its group root lacks"; throw StatusFail{UNIFRAC_ERR_CUDA}; }
             }
             int dev2 = 0, n_sm2 = 0;
@@ -1062,7 +1110,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     A.release();
     g_stats.workspace_bytes = A.total;
     if (timing) {
-        CU(cudaStreamSynchronize(st));
+        RDB.sync();
         g_stats.ms_plan = tm.ms(0, 1); g_stats.ms_embed = tm.ms(1, 3); g_stats.ms_tail = tm.ms(3, 4); g_stats.ms_mid = tm.ms(4, 5); g_stats.ms_stripe = tm.ms(5, 6);
         g_stats.ms_total = tm.ms(0, 6);
     }
