@@ -923,7 +923,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
         std::vector<Seg> segs;
         const uint32_t np = (uint32_t)pl.size();
         const bool split = progress && n_shards == 1 && !inv_perm && np >= 64;
-        const int n_seg = split ? (int)env_double("UNIFRAC_B200_E2E_SEGMENTS", 4) : 1;
+        const int n_seg = split ? (int)env_double("UNIFRAC_B200_E2E_SEGMENTS", 8) : 1;
         uint32_t begin = 0;
         for (int k = 1; k <= n_seg && begin < np; ++k) {
             uint32_t end = k == n_seg ? np : (uint32_t)((unsigned long long)np * k / n_seg);
