@@ -27,6 +27,7 @@ constexpr int MIDG_R = 2;            // I positions per lane of k_midg; every (g
 constexpr uint8_t CLS_MIDG_ROOT = 4, CLS_MIDG_MEMBER = 5;
 constexpr int MIDG_THREADS = 384;       // x 3 CTAs per SM: 56 registers per thread
 constexpr int MIDG_MINB = 3;
+constexpr uint32_t MIDG_MASK0 = 0x200u;  // mask mode: bit 9 + slot of a position's 16-bit word = member `slot` is present there (bits 2..8: cell << 2)
 
 // children of the internal nodes of one tree level: groot[c] = root of c's group, gslot[c] = its slot, gcnt[r] = members so far
 __global__ void k_midg_level(uint32_t n_lv, const int32_t* __restrict__ level_nodes, const uint32_t* __restrict__ child_off,
@@ -124,7 +125,8 @@ __global__ void __launch_bounds__(256)
 k_midg_pack_roots(uint32_t n_g, const int32_t* __restrict__ grows, const uint32_t* __restrict__ gbase, const uint32_t* __restrict__ glen,
                   const uint32_t* __restrict__ ts, const float* __restrict__ tv, const uint4* __restrict__ bits4, uint32_t NW4,
                   const uint32_t* __restrict__ off, const uint32_t* __restrict__ tbase, float qscale, double inv_qscale,
-                  double* __restrict__ sums, double* __restrict__ qerr, uint32_t* __restrict__ ex, uint32_t* __restrict__ eq)
+                  double* __restrict__ sums, double* __restrict__ qerr, uint32_t* __restrict__ ex, uint32_t* __restrict__ eq,
+                  uint16_t* __restrict__ em, uint32_t* __restrict__ gq /* mask mode (unweighted), else NULL: see k_midg<true> */)
 {
     const uint32_t g = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
@@ -140,9 +142,11 @@ k_midg_pack_roots(uint32_t n_g, const int32_t* __restrict__ grows, const uint32_
         const uint32_t pos = tbase[t] + off[(size_t)t * (n_g + 1) + g] + rk;
         const uint32_t x = (g << 9) | (a << 2);
         ex[pos] = x;
-        eq[(size_t)pos * MIDG_L] = midg_quant(tv[base + k], s, qscale, inv_qscale, sums, qerr);
+        const uint32_t q = midg_quant(tv[base + k], s, qscale, inv_qscale, sums, qerr);
+        if (em) { em[pos] = (uint16_t)((a << 2) | MIDG_MASK0); gq[(size_t)g * MIDG_L] = q; }     // the same q for every entry of the row
+        else eq[(size_t)pos * MIDG_L] = q;
         if (rk + 1 == len)
-            for (uint32_t f = len; f & (MIDG_R - 1); ++f) ex[pos + 1 + (f - len)] = x;
+            for (uint32_t f = len; f & (MIDG_R - 1); ++f) { ex[pos + 1 + (f - len)] = x; if (em) em[pos + 1 + (f - len)] = (uint16_t)(a << 2); }
     }
 }
 
@@ -153,7 +157,8 @@ k_midg_pack_members(int n, const uint8_t* __restrict__ cls, const int32_t* __res
                     const int32_t* __restrict__ rootidx, const uint32_t* __restrict__ tptr, const uint32_t* __restrict__ nv,
                     const uint32_t* __restrict__ ts, const float* __restrict__ tv, const uint4* __restrict__ bits4, uint32_t NW4,
                     uint32_t n_g, const uint32_t* __restrict__ off, const uint32_t* __restrict__ tbase, float qscale, double inv_qscale,
-                    double* __restrict__ sums, double* __restrict__ qerr, uint32_t* __restrict__ eq, unsigned long long* __restrict__ misses)
+                    double* __restrict__ sums, double* __restrict__ qerr, uint32_t* __restrict__ eq, unsigned long long* __restrict__ misses,
+                    uint16_t* __restrict__ em, uint32_t* __restrict__ gq)
 {
     const int v = (int)((blockIdx.x * (unsigned)blockDim.x + threadIdx.x) >> 5);
     const int lane = threadIdx.x & 31;
@@ -168,7 +173,11 @@ k_midg_pack_members(int n, const uint8_t* __restrict__ cls, const int32_t* __res
         const uint4 w = wrow[t];
         if (!midg_has(w, a)) { atomicAdd(misses, 1ull); continue; }
         const uint32_t pos = tbase[t] + off[(size_t)t * (n_g + 1) + g] + midg_rank(w, a);
-        eq[(size_t)pos * MIDG_L + slot] = midg_quant(tv[base + k], s, qscale, inv_qscale, sums, qerr);
+        const uint32_t q = midg_quant(tv[base + k], s, qscale, inv_qscale, sums, qerr);
+        if (em) {                                                // set the member's bit in the position's 16-bit word
+            atomicOr(reinterpret_cast<uint32_t*>(em) + (pos >> 1), (MIDG_MASK0 << slot) << (16u * (pos & 1u)));
+            gq[(size_t)g * MIDG_L + slot] = q;
+        } else eq[(size_t)pos * MIDG_L + slot] = q;
     }
 }
 
@@ -183,6 +192,8 @@ struct MidgParams {
     int n_samples;
     float* out;
     double inv_qscale;            // 2^-F
+    const uint16_t* em;           // mask mode (k_midg<true>, unweighted): per position cell << 2 | member mask << 9 ...
+    const uint4* gq;              // ... and per group the members' (constant) fixed-point values
     MidParams rows;               // the mid rows that stayed alone: joined by the same CTA into the same accumulators (n_mid = 0: none)
 };
 
@@ -195,6 +206,13 @@ __device__ __forceinline__ uint32_t midg_dot(const uint4& a, const uint4& b) {
 // a chunk of 128; every J position a lane loads (20 bytes: cell + 4 values) feeds 4 atomics.  That ratio is the point: a
 // warp-wide 16-byte load occupies the L1 data pipe for 4 cycles whether or not the lanes read the same address, and with
 // one I position per lane those loads, not the atomics, bounded the kernel (ncu: data pipe 94 %, of it atomics 31 %).
+// MASK = true (unweighted): a member's value is the same at every sample where it is present (u~ = the branch length), so a
+// position carries 4 presence bits instead of 4 values -- 2 bytes per J position instead of 20 -- and the lane adds the group's
+// values q[k] where both positions have the bit.
+__device__ __forceinline__ uint32_t midg_sel(uint32_t m, const uint4& q) {
+    return ((m & MIDG_MASK0) ? q.x : 0u) + ((m & (MIDG_MASK0 << 1)) ? q.y : 0u) + ((m & (MIDG_MASK0 << 2)) ? q.z : 0u) + ((m & (MIDG_MASK0 << 3)) ? q.w : 0u);
+}
+template <bool MASK>
 __global__ void __launch_bounds__(MIDG_THREADS, MIDG_MINB)
 k_midg(const MidgParams P)
 {
@@ -248,16 +266,45 @@ k_midg(const MidgParams P)
             jC0 = jB0; jC1 = jB1;
             const uint32_t e = eI0 + (c * 32u + lane) * MIDG_R;
             uint4 q[MIDG_R];
-            uint32_t row[MIDG_R];
+            uint32_t row[MIDG_R], mA[MIDG_R];
+            if (MASK) {
+                static_assert(MIDG_R == 2, "mask mode reads the lane's two 16-bit words as one 32-bit load");
+                q[0] = make_uint4(0u, 0u, 0u, 0u);
+                uint32_t w = 0u;
+                if (jC0 < jC1) { q[0] = __ldg(P.gq + (xC[0] >> 9)); w = __ldg(reinterpret_cast<const uint32_t*>(P.em + e)); }
+                mA[0] = w & 0x1e00u; mA[1] = (w >> 16) & 0x1e00u;
+            }
 #pragma unroll
             for (int k = 0; k < MIDG_R; ++k) {
-                q[k] = make_uint4(0u, 0u, 0u, 0u);
-                if (jC0 < jC1) q[k] = __ldg(eq + e + k);
+                if (!MASK) { q[k] = make_uint4(0u, 0u, 0u, 0u); if (jC0 < jC1) q[k] = __ldg(eq + e + k); }
                 const uint32_t a4 = xC[k] & 0x1fcu;
                 row[k] = (macc_s + (a4 << 7)) | (a4 & 0x7cu);              // row base | (a & 31) << 2
             }
             load_pos(c + NWARP, xB, jB0, jB1);
             // 4 J positions per iteration (two independent pairs of loads in flight)
+            if (MASK) {
+                for (uint32_t l = jC0; __any_sync(0xffffffffu, l < jC1); l += 4) {
+                    const bool p0 = l < jC1, p1 = l + 2u < jC1;
+                    uint32_t w0 = 0u, w1 = 0u;
+                    if (p0) w0 = __ldg(reinterpret_cast<const uint32_t*>(P.em + l));
+                    if (p1) w1 = __ldg(reinterpret_cast<const uint32_t*>(P.em + l + 2));
+                    if (p0) {
+#pragma unroll
+                        for (int k = 0; k < MIDG_R; ++k) {
+                            mid_red(row[k] ^ (w0 & 0x1fcu), midg_sel(mA[k] & w0, q[0]));
+                            mid_red(row[k] ^ ((w0 >> 16) & 0x1fcu), midg_sel(mA[k] & (w0 >> 16), q[0]));
+                        }
+                    }
+                    if (p1) {
+#pragma unroll
+                        for (int k = 0; k < MIDG_R; ++k) {
+                            mid_red(row[k] ^ (w1 & 0x1fcu), midg_sel(mA[k] & w1, q[0]));
+                            mid_red(row[k] ^ ((w1 >> 16) & 0x1fcu), midg_sel(mA[k] & (w1 >> 16), q[0]));
+                        }
+                    }
+                }
+                continue;
+            }
             for (uint32_t l = jC0; __any_sync(0xffffffffu, l < jC1); l += 4) {
                 const bool p0 = l < jC1, p1 = l + 2u < jC1;
                 uint2 xa, xb; uint4 b0, b1, b2, b3;

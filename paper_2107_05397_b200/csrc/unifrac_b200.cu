@@ -836,19 +836,29 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
                                                                           qscale, inv_qscale, sums, qerr, pk, sk_cut); CU_LAUNCH(); ++launches;
             }
             uint32_t* gex = nullptr; uint32_t* geq = nullptr;
+            uint16_t* gem = nullptr; uint32_t* ggq = nullptr;    // mask mode (unweighted: a member's value is one number per row)
+            const bool mask_mode = !weighted && envd("UNIFRAC_B200_MID_MASKS", 1.0) != 0.0;
             unsigned long long* gmiss = work + 24;
             if (n_g) {
-                gex = A.get_n<uint32_t>((size_t)h_g_total + 4);
-                geq = A.get_n<uint32_t>(((size_t)h_g_total + 4) * MIDG_L);
+                const size_t n_pos = (size_t)h_g_total + 4;
+                gex = A.get_n<uint32_t>(n_pos);
+                CU(cudaMemsetAsync(gex, 0, sizeof(uint32_t) * n_pos, st));
+                if (mask_mode) {
+                    gem = A.get_n<uint16_t>(n_pos);
+                    ggq = A.get_n<uint32_t>((size_t)n_g * MIDG_L);
+                    CU(cudaMemsetAsync(gem, 0, sizeof(uint16_t) * n_pos, st));
+                    CU(cudaMemsetAsync(ggq, 0, sizeof(uint32_t) * (size_t)n_g * MIDG_L, st));
+                } else {
+                    geq = A.get_n<uint32_t>(n_pos * MIDG_L);
+                    CU(cudaMemsetAsync(geq, 0, sizeof(uint32_t) * n_pos * MIDG_L, st));
+                }
                 int32_t* rootidx = A.get_n<int32_t>(n);
-                CU(cudaMemsetAsync(gex, 0, sizeof(uint32_t) * ((size_t)h_g_total + 4), st));
-                CU(cudaMemsetAsync(geq, 0, sizeof(uint32_t) * ((size_t)h_g_total + 4) * MIDG_L, st));
                 k_midg_index<<<cdiv(n_g, TB), TB, 0, st>>>(n_g, grows, rootidx); CU_LAUNCH(); ++launches;
                 const uint4* bits4 = reinterpret_cast<const uint4*>(bits);
                 k_midg_pack_roots<<<cdiv((long long)n_g * 32, TB), TB, 0, st>>>(n_g, grows, gbase, glen, ts, reinterpret_cast<const float*>(tv), bits4, NW4,
-                                                                               GLs.off, GLs.tbase, qscale, inv_qscale, sums, qerr, gex, geq); CU_LAUNCH(); ++launches;
+                                                                               GLs.off, GLs.tbase, qscale, inv_qscale, sums, qerr, gex, geq, gem, ggq); CU_LAUNCH(); ++launches;
                 k_midg_pack_members<<<cdiv((long long)n * 32, TB), TB, 0, st>>>(n, cls, groot, gslot, rootidx, tptr, nv, ts, reinterpret_cast<const float*>(tv),
-                                                                               bits4, NW4, n_g, GLs.off, GLs.tbase, qscale, inv_qscale, sums, qerr, geq, gmiss);
+                                                                               bits4, NW4, n_g, GLs.off, GLs.tbase, qscale, inv_qscale, sums, qerr, geq, gmiss, gem, ggq);
                 CU_LAUNCH(); ++launches;
             }
             mid_packed = true;
@@ -879,11 +889,13 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
                 M.n_g = n_g; M.off = GLs.off; M.tbase = GLs.tbase; M.ex = gex; M.eq = reinterpret_cast<const uint4*>(geq);
                 M.n_samples = N; M.out = reinterpret_cast<float*>(out); M.inv_qscale = inv_qscale;
                 M.rows = MP;                                      // (groups are off in the zones path: MP.cut = NULL here)
-                CU(cudaFuncSetAttribute(k_midg, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MID_SMEM));
+                M.em = gem; M.gq = reinterpret_cast<const uint4*>(ggq);
+                auto kern = mask_mode ? k_midg<true> : k_midg<false>;
+                CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MID_SMEM));
                 int occ = 0;
-                CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_midg, MIDG_THREADS, MID_SMEM));
+                CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, MIDG_THREADS, MID_SMEM));
                 if (occ < 1) occ = 1;
-                k_midg<<<(unsigned)std::min<long long>((long long)n_sm2 * occ, (long long)n_all_pairs), MIDG_THREADS, MID_SMEM, st>>>(M);
+                kern<<<(unsigned)std::min<long long>((long long)n_sm2 * occ, (long long)n_all_pairs), MIDG_THREADS, MID_SMEM, st>>>(M);
                 CU_LAUNCH(); ++launches; ++mid_launches;
             }
         }
