@@ -120,7 +120,7 @@ def test_guard_in_shard_mode(B, O):
 
 def test_guard_with_segmented_finalize_in_host_multi(B, O):
     """unifrac_dm_host_multi finalizes the last variant in segments of block rows (guard + result copy after each one): planted
-    duplicates stay exactly 0 and the host result equals the device entry point's bit for bit.  1,700 samples = 105 tile pairs,
+    duplicates stay exactly 0 and the host result equals the device entry point's (to the last bits).  1,700 samples = 105 tile pairs,
     enough for the segmentation to kick in."""
     cfg = synth.CONFIGS["small"]
     base = synth.make_problem(2000, 1700, 0.1, 1.1, cfg[4], cfg[5], seed=17)
@@ -131,5 +131,6 @@ def test_guard_with_segmented_finalize_in_host_multi(B, O):
         outs = B.unifrac_dm_host_multi(p.parent, p.branch_len, p.postorder, p.indptr, p.indices, p.counts, n, order, B.FP32)
         for v, got in zip(order, outs):
             assert np.all(got[idx[kinds < 2]] == 0.0)
-            assert np.array_equal(got.astype(np.float64), gpu_dm(B, p, v, 0))
+            # (not bit for bit: the tail's fp32 REDs reach a cell in arbitrary order, so the last bit may differ between two runs)
+            assert np.allclose(got.astype(np.float64), gpu_dm(B, p, v, 0), rtol=2e-6, atol=1e-7)
     B.unifrac_release_host_pool()
