@@ -449,7 +449,7 @@ void run(int32_t n, const int32_t* parent, const double* len, const int32_t* pos
     // the rows that compete with the Gram kernel are sparse (a few entries per tile), where k_mid's per-entry overhead
     // halves its update rate (measured 5.9e11 /s at Large against 1.3e12 - 1.6e12 /s for the denser rows of the weighted variant)
     const double R_mid_head = gram ? envd("UNIFRAC_B200_R_MID_SPARSE", (groups_expected ? 8e11 : 5.5e11) * cal.f_atom) : R_mid;
-    const double c_ent = envd("UNIFRAC_B200_MID_ENT_S", 3e-12);         // seconds per (mid entry, tile pair) visit of the join kernel
+    const double c_ent = envd("UNIFRAC_B200_MID_ENT_S", groups_expected ? 4e-12 : 3e-12);         // seconds per (mid entry, tile pair) visit of the join kernel
     const double head_s = gram ? n_tp * 512.0 / gram_Bps : Pd / R_head;  // seconds per head branch
     double c2_head, c2_mid;
     if (mid_ok) {
