@@ -44,7 +44,7 @@ SMEM_ATOMIC_PER_S, L2_RED_PER_S = 8.84 * SM_COUNT * SM_MAX_GHZ * 1e9, 1.94e11
 # the earlier captures of section 2, for runs with UNIFRAC_B200_MID_GROUPS=0 / --flags 512); not measured by this
 # run -- other workloads and kernels that changed since the capture report null
 TRAFFIC_SOURCE = "profiles/r02_summary.md section 0 (ncu --set full captures of the final kernels of the round, Large, seed 0)"
-NCU_TRAFFIC_BYTES = {"large": {"k_dense16": 80.5e9, "k_gram": 260.8e9, "k_midg": 219.1e9, "k_mid": 240.1e9, "k_zone": 307.1e9}}
+NCU_TRAFFIC_BYTES = {"large": {"k_dense16": 80.5e9, "k_gram": 260.8e9, "k_midg": 187.3e9, "k_mid": 240.1e9, "k_zone": 307.1e9}}
 
 WORKLOADS = {   # name -> (variants, precision)    BASELINE.json:7-11
     "tiny": ((0, 1), 1), "small": ((0, 1), 1), "medium": ((0,), 0), "emp": ((0, 1), 0), "large": ((0, 1), 0),
